@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py -- coupled RT + thermo-chemistry throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 512] [--variant b]
+
+Workload: BASELINE.json config 5 ("throughput sweep"): 512^3 coarse grid x 3 photon groups, lognormal density,
+4096 sources, random x and T, seeded background radiation (variant b, so that transport does not move zeros) --
+`workloads.make_config(5)`.  A "step" is one pass of the whole hot path (transport -> chemistry main -> chemistry
+tail -> diagnostics) over all cells.  `value` = cell-group updates per second, inputs resident in HBM.
+`e2e` = the same metric through the C-ABI with HOST buffers: every step uploads (U, x, T) from pinned host memory
+and reads (U, x, T) back.  N > 1 GPUs: independent replicas, one process per GPU.
+
+`--impl reference` times the fp64 CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell_group_updates_per_s"
+UNIT = "cell-group updates/s"
+ORACLE_SAMPLE_N = 128
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [s.strip() for s in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(n, steps, warmup, variant):
+    """The oracle as it stands on the host cores, on config 5 at n^3 (a bounded sample of the 512^3 workload)."""
+    import oracle as O
+    from workloads import make_config
+    w = make_config(5, n=n, variant=variant)
+    orc = O.Oracle(w)
+    if warmup:
+        orc.step(w.dt, warmup)
+    t0 = time.perf_counter()
+    rc, d = orc.step(w.dt, steps)
+    dt = time.perf_counter() - t0
+    units = n ** 3 * w.G * steps
+    return units / dt, dt, O.lib().orc_threads(), d
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = ORACLE_SAMPLE_N
+    steps, warm = max(1, min(args.steps, 5)), min(args.warmup, 1)
+    # per "step" of this arm: one oracle step on the n^3 sample; the whole run stays within a few minutes
+    val, secs, cores, d = time_oracle(n, steps, warm, args.variant)
+    sample = "config 5%s recipe at %d^3 x 3 groups (1/%d of the 512^3 cells), %d coupled steps, fp64 C oracle with OpenMP" % (
+        args.variant, n, (512 // n) ** 3, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE config 5%s sampled at %d^3 (oracle on host cores)" % (args.variant, n)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import paper_1508_07888_b200 as E
+    from workloads import make_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = local
+
+    n, K, W = args.n, args.steps, args.warmup
+    t0 = time.time()
+    w = make_config(5, n=n, variant=args.variant, seed=None if world == 1 else 150807893 + 1000 * rank)
+    G = w.G
+    ncell = n ** 3
+    log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
+
+    gpu = E.EmmaRT(w, device=dev)
+    dt = w.dt
+    units_per_step = ncell * G
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    # ---------------- device-resident: W warm-up steps, then exactly K timed steps
+    rc, _ = gpu.step(dt, W, diag=False)
+    assert rc == E.OK, gpu.last_error()
+    gpu.profile(True)
+    launches0 = gpu.kernel_launches()
+    clocks = ClockSampler(dev)
+    clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    rc, diag = gpu.step(dt, K, diag=True)
+    e1.record()
+    barrier()
+    clk = clocks.stop()
+    assert rc == E.OK, (rc, gpu.last_error())
+    ms = e0.elapsed_time(e1)
+    launches = gpu.kernel_launches() - launches0
+    prof = gpu.profile(False)
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = units_per_step * K * world / (ms * 1e-3)
+
+    # per-kernel roofline (algorithmic bytes of DESIGN.md section 7 / live CUDA-event durations)
+    peak, peak_src = measured_peaks()
+    alg = {"transport": 32.0 * ncell * G,                    # 16 B read + 16 B write per cell-group
+           "chem_main": (32.0 * G + 20.0) * ncell}           # U in/out + n0, x, e in + x, e out per cell
+    kern = {}
+    for k, (kms, cnt) in prof.items():
+        if cnt:
+            kern[k] = {"ms_per_launch": kms / cnt, "launches": int(cnt), "share": kms / ms}
+            if k in alg:
+                kern[k]["GBps"] = alg[k] / (kms / cnt * 1e-3) / 1e9
+                kern[k]["frac"] = kern[k]["GBps"] / peak
+    dominant = max((k for k in kern if k in alg), key=lambda k: kern[k]["share"])
+    roofline = {"kernel": dominant, "bound": "hbm", "achieved": kern[dominant]["GBps"], "peak": peak, "unit": "GB/s",
+                "frac": kern[dominant]["frac"], "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg[dominant]}
+    tfile = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tfile):
+        try:
+            roofline["traffic"] = json.load(open(tfile)).get(dominant)
+        except Exception:
+            pass
+
+    # ---------------- transport-only throughput (chemistry = 0), same grid, K steps
+    tr = None
+    if not args.skip_transport_only:
+        gpu.close()
+        gpu = None
+        torch.cuda.empty_cache()
+        g2 = E.EmmaRT(w, device=dev, chemistry=0)
+        g2.step(dt, W, diag=False)
+        barrier()
+        e0.record()
+        g2.step(dt, K, diag=False)
+        e1.record()
+        barrier()
+        ms_t = e0.elapsed_time(e1)
+        tr = {"value": units_per_step * K / (ms_t * 1e-3), "unit": UNIT, "ms_per_step": ms_t / K,
+              "GBps": 32.0 * units_per_step * K / (ms_t * 1e-3) / 1e9}
+        tr["frac"] = tr["GBps"] / peak
+        g2.close()
+        torch.cuda.empty_cache()
+        gpu = E.EmmaRT(w, device=dev)
+
+    # ---------------- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
+    Ke = max(1, min(K, args.e2e_steps))
+    hU = [torch.from_numpy(np.ascontiguousarray(w.U0[g])).pin_memory() if w.U0 is not None
+          else torch.zeros((ncell, 4), dtype=torch.float32).pin_memory() for g in range(G)]
+    hx = torch.from_numpy(w.x[0].copy()).pin_memory()
+    hT = torch.from_numpy(w.T[0].copy()).pin_memory()
+    h2d = sum(t.numel() * 4 for t in hU) + hx.numel() * 4 + hT.numel() * 4
+    d2h = h2d
+
+    def e2e_step():
+        for g in range(G):
+            assert gpu.write(E.FIELD_U, 0, g, hU[g]) == E.OK
+        assert gpu.write(E.FIELD_X, 0, 0, hx) == E.OK
+        assert gpu.write(E.FIELD_T, 0, 0, hT) == E.OK
+        rc, _ = gpu.step(dt, 1, diag=False)
+        assert rc == E.OK
+        for g in range(G):
+            assert gpu.read_into(E.FIELD_U, 0, g, hU[g]) == E.OK
+        assert gpu.read_into(E.FIELD_X, 0, 0, hx) == E.OK
+        assert gpu.read_into(E.FIELD_T, 0, 0, hT) == E.OK
+
+    e2e_step()                                                # warm-up (page-locks, first-touch)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": units_per_step * Ke * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "steps": Ke, "ms_per_step": 1e3 * e2e_s / Ke}
+    gpu.close()
+
+    # ---------------- oracle on the host cores, bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.skip_cpu_baseline:
+        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N, 3, 0, args.variant)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
+               "sample": "config 5%s recipe at %d^3 x 3 groups, 3 coupled steps from the initial state, fp64 C oracle, "
+                         "OpenMP on all host cores" % (args.variant, ORACLE_SAMPLE_N)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": "BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
+                                       "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)),
+                           "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
+                           "parallelism": "replicas" if world > 1 else "single"},
+                "roofline": roofline, "kernels": kern, "transport_only": tr, "e2e": e2e, "cpu_baseline": cpu,
+                "gpu_launches": int(launches), "clocks": clk,
+                "subcycles": {"mean_last_step": diag["subcycles_total"] / float(ncell), "max_last_step": diag["subcycles_max"],
+                              "deferred_last_step": diag["n_deferred"]}}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=512)
+    ap.add_argument("--variant", default="b", choices=["a", "b"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--skip-transport-only", action="store_true")
+    ap.add_argument("--skip-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

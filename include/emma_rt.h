@@ -1,0 +1,168 @@
+/* emma_rt.h -- C-ABI of the B200-native radiative-transfer + thermo-chemistry hot path of EMMA
+ * (arXiv 1508.07888).  Citations are /root/reference/PAPER.md line numbers; "A<n>" are the readings of the
+ * paper listed in DESIGN.md section 2.1.
+ *
+ * What one coupled step computes:
+ *   1. explicit M1 transport on the coarse level, per photon group: Levermore closure (Eq. 22-23, A1/A2),
+ *      Lax-Friedrichs/GLF interface flux (Eq. 32) with the reduced speed of light (A3), unsplit
+ *      conservative update (Eq. 30, A4), boundary conditions of PAPER.md:436 (A13);
+ *   2. CRTA injection of the coarse radiation into refined cells (A14);
+ *   3. hydrogen thermo-chemistry on every leaf cell, sub-cycled semi-implicitly (Eq. 43-48, A5-A9), with
+ *      point sources entering Eq. 43 (A12);
+ *   4. restriction of N, F, x, e to split cells (children mean, A14);
+ *   5. fp64 diagnostics (photon budget A15, min chemical time, sub-cycle counts).
+ *
+ * Conventions
+ *   - All pointers are HOST pointers unless the argument name ends in `_dev` or the call has an
+ *     `*_is_device` flag.  Plain C types only; no C++/torch types cross this boundary.
+ *   - Units are cgs: N [photons cm^-3], F [photons cm^-2 s^-1], n0 [cm^-3], T [K], e [erg cm^-3], Q [photons s^-1].
+ *   - Coarse cell id = ix + n*(iy + n*iz) (x fastest).  Cell id on refined level l = oct*8 + (ix + 2*iy + 4*iz);
+ *     arrays on level l have 8*n_octs[l-1] entries in oct order.  Entries of split cells are ignored on input and
+ *     hold the restricted (children-mean) value on output.
+ *   - Ownership: the handle owns host bookkeeping only.  Device memory is ONE caller-allocated arena
+ *     (`emma_rt_arena_bytes`), which must stay alive and untouched until `emma_rt_free`.  Host input arrays are
+ *     borrowed for the duration of the call.  The CUDA stream is borrowed.
+ *   - Errors: every entry point returns EMMA_RT_OK or a negative code; nothing throws, aborts or prints.
+ *     `emma_rt_last_error` gives a handle-owned message.  There is no CPU fallback: without a CUDA device
+ *     `emma_rt_init` returns EMMA_RT_ECUDA.
+ *   - Threading: one handle <-> one stream, not re-entrant.
+ *   - Sync: `emma_rt_step` only enqueues work unless `diag_last != NULL` (then it waits for the stream);
+ *     `emma_rt_read` / `emma_rt_write` with host buffers wait for the stream.
+ */
+#ifndef EMMA_RT_H
+#define EMMA_RT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define EMMA_RT_API __attribute__((visibility("default")))
+#else
+#define EMMA_RT_API
+#endif
+
+#define EMMA_RT_ABI_VERSION 1
+#define EMMA_RT_MAX_GROUPS 4
+#define EMMA_RT_MAX_LEVELS 4          /* refined levels above the base */
+#define EMMA_RT_MAX_SUBSTEPS 65535    /* accepted sub-steps per cell per step before EMMA_RT_ESUBCYCLE (A9) */
+
+typedef struct emma_rt emma_rt;      /* opaque */
+
+enum { EMMA_RT_OK = 0, EMMA_RT_EINVAL = -1, EMMA_RT_ENOMEM = -2, EMMA_RT_ECUDA = -3, EMMA_RT_ENONFINITE = -4,
+       EMMA_RT_ESTATE = -5, EMMA_RT_ECFL = -6, EMMA_RT_ESUBCYCLE = -7 };
+
+/* boundary conditions: periodic by nature; transmissive = ghost copies the cell;
+ * reflective = the same with the face-normal flux component inverted (A13) */
+enum { EMMA_RT_BC_PERIODIC = 0, EMMA_RT_BC_TRANSMISSIVE = 1, EMMA_RT_BC_REFLECTIVE = 2 };
+
+/* fields of emma_rt_read / emma_rt_write.  Element type and count per cell in brackets. */
+enum {
+  EMMA_RT_FIELD_U = 0,          /* [float x4] (N,Fx,Fy,Fz) of `group`; level 0 only             (read, write) */
+  EMMA_RT_FIELD_N = 1,          /* [float]    photon density of `group`; level 0 only           (read)        */
+  EMMA_RT_FIELD_F = 2,          /* [float x3] photon flux of `group`; level 0 only              (read)        */
+  EMMA_RT_FIELD_X = 3,          /* [float]    ionised fraction x                                (read, write) */
+  EMMA_RT_FIELD_T = 4,          /* [float]    temperature, T = e / (1.5 (1+x) n0 k_B) (A10)     (read, write: uses the x
+                                               currently stored, so write X before T)                          */
+  EMMA_RT_FIELD_E = 5,          /* [float]    internal energy density e                         (read)        */
+  EMMA_RT_FIELD_N0 = 6,         /* [float]    hydrogen number density n0                        (read, write) */
+  EMMA_RT_FIELD_SUBCYCLES = 7,  /* [uint32]   last step: accepted sub-steps | rejected (halved) attempts << 16,
+                                               each saturating at 65535; needs config.record_subcycles (read) */
+  EMMA_RT_FIELD_XNEUTRAL = 8    /* [float]    neutral fraction 1-x, kept to full relative precision (read)     */
+};
+
+typedef struct {
+  uint32_t struct_size;         /* sizeof(emma_rt_config), checked                                            */
+  uint32_t abi_version;         /* EMMA_RT_ABI_VERSION                                                        */
+  int32_t  n_coarse;            /* cells per side of the base level, 2^lc in the paper; >= 2    */
+  int32_t  n_groups;            /* 1..EMMA_RT_MAX_GROUPS                                  */
+  int32_t  bc[6];               /* -x,+x,-y,+y,-z,+z                                                          */
+  int32_t  otsa;                /* 1: alpha_A := alpha_B in Eq. 33/35, no recombination radiation */
+  int32_t  chemistry;           /* 0: transport + sources only (N += S dt); 1: Eq. 43-48                      */
+  int32_t  thermal;             /* 0: isothermal test mode (T held, Eq. 46-48 skipped, one sub-step); 1: full */
+  int32_t  record_subcycles;    /* 1: keep per-cell sub-cycle signatures of the last step (4 B/cell)          */
+  int32_t  max_halvings;        /* guard on the "divide by 2" retries of one sub-step          */
+  int32_t  device;              /* CUDA ordinal                                                               */
+  int64_t  max_source_cells;    /* capacity of the per-level source lists (0 -> 65536)                        */
+  double   box_len_cm;          /* L; dx = L / n_coarse                                                       */
+  double   c_red_cm_s;          /* reduced speed of light                                      */
+  double   sigma_N[EMMA_RT_MAX_GROUPS];   /* Eq. 29 [cm^2]                                                    */
+  double   sigma_E[EMMA_RT_MAX_GROUPS];   /* Eq. 37 [cm^2]                                                    */
+  double   E_mean[EMMA_RT_MAX_GROUPS];    /* Eq. 38 [erg]                                                     */
+  double   e_tol;               /* 0.1                                                         */
+  void*    stream;              /* cudaStream_t of the caller (e.g. torch's current stream); 0 = default      */
+} emma_rt_config;
+
+typedef struct {                /* static AMR description (host pointers, borrowed during init only)          */
+  int32_t  n_levels;            /* refined levels above the base: 0 = uniform grid; <= EMMA_RT_MAX_LEVELS     */
+  const int64_t* n_octs;        /* [n_levels]                                                                 */
+  const int64_t* const* parent; /* [n_levels][n_octs[l]] -> id of the split cell on the level below           */
+} emma_rt_amr;
+
+typedef struct {                /* initial state (host pointers, borrowed during init only)                   */
+  const float* const* U0;       /* [n_groups] -> n^3 x (N,Fx,Fy,Fz); NULL (or a NULL entry) => zeros          */
+  const float* const* n0;       /* [n_levels+1] hydrogen number density                                       */
+  const float* const* x;        /* [n_levels+1] ionised fraction in [0,1]                                     */
+  const float* const* T;        /* [n_levels+1] temperature [K]; the library stores the energy (A10)          */
+} emma_rt_fields;
+
+typedef struct {                /* diagnostics of the LAST step of an emma_rt_step call (A15), plus totals     */
+  double  photons_total;        /* sum over leaves of sum_g N_g dV after the step                             */
+  double  photons_injected;     /* sum S_g dtau dV  (= sum Q dt)                                              */
+  double  photons_absorbed;     /* sum c sigma_g (1-x^p) n0 dtau N_g^{p+1} dV, the sink of Eq. 43             */
+  double  photons_recomb_emitted; /* (alpha_A-alpha_B) x^2 n0^2 dtau dV into group 1; 0 under OTSA (A6)       */
+  double  photons_outflow;      /* net GLF flux through non-periodic box faces x dx^2 dt                      */
+  double  dtau_min;             /* min over leaves and sub-steps of the first guess e/abs(H-Lambda) */
+  int64_t subcycles_total;      /* accepted sub-steps, all leaves                                             */
+  int64_t subcycles_max;        /* max accepted sub-steps of one cell                                         */
+  int64_t halvings_total;       /* rejected attempts                                                          */
+  int64_t n_nonfinite;          /* cells holding a non-finite N, F, x or e after the step                     */
+  int64_t n_deferred;           /* leaves that needed more than the single fast-path attempt                  */
+  double  t_sim;                /* simulated time since init [s]                                              */
+} emma_rt_diag;
+
+/* Bytes of device memory the arena must hold for this problem; 0 if the arguments are invalid. */
+EMMA_RT_API size_t emma_rt_arena_bytes(const emma_rt_config* cfg, const emma_rt_amr* amr);
+
+/* Validate, lay out the arena (256-byte aligned device pointer `arena_dev`, >= emma_rt_arena_bytes), upload the
+ * fields, compute e from T (A10) and the restricted values of split cells.  `amr` may be NULL (uniform grid). */
+EMMA_RT_API int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, const emma_rt_fields* fields,
+                 void* arena_dev, size_t arena_bytes);
+
+/* Replace the point-source list.  pos_box: [n_src][3] in [0,1)^3 box units; Q: [n_src][n_groups] photons/s (fp64:
+ * Q ~ 1e48 overflows fp32).  Each source goes to the LEAF cell containing it, S_g = Q_g / dV_leaf; sources in the
+ * same cell add (A12).  Invalid position / negative or non-finite Q -> EMMA_RT_EINVAL and the list is unchanged. */
+EMMA_RT_API int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos_box, const double* Q);
+
+/* courant * dx / (3 c_red): the largest stable step is courant = 1 (A4). */
+EMMA_RT_API double emma_rt_dt_cfl(const emma_rt* h, double courant);
+
+/* Advance n_steps coupled steps of size dt.  dt > dx/(3 c_red) -> EMMA_RT_ECFL, state untouched.
+ * diag_last == NULL: asynchronous.  Otherwise waits and fills *diag_last; returns EMMA_RT_ENONFINITE /
+ * EMMA_RT_ESUBCYCLE if the last step saw them (the step still completed). */
+EMMA_RT_API int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last);
+
+/* Copy a field of one level (and group) out of / into the library.  dst/src holds exactly n_cells(level) elements
+ * of the field's type; `bytes` must match.  *_is_device != 0: the pointer is a device pointer on the same device
+ * and the copy is stream-ordered; otherwise it is a host pointer and the call waits for the stream. */
+EMMA_RT_API int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device);
+EMMA_RT_API int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const void* src, size_t bytes, int32_t src_is_device);
+
+EMMA_RT_API int64_t emma_rt_level_cells(const emma_rt* h, int32_t level);      /* n^3 or 8*n_octs; -1 if out of range       */
+EMMA_RT_API int64_t emma_rt_kernel_launches(const emma_rt* h);                 /* kernels launched by this handle so far     */
+/* Per-kernel device timing.  Waits for the stream, returns in ms_out / launches_out (each EMMA_RT_K_COUNT long,
+ * nullable) the summed CUDA-event durations and launch counts of the emma_rt_step kernels recorded since the last
+ * call, clears them, and switches recording on (enable != 0) or off for the steps that follow.  Off by default. */
+enum { EMMA_RT_K_TRANSPORT = 0, EMMA_RT_K_CHEM_MAIN = 1, EMMA_RT_K_CHEM_TAIL = 2, EMMA_RT_K_CHEM_REFINED = 3,
+       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_COUNT = 6 };
+EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out);
+EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */
+EMMA_RT_API void emma_rt_free(emma_rt* h);                                     /* does not free the arena                    */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

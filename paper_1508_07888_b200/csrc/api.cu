@@ -1,0 +1,523 @@
+// api.cu -- host side of the C-ABI (include/emma_rt.h): validation, arena layout, AMR index arrays, sources,
+// the step loop (kernel sequence of SURVEY.md section 3(c)) and field I/O.  No compute happens on the host; without
+// a CUDA device every entry point that needs one fails with EMMA_RT_ECUDA.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <unordered_map>
+#include <vector>
+
+#include "emma_rt_internal.cuh"
+
+using namespace emma;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+constexpr int PART_SLOTS = 24576;
+constexpr int TRANSPORT_MAX_BLOCKS = 8192;
+constexpr double E_HI_ERG = 13.6 * 1.602176634e-12;          // "E_13.6" of PAPER.md:266
+
+size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+  size_t U[2];
+  size_t n0[MAXL + 1], xs[MAXL + 1], eps[MAXL + 1], subc[MAXL + 1];
+  size_t refined0;
+  size_t parent[MAXL + 1], anc0[MAXL + 1], child[MAXL + 1], Ut[MAXL + 1];
+  size_t srcmask[MAXL + 1], src_cell[MAXL + 1], src_S[MAXL + 1];
+  size_t queue, qcount, parts, diag;
+  size_t total;
+};
+
+struct Shape {
+  int n, G, nl;
+  long long ncell[MAXL + 1], nocts[MAXL + 1];
+  long long max_src;
+  bool record, need_queue;
+};
+
+bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
+{
+  if (!c || c->struct_size != sizeof(emma_rt_config) || c->abi_version != EMMA_RT_ABI_VERSION) return false;
+  if (c->n_coarse < 2 || c->n_coarse > 1290 || c->n_groups < 1 || c->n_groups > MAXG) return false;
+  for (int f = 0; f < 6; f++)
+    if (c->bc[f] < 0 || c->bc[f] > 2) return false;
+  for (int d = 0; d < 3; d++)                                   // periodic faces come in pairs
+    if ((c->bc[2 * d] == EMMA_RT_BC_PERIODIC) != (c->bc[2 * d + 1] == EMMA_RT_BC_PERIODIC)) return false;
+  if (!(c->box_len_cm > 0) || !(c->c_red_cm_s > 0) || !(c->e_tol > 0) || c->max_halvings < 0) return false;
+  for (int g = 0; g < c->n_groups; g++)
+    if (!(c->sigma_N[g] >= 0) || !(c->sigma_E[g] >= 0) || !(c->E_mean[g] >= 0)) return false;
+  s.n = c->n_coarse; s.G = c->n_groups;
+  s.nl = a ? a->n_levels : 0;
+  if (s.nl < 0 || s.nl > MAXL) return false;
+  s.ncell[0] = (long long)s.n * s.n * s.n; s.nocts[0] = 0;
+  for (int l = 1; l <= s.nl; l++) {
+    if (!a->n_octs || a->n_octs[l - 1] < 0 || a->n_octs[l - 1] > s.ncell[l - 1] || 8 * a->n_octs[l - 1] > 2000000000LL)
+      return false;
+    s.nocts[l] = a->n_octs[l - 1];
+    s.ncell[l] = 8 * s.nocts[l];
+  }
+  s.max_src = c->max_source_cells > 0 ? c->max_source_cells : 65536;
+  s.record = c->record_subcycles != 0;
+  s.need_queue = c->chemistry != 0 && c->thermal != 0;
+  return true;
+}
+
+void make_layout(const Shape& s, Layout& L)
+{
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + (bytes ? bytes : 1)); return o; };
+  memset(&L, 0, sizeof L);
+  for (int b = 0; b < 2; b++) L.U[b] = take((size_t)s.G * s.ncell[0] * sizeof(float4));
+  for (int l = 0; l <= s.nl; l++) {
+    L.n0[l] = take(s.ncell[l] * 4); L.xs[l] = take(s.ncell[l] * 4); L.eps[l] = take(s.ncell[l] * 4);
+    L.subc[l] = s.record ? take(s.ncell[l] * 4) : 0;
+    const size_t words = (size_t)(s.ncell[l] + 31) / 32;
+    L.srcmask[l] = take(words * 4);
+    L.src_cell[l] = take(s.max_src * 4);
+    L.src_S[l] = take(s.max_src * s.G * 4);
+    if (l >= 1) {
+      L.parent[l] = take(s.nocts[l] * 4);
+      L.anc0[l] = take(s.nocts[l] * 4);
+      if (l < s.nl) L.child[l] = take(s.ncell[l] * 4);
+      if (l >= 2) L.Ut[l] = take((size_t)s.G * s.nocts[l] * sizeof(float4));
+    }
+  }
+  L.refined0 = s.nl > 0 ? take((size_t)(s.ncell[0] + 31) / 32 * 4) : 0;
+  L.queue = s.need_queue ? take(s.ncell[0] * 4) : 0;
+  L.qcount = take(256);
+  L.parts = take((size_t)PART_SLOTS * sizeof(Partial));
+  L.diag = take(sizeof(DiagDev));
+  L.total = off;
+}
+
+}  // namespace
+
+struct emma_rt {
+  emma_rt_config cfg;
+  Shape sh;
+  Layout lay;
+  char* arena;
+  cudaStream_t st;
+  int sm_count;
+  int cur;                                     // U[cur] holds the current radiation field
+  LevelDev lv[MAXL + 1];
+  std::unordered_map<long long, int> child_of[MAXL + 1];   // split cell -> oct on the level above (host copy)
+  std::vector<int> anc0_h[MAXL + 1];
+  double dx, t_sim;
+  long long launches;
+  DiagDev* diag_pinned;
+  Profiler prof;
+  char err[256];
+
+  float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
+  Partial* parts() const { return (Partial*)(arena + lay.parts); }
+  unsigned int* qcount() const { return (unsigned int*)(arena + lay.qcount); }
+  DiagDev* diag() const { return (DiagDev*)(arena + lay.diag); }
+};
+
+namespace {
+
+int fail(emma_rt* h, int code, const char* fmt, ...)
+{
+  if (h) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(h->err, sizeof h->err, fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+#define CUDA_TRY(h, call)                                                                       \
+  do {                                                                                          \
+    cudaError_t e__ = (call);                                                                   \
+    if (e__ != cudaSuccess) return fail(h, EMMA_RT_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
+  } while (0)
+
+size_t field_elem_bytes(int field)
+{
+  switch (field) {
+    case EMMA_RT_FIELD_U: return 16;
+    case EMMA_RT_FIELD_F: return 12;
+    default: return 4;
+  }
+}
+
+// host -> library, one field of one level, through the scratch (= the inactive radiation buffer), chunked
+int upload_field(emma_rt* h, int field, int level, int group, const void* src, bool src_is_device)
+{
+  const long long nc = h->sh.ncell[level];
+  const size_t eb = field_elem_bytes(field);
+  float4* Ug = (field == EMMA_RT_FIELD_U) ? h->U(h->cur) + (size_t)group * nc : nullptr;
+  if (src_is_device) {
+    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, 0, nc, src, h->st);
+    CUDA_TRY(h, cudaGetLastError());
+    return EMMA_RT_OK;
+  }
+  char* scratch = (char*)h->U(1 - h->cur);
+  const size_t cap = (size_t)h->sh.G * h->sh.ncell[0] * sizeof(float4);
+  const long long chunk = (long long)(cap / eb);
+  for (long long off = 0; off < nc; off += chunk) {
+    const long long cnt = std::min(chunk, nc - off);
+    CUDA_TRY(h, cudaMemcpyAsync(scratch, (const char*)src + (size_t)off * eb, (size_t)cnt * eb, cudaMemcpyHostToDevice, h->st));
+    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, off, cnt, scratch, h->st);
+    CUDA_TRY(h, cudaGetLastError());
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  return EMMA_RT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t emma_rt_arena_bytes(const emma_rt_config* cfg, const emma_rt_amr* amr)
+{
+  Shape s;
+  if (!make_shape(cfg, amr, s)) return 0;
+  Layout L;
+  make_layout(s, L);
+  return L.total;
+}
+
+int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, const emma_rt_fields* fields,
+                 void* arena_dev, size_t arena_bytes)
+{
+  if (!out) return EMMA_RT_EINVAL;
+  *out = nullptr;
+  Shape s;
+  if (!make_shape(cfg, amr, s) || !fields || !fields->n0 || !fields->x || !fields->T) return EMMA_RT_EINVAL;
+  for (int l = 0; l <= s.nl; l++)
+    if (!fields->n0[l] || !fields->x[l] || !fields->T[l]) return EMMA_RT_EINVAL;
+  if (!arena_dev || ((uintptr_t)arena_dev % ALIGN) != 0) return EMMA_RT_EINVAL;
+  emma_rt* h = new (std::nothrow) emma_rt();
+  if (!h) return EMMA_RT_ENOMEM;
+  h->cfg = *cfg; h->sh = s; h->err[0] = 0;
+  make_layout(s, h->lay);
+  h->arena = (char*)arena_dev;
+  h->st = (cudaStream_t)cfg->stream;
+  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr;
+  h->prof.st = h->st;
+  h->dx = cfg->box_len_cm / s.n;
+  *out = h;                                    // returned even on failure so the caller can read last_error
+  if (arena_bytes < h->lay.total) return fail(h, EMMA_RT_ENOMEM, "arena too small: %zu < %zu", arena_bytes, h->lay.total);
+  CUDA_TRY(h, cudaSetDevice(cfg->device));
+  cudaDeviceProp prop;
+  CUDA_TRY(h, cudaGetDeviceProperties(&prop, cfg->device));
+  h->sm_count = prop.multiProcessorCount;
+  CUDA_TRY(h, cudaMallocHost((void**)&h->diag_pinned, sizeof(DiagDev)));
+
+  // ---- AMR index arrays (a-0: per-level oct arrays with parent / coarse-ancestor / child indices)
+  std::vector<std::vector<int>> parent_h(s.nl + 1), child_h(s.nl + 1);
+  for (int l = 1; l <= s.nl; l++) {
+    parent_h[l].resize(s.nocts[l]);
+    h->anc0_h[l].resize(s.nocts[l]);
+    for (long long o = 0; o < s.nocts[l]; o++) {
+      const long long p = amr->parent[l - 1][o];
+      if (p < 0 || p >= s.ncell[l - 1]) return fail(h, EMMA_RT_EINVAL, "parent[%d][%lld] out of range", l - 1, o);
+      if (!h->child_of[l - 1].emplace(p, (int)o).second) return fail(h, EMMA_RT_EINVAL, "cell split twice on level %d", l - 1);
+      parent_h[l][o] = (int)p;
+      h->anc0_h[l][o] = (l == 1) ? (int)p : h->anc0_h[l - 1][p >> 3];
+    }
+  }
+  CUDA_TRY(h, cudaMemsetAsync(h->arena, 0, h->lay.total, h->st));
+  for (int l = 0; l <= s.nl; l++) {
+    LevelDev& L = h->lv[l];
+    memset(&L, 0, sizeof L);
+    L.ncell = s.ncell[l]; L.nocts = s.nocts[l];
+    L.n0 = (float*)(h->arena + h->lay.n0[l]); L.xs = (float*)(h->arena + h->lay.xs[l]); L.eps = (float*)(h->arena + h->lay.eps[l]);
+    L.subc = s.record ? (unsigned int*)(h->arena + h->lay.subc[l]) : nullptr;
+    L.srcmask = (unsigned int*)(h->arena + h->lay.srcmask[l]);
+    L.src_cell = (int*)(h->arena + h->lay.src_cell[l]);
+    L.src_S = (float*)(h->arena + h->lay.src_S[l]);
+    L.n_src = 0;
+    const double dxl = h->dx / (double)(1 << l);
+    L.dV = dxl * dxl * dxl;
+    if (l >= 1) {
+      L.parent = (int*)(h->arena + h->lay.parent[l]);
+      L.anc0 = (int*)(h->arena + h->lay.anc0[l]);
+      CUDA_TRY(h, cudaMemcpyAsync(L.parent, parent_h[l].data(), s.nocts[l] * 4, cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(L.anc0, h->anc0_h[l].data(), s.nocts[l] * 4, cudaMemcpyHostToDevice, h->st));
+      if (l < s.nl) {
+        L.child = (int*)(h->arena + h->lay.child[l]);
+        child_h[l].assign(s.ncell[l], -1);
+        for (auto& kv : h->child_of[l]) child_h[l][kv.first] = kv.second;
+        CUDA_TRY(h, cudaMemcpyAsync(L.child, child_h[l].data(), s.ncell[l] * 4, cudaMemcpyHostToDevice, h->st));
+      }
+      if (l >= 2) L.Ut = (float4*)(h->arena + h->lay.Ut[l]);
+    }
+  }
+  std::vector<unsigned int> refined_h;
+  if (s.nl > 0) {
+    h->lv[0].refined = (unsigned int*)(h->arena + h->lay.refined0);
+    refined_h.assign((size_t)(s.ncell[0] + 31) / 32, 0u);
+    for (auto& kv : h->child_of[0]) refined_h[kv.first >> 5] |= 1u << (kv.first & 31);
+    CUDA_TRY(h, cudaMemcpyAsync(h->lv[0].refined, refined_h.data(), refined_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));   // host staging vectors go out of scope below
+
+  // ---- fields: N0, X, T (-> eps, A10) per level; U0 per group; then the children means of split cells (A14)
+  int rc;
+  for (int l = 0; l <= s.nl; l++) {
+    if ((rc = upload_field(h, EMMA_RT_FIELD_N0, l, 0, fields->n0[l], false)) != EMMA_RT_OK) return rc;
+    if ((rc = upload_field(h, EMMA_RT_FIELD_X, l, 0, fields->x[l], false)) != EMMA_RT_OK) return rc;
+    if ((rc = upload_field(h, EMMA_RT_FIELD_T, l, 0, fields->T[l], false)) != EMMA_RT_OK) return rc;
+  }
+  if (fields->U0)
+    for (int g = 0; g < s.G; g++)
+      if (fields->U0[g] && (rc = upload_field(h, EMMA_RT_FIELD_U, 0, g, fields->U0[g], false)) != EMMA_RT_OK) return rc;
+  for (int l = s.nl; l >= 1; l--) h->launches += launch_restrict_init(h->lv, l, h->st);
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  return EMMA_RT_OK;
+}
+
+int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos, const double* Q)
+{
+  if (!h) return EMMA_RT_EINVAL;
+  const Shape& s = h->sh;
+  if (n_src < 0 || (n_src > 0 && (!pos || !Q))) return fail(h, EMMA_RT_EINVAL, "bad source arguments");
+  for (int64_t i = 0; i < n_src; i++) {
+    for (int k = 0; k < 3; k++)
+      if (!(pos[3 * i + k] >= 0.0 && pos[3 * i + k] < 1.0)) return fail(h, EMMA_RT_EINVAL, "source %lld outside the box", (long long)i);
+    for (int g = 0; g < s.G; g++)
+      if (!(Q[i * s.G + g] >= 0.0) || std::isinf(Q[i * s.G + g])) return fail(h, EMMA_RT_EINVAL, "source %lld: bad Q", (long long)i);
+  }
+  // A12: NGP into the leaf containing the position; S_g = Q_g / dV_leaf; same-cell sources add (in fp64)
+  std::map<long long, std::vector<double>> per_level[MAXL + 1];
+  for (int64_t i = 0; i < n_src; i++) {
+    const double fx = pos[3 * i] * s.n, fy = pos[3 * i + 1] * s.n, fz = pos[3 * i + 2] * s.n;
+    int ix = std::min((int)std::floor(fx), s.n - 1), iy = std::min((int)std::floor(fy), s.n - 1), iz = std::min((int)std::floor(fz), s.n - 1);
+    double ox = fx - ix, oy = fy - iy, oz = fz - iz;
+    int lvl = 0;
+    long long cell = ix + (long long)s.n * (iy + (long long)s.n * iz);
+    if (h->cfg.chemistry) {                      // chemistry off: sources are folded to the coarse cell (A9)
+      while (lvl < s.nl) {
+        auto it = h->child_of[lvl].find(cell);
+        if (it == h->child_of[lvl].end()) break;
+        const int cx = ox >= 0.5, cy = oy >= 0.5, cz = oz >= 0.5;
+        ox = 2 * ox - cx; oy = 2 * oy - cy; oz = 2 * oz - cz;
+        cell = 8LL * it->second + (cx + 2 * cy + 4 * cz);
+        lvl++;
+      }
+    }
+    auto& v = per_level[lvl][cell];
+    if (v.empty()) v.assign(s.G, 0.0);
+    for (int g = 0; g < s.G; g++) v[g] += Q[i * s.G + g] / h->lv[lvl].dV;
+  }
+  for (int l = 0; l <= s.nl; l++)
+    if ((long long)per_level[l].size() > s.max_src) return fail(h, EMMA_RT_EINVAL, "more than max_source_cells source cells");
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  for (int l = 0; l <= s.nl; l++) {
+    LevelDev& L = h->lv[l];
+    std::vector<int> cells;
+    std::vector<float> S;
+    for (auto& kv : per_level[l]) {
+      cells.push_back((int)kv.first);
+      for (int g = 0; g < s.G; g++) S.push_back((float)kv.second[g]);
+    }
+    CUDA_TRY(h, cudaMemsetAsync(L.srcmask, 0, (size_t)(L.ncell + 31) / 32 * 4, h->st));
+    L.n_src = (int)cells.size();
+    if (L.n_src) {
+      CUDA_TRY(h, cudaMemcpyAsync(L.src_cell, cells.data(), cells.size() * 4, cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(L.src_S, S.data(), S.size() * 4, cudaMemcpyHostToDevice, h->st));
+      h->launches += launch_set_bits(L.srcmask, L.src_cell, L.n_src, h->st);
+      CUDA_TRY(h, cudaGetLastError());
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  }
+  return EMMA_RT_OK;
+}
+
+double emma_rt_dt_cfl(const emma_rt* h, double courant)
+{
+  return h ? courant * h->dx / (3.0 * h->cfg.c_red_cm_s) : 0.0;
+}
+
+int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
+{
+  if (!h) return EMMA_RT_EINVAL;
+  if (!(dt > 0.0) || n_steps < 0) return fail(h, EMMA_RT_EINVAL, "dt must be > 0 and n_steps >= 0");
+  const Shape& s = h->sh;
+  const double c = h->cfg.c_red_cm_s;
+  if (3.0 * c * dt > h->dx * (1.0 + 1e-12)) return fail(h, EMMA_RT_ECFL, "dt = %g exceeds dx/(3 c) = %g (A4)", dt, h->dx / (3 * c));
+
+  TransportParams tp;
+  tp.n = s.n; tp.G = s.G;
+  for (int f = 0; f < 6; f++) tp.bc[f] = h->cfg.bc[f];
+  tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
+  {
+    // z chunks: enough CTAs for ~8 per SM (two waves at 2 CTAs/SM x 4), chunks of at least 8 planes
+    const int per = tp.tiles_x * tp.tiles_y * s.G;
+    int nzc = (h->sm_count * 8 + per - 1) / per;
+    nzc = std::max(1, std::min(nzc, std::max(1, s.n / 8)));
+    while (nzc > 1 && (long long)per * nzc > TRANSPORT_MAX_BLOCKS) nzc--;
+    tp.zchunk = (s.n + nzc - 1) / nzc;
+    tp.nzc = (s.n + tp.zchunk - 1) / tp.zchunk;
+    if ((long long)per * tp.nzc > TRANSPORT_MAX_BLOCKS) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+  }
+  tp.want_total = h->cfg.chemistry ? 0 : 1;
+  tp.nu = (float)(c * dt / h->dx);
+  tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
+  tp.c1 = (float)(0.5 * (c * dt / h->dx));
+  tp.dV = h->lv[0].dV;
+
+  ChemParams cp;
+  memset(&cp, 0, sizeof cp);
+  cp.G = s.G; cp.otsa = h->cfg.otsa; cp.thermal = h->cfg.thermal; cp.max_halvings = h->cfg.max_halvings;
+  cp.record = s.record ? 1 : 0;
+  cp.dt = (float)dt; cp.e_tol = (float)h->cfg.e_tol;
+  for (int g = 0; g < s.G; g++) {
+    cp.csig[g] = (float)(c * h->cfg.sigma_N[g]);
+    cp.csigE[g] = (float)(c * (h->cfg.sigma_E[g] * h->cfg.E_mean[g] - h->cfg.sigma_N[g] * E_HI_ERG));
+  }
+
+  for (int step = 0; step < n_steps; step++) {
+    int off = 0, np = 0;
+    Partial* P = h->parts();
+    // 1. coarse transport, old buffer -> new buffer (Jacobi)
+    h->prof.begin(EMMA_RT_K_TRANSPORT);
+    h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
+    h->prof.end();
+    off += np;
+    h->cur = 1 - h->cur;
+    float4* U = h->U(h->cur);
+    if (h->cfg.chemistry) {
+      // 2-4. CRTA: deepest refined level first (inject -> leaf chemistry -> restrict), then the unrefined coarse cells
+      for (int l = s.nl; l >= 1; l--) {
+        h->prof.begin(EMMA_RT_K_CHEM_REFINED);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->st);
+        h->prof.end();
+        off += np;
+      }
+      h->launches += launch_chem_level0(cp, h->lv[0], U, s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
+                                        P + off, &np, h->sm_count, h->st, &h->prof);
+      off += np;
+    } else {
+      h->prof.begin(EMMA_RT_K_OTHER);
+      h->launches += launch_inject_sources(h->lv[0], s.G, (float)dt, U, s.ncell[0], P + off, &np, h->st);
+      h->prof.end();
+      off += np;
+    }
+    h->t_sim += dt;
+    // 5. diagnostics
+    h->prof.begin(EMMA_RT_K_FINALIZE);
+    h->launches += launch_finalize(P, off, h->diag(), h->qcount(), h->t_sim, h->st);
+    h->prof.end();
+  }
+  CUDA_TRY(h, cudaGetLastError());
+  if (!diag_last) return EMMA_RT_OK;
+  if (n_steps == 0) {                          // state query: photons currently in the box
+    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+    memset(diag_last, 0, sizeof *diag_last);
+    diag_last->t_sim = h->t_sim;
+    diag_last->dtau_min = INFINITY;
+    std::vector<float> N((size_t)s.ncell[0]);
+    double tot = 0;
+    for (int g = 0; g < s.G; g++) {
+      int rc = emma_rt_read(h, EMMA_RT_FIELD_N, 0, g, N.data(), N.size() * 4, 0);
+      if (rc != EMMA_RT_OK) return rc;
+      for (float v : N) tot += (double)v;
+    }
+    diag_last->photons_total = tot * h->lv[0].dV;
+    return EMMA_RT_OK;
+  }
+  CUDA_TRY(h, cudaMemcpyAsync(h->diag_pinned, h->diag(), sizeof(DiagDev), cudaMemcpyDeviceToHost, h->st));
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  *diag_last = h->diag_pinned->d;
+  if (h->diag_pinned->d.n_nonfinite > 0) return fail(h, EMMA_RT_ENONFINITE, "%lld non-finite cells", (long long)h->diag_pinned->d.n_nonfinite);
+  if (h->diag_pinned->err_last & 1u) return fail(h, EMMA_RT_ESUBCYCLE, "sub-cycle guard hit (max_halvings or %d sub-steps)", EMMA_RT_MAX_SUBSTEPS);
+  return EMMA_RT_OK;
+}
+
+int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
+{
+  if (!h || !dst) return EMMA_RT_EINVAL;
+  const Shape& s = h->sh;
+  if (level < 0 || level > s.nl) return fail(h, EMMA_RT_EINVAL, "level out of range");
+  if (field < EMMA_RT_FIELD_U || field > EMMA_RT_FIELD_XNEUTRAL) return fail(h, EMMA_RT_EINVAL, "unknown field");
+  const bool rad = field == EMMA_RT_FIELD_U || field == EMMA_RT_FIELD_N || field == EMMA_RT_FIELD_F;
+  if (rad && (level != 0 || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "radiation fields live on level 0, group in range");
+  if (field == EMMA_RT_FIELD_SUBCYCLES && !s.record) return fail(h, EMMA_RT_ESTATE, "record_subcycles was not set");
+  const long long nc = s.ncell[level];
+  const size_t eb = field_elem_bytes(field);
+  if (bytes != (size_t)nc * eb) return fail(h, EMMA_RT_EINVAL, "size mismatch: %zu != %zu", bytes, (size_t)nc * eb);
+  const float4* Ug = rad ? h->U(h->cur) + (size_t)group * nc : nullptr;
+  const float cr = (float)h->cfg.c_red_cm_s;
+  if (dst_is_device) {
+    h->launches += launch_export(field, h->lv[level], Ug, cr, 0, nc, dst, h->st);
+    CUDA_TRY(h, cudaGetLastError());
+    return EMMA_RT_OK;
+  }
+  char* scratch = (char*)h->U(1 - h->cur);
+  const size_t cap = (size_t)s.G * s.ncell[0] * sizeof(float4);
+  const long long chunk = (long long)(cap / eb);
+  for (long long off = 0; off < nc; off += chunk) {
+    const long long cnt = std::min(chunk, nc - off);
+    h->launches += launch_export(field, h->lv[level], Ug, cr, off, cnt, scratch, h->st);
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync((char*)dst + (size_t)off * eb, scratch, (size_t)cnt * eb, cudaMemcpyDeviceToHost, h->st));
+    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  }
+  return EMMA_RT_OK;
+}
+
+int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const void* src, size_t bytes, int32_t src_is_device)
+{
+  if (!h || !src) return EMMA_RT_EINVAL;
+  const Shape& s = h->sh;
+  if (level < 0 || level > s.nl) return fail(h, EMMA_RT_EINVAL, "level out of range");
+  if (field != EMMA_RT_FIELD_U && field != EMMA_RT_FIELD_X && field != EMMA_RT_FIELD_T && field != EMMA_RT_FIELD_N0)
+    return fail(h, EMMA_RT_EINVAL, "field is not writable");
+  if (field == EMMA_RT_FIELD_U && (level != 0 || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "U lives on level 0, group in range");
+  const size_t eb = field_elem_bytes(field);
+  if (bytes != (size_t)s.ncell[level] * eb) return fail(h, EMMA_RT_EINVAL, "size mismatch");
+  return upload_field(h, field, level, group, src, src_is_device != 0);
+}
+
+int64_t emma_rt_level_cells(const emma_rt* h, int32_t level)
+{
+  if (!h || level < 0 || level > h->sh.nl) return -1;
+  return h->sh.ncell[level];
+}
+
+int64_t emma_rt_kernel_launches(const emma_rt* h) { return h ? h->launches : 0; }
+
+int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out)
+{
+  if (!h) return EMMA_RT_EINVAL;
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  double ms[EMMA_RT_K_COUNT] = {0};
+  int64_t cnt[EMMA_RT_K_COUNT] = {0};
+  for (const Profiler::Span& sp : h->prof.spans) {
+    float t = 0.f;
+    CUDA_TRY(h, cudaEventElapsedTime(&t, sp.a, sp.b));
+    ms[sp.kind] += t;
+    cnt[sp.kind]++;
+  }
+  for (int k = 0; k < EMMA_RT_K_COUNT; k++) {
+    if (ms_out) ms_out[k] = ms[k];
+    if (launches_out) launches_out[k] = cnt[k];
+  }
+  h->prof.reset();
+  h->prof.on = enable != 0;
+  return EMMA_RT_OK;
+}
+
+const char* emma_rt_last_error(const emma_rt* h) { return h ? h->err : ""; }
+
+void emma_rt_free(emma_rt* h)
+{
+  if (!h) return;
+  if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
+  for (cudaEvent_t e : h->prof.pool) cudaEventDestroy(e);
+  delete h;
+}
+
+}  // extern "C"

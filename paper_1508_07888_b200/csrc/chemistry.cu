@@ -1,0 +1,570 @@
+// chemistry.cu -- sub-cycled semi-implicit hydrogen thermo-chemistry.
+//
+// Eq. 43 (N), 44 (F), 45 (x), 46-48 (e), "in that order ... new information immediately used"
+// (PAPER.md:306), chemical step dtau first guessed as e/(H - Lambda) and halved until e varies by <= 10 %
+// (reading A9).  Point sources S = Q/dV enter Eq. 43 in every sub-step (A12).  CRTA
+// (A14): leaves of refined cells start from the coarse N*, F*; split cells take the children mean.
+//
+// fp32 arithmetic, arranged so that nothing cancels:
+//   * both x and y = 1-x are carried; Eq. 45 is evaluated as  y' = (y + r)/(1 + dtau G)  [its printed form] and
+//     x' = (x + dtau G - r)/(1 + dtau G), r = alpha x^2 n0 dtau, G = beta x n0 + c sum sigma_i N_i'; whichever of
+//     x', y' is <= 1/2 is kept and the other derived from it;
+//   * energies are per hydrogen atom (eps = e/n0), so tiny n0^2 Lambda products never reach the denormal range;
+//   * T-dependent rates are evaluated once per sub-step (state p) through lg2/ex2 (MUFU) and reused by its retries.
+//
+// Work distribution (north_star item 3): the level-0 pass `chem_main_kernel` is HBM-bound and gives every cell
+// exactly one attempt with dtau = dt; cells whose first guess is shorter than dt, or whose attempt breaks the 10 %
+// rule, are appended to a queue with one warp-aggregated atomic and left untouched.  `chem_tail_kernel` then runs
+// persistent warps over that (compacted) queue: each lane owns one queued cell, advances it one accepted sub-step
+// per loop trip and refills from the queue as soon as its cell is done, so lanes stay busy while any work is left.
+#include "emma_rt_internal.cuh"
+
+namespace emma {
+
+namespace {
+
+constexpr float KB15 = 1.5f * 1.380649e-16f;          // (3/2) k_B  [erg/K]   (A10: e = (3/2)(1+x) n0 k_B T)
+constexpr float LOG2E = 1.4426950408889634f;
+constexpr float FINF = __builtin_huge_valf();
+
+template <int G>
+struct CellState {
+  float N[G], px[G], py[G], pz[G];
+  float S[G];
+  float n0, x, y, eps;
+};
+
+struct Rates { float alpha, beta, cHI, cHII, rec; };
+
+// per-cell tallies, folded into the thread's fp64 Acc when the cell completes
+struct CellTally { float absorbed = 0.f, injected = 0.f, recomb = 0.f; unsigned nsub = 0, nhalv = 0; };
+
+__device__ __forceinline__ void decode_x(float xs, float& x, float& y)
+{
+  if (__float_as_int(xs) < 0) { y = -xs; x = 1.f - y; } else { x = xs; y = 1.f - xs; }
+}
+__device__ __forceinline__ float encode_x(float x, float y)
+{
+  return (x <= 0.5f) ? fabsf(x) : __int_as_float(__float_as_int(fabsf(y)) | 0x80000000);
+}
+
+// A11 rate fits at temperature T.  lam = 2 * 157807 / T.
+__device__ __forceinline__ Rates rates_at(float T, int otsa, float x, float n0)
+{
+  Rates r;
+  const float lT = flg2(T), rT = frcp(T);
+  const float llam = 18.267802f - lT;                 // log2(315614 / T)
+  const float lam = 315614.f * rT;
+  // alpha_B = 2.753e-14 lam^1.5 / (1 + (lam/2.740)^0.407)^2.242
+  const float aB = 2.753e-14f * fex2(1.5f * llam - 2.242f * flg2(1.f + fex2(0.407f * (llam - 1.4541759f))));
+  // beta = 21.11 T^-1.5 e^{-lam/2} lam^-1.089 / (1 + (lam/0.354)^0.874)^1.101
+  const float be = 21.11f * fex2(-1.5f * lT - 1.089f * llam - 1.101f * flg2(1.f + fex2(0.874f * (llam + 1.4981787f)))) *
+                   fex2(-0.5f * LOG2E * lam);
+  const float sqT = fsqrt(T);
+  // collisional excitation + collisional ionisation cooling, per n_e n_HI
+  r.cHI = 7.5e-19f * fex2(-118348.f * LOG2E * rT) * frcp(1.f + sqT * 3.1622776e-3f) + 2.179e-11f * be;
+  const float dl = 5.5f - 0.30103f * lT;              // 5.5 - log10 T
+  const float ff = 1.42e-27f * (1.1f + 0.34f * fex2(-(LOG2E / 3.f) * dl * dl)) * sqT;     // bremsstrahlung
+  r.beta = be;
+  if (otsa) {
+    // Lambda_rec,B = 3.435e-30 T lam^1.970 / (1 + (lam/2.250)^0.376)^3.720
+    const float recB = 3.435e-30f * T * fex2(1.970f * llam - 3.720f * flg2(1.f + fex2(0.376f * (llam - 1.169925f))));
+    r.alpha = aB;                                     // alpha_A := alpha_B
+    r.cHII = recB + ff;
+    r.rec = 0.f;
+  } else {
+    const float aA = 1.269e-13f * fex2(1.503f * llam - 1.923f * flg2(1.f + fex2(0.470f * (llam + 0.9378783f))));
+    const float recA = 1.778e-29f * T * fex2(1.965f * llam - 2.697f * flg2(1.f + fex2(0.502f * (llam + 0.8862995f))));
+    r.alpha = aA;
+    r.cHII = recA + ff;
+    r.rec = (aA - aB) * x * x * n0 * n0;              // A6: recombination radiation, group 1 only
+  }
+  return r;
+}
+
+// Eq. 44 with the factor chosen by attempt(): m > 0 -> F' = F m (m = 1/(1 + k dtau), strong sink);
+// m <= 0 -> F' = F + F m (m = -k dtau/(1 + k dtau), weak sink: only the small decrement is rounded)
+__device__ __forceinline__ float decay(float v, float m) { return (m > 0.f) ? v * m : fmaf(v, m, v); }
+
+// One attempt of Eq. 43-48 with step dtau from state p = c.  Returns the 10 % verdict.
+template <int G>
+__device__ __forceinline__ bool attempt(const ChemParams& cp, const CellState<G>& c, const Rates& r, float dtau,
+                                        float (&N1)[G], float (&iden)[G], float& x1, float& y1, float& eps1)
+{
+  // Every backward-Euler quotient q' = (q + a dtau)/(1 + k dtau) is evaluated in the form that loses nothing:
+  // for a weak sink (k dtau <= 1/2) as the increment q + (a dtau - k dtau q)/(1 + k dtau), whose rounding is
+  // relative to the (small) increment, so a slowly relaxing cell does not drift by an ulp per step; for a strong
+  // sink as the printed quotient (the increment form would cancel there).
+  const float k = c.y * c.n0 * dtau;
+  float ion = 0.f, hsum = 0.f;
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float kd = cp.csig[g] * k;                                  // A5: c sigma (1-x^p) n0 dtau
+    const float id = frcp(1.f + kd);
+    const float kid = kd * id;
+    const float sdt = (c.S[g] + (g == 0 ? r.rec : 0.f)) * dtau;
+    const bool strong = kd > 0.5f;
+    N1[g] = strong ? (c.N[g] + sdt) * id : c.N[g] + fmaf(-kid, c.N[g], sdt * id);     // Eq. 43
+    iden[g] = strong ? id : -kid;                                     // Eq. 44, applied on commit by decay()
+    ion = fmaf(cp.csig[g], N1[g], ion);                               // Eq. 41
+    hsum = fmaf(cp.csigE[g], N1[g], hsum);                            // Eq. 42
+  }
+  const float Gt = dtau * fmaf(r.beta * c.x, c.n0, ion);
+  const float rr = r.alpha * c.x * c.x * c.n0 * dtau;
+  const float inv = frcp(1.f + Gt);
+  float xa, ya;
+  if (Gt > 0.5f) {
+    xa = (c.x + (Gt - rr)) * inv;                                     // Eq. 45, solved for x
+    ya = (c.y + rr) * inv;                                            // Eq. 45 as printed (1 - x^{p+1})
+  } else {
+    const float dx = fmaf(Gt, c.y, -rr) * inv;                        // x' - x
+    xa = c.x + dx;
+    ya = c.y - dx;
+  }
+  if (xa <= 0.5f) ya = 1.f - xa; else xa = 1.f - ya;
+  xa = fminf(fmaxf(xa, 0.f), 1.f);                                    // guards (A7)
+  ya = fminf(fmaxf(ya, 0.f), 1.f);
+  x1 = xa; y1 = ya;
+  if (!cp.thermal) {                                                  // isothermal test mode: T held (A9)
+    const float dx = (xa <= 0.5f) ? xa - c.x : c.y - ya;
+    eps1 = fmaf(c.eps * dx, frcp(1.f + c.x), c.eps);
+    return true;
+  }
+  // Eq. 46-48 per atom: heating c (1-x') sum Sigma_E N', cooling Lambda(n0, x', T^p)/n0
+  const float de = dtau * (ya * hsum - c.n0 * xa * fmaf(ya, r.cHI, xa * r.cHII));
+  eps1 = c.eps + de;
+  return (fabsf(de) <= cp.e_tol * c.eps) && (eps1 > 0.f);
+}
+
+// One ACCEPTED sub-step (rates at state p, first guess, halvings).  Returns false on ESUBCYCLE.
+template <int G>
+__device__ __forceinline__ bool substep(const ChemParams& cp, CellState<G>& c, float& rem, CellTally& tl, float& dtau_min)
+{
+  const float T = c.eps * frcp(KB15 * (1.f + c.x));
+  const Rates r = rates_at(T, cp.otsa, c.x, c.n0);
+  float dtau = rem;
+  if (cp.thermal) {
+    float hsum = 0.f;
+#pragma unroll
+    for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
+    const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);      // (H - Lambda)/n0 at state p
+    const float guess = (d == 0.f) ? rem : fabsf(c.eps / d);                        // PAPER.md:290 (A9: abs)
+    dtau_min = fminf(dtau_min, guess);
+    dtau = fminf(rem, guess);
+  }
+  float N1[G], iden[G], x1, y1, eps1;
+  unsigned halv = 0;
+  bool ok = true;
+  while (!attempt<G>(cp, c, r, dtau, N1, iden, x1, y1, eps1)) {
+    if (halv >= (unsigned)cp.max_halvings) { ok = false; break; }
+    dtau *= 0.5f;                                                     // PAPER.md:312 "divided by 2"
+    halv++;
+  }
+  tl.nhalv += halv;
+  if (!ok) return false;
+  const float k = c.y * c.n0 * dtau;
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);           // A15: the sink of Eq. 43
+    tl.injected = fmaf(c.S[g], dtau, tl.injected);
+    c.N[g] = N1[g];
+    c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);   // Eq. 44
+  }
+  tl.recomb = fmaf(r.rec, dtau, tl.recomb);
+  c.x = x1; c.y = y1; c.eps = eps1;
+  tl.nsub++;
+  rem = (dtau >= rem) ? 0.f : rem - dtau;
+  if (tl.nsub >= EMMA_RT_MAX_SUBSTEPS && rem > 0.f) return false;
+  return true;
+}
+
+__device__ __forceinline__ void fold(Acc& a, const CellTally& tl, const float* N, int G, double dV)
+{
+  a.absorbed += (double)tl.absorbed * dV;
+  a.injected += (double)tl.injected * dV;
+  a.recomb += (double)tl.recomb * dV;
+  a.nsub += tl.nsub; a.nhalv += tl.nhalv;
+  a.nsub_max = max(a.nsub_max, tl.nsub);
+  float s = 0.f;
+  for (int g = 0; g < G; g++) s += N[g];
+  a.total += (double)s * dV;
+}
+
+template <int G>
+__device__ __forceinline__ void load_sources(const LevelDev& L, long long cell, float (&S)[G])
+{
+#pragma unroll
+  for (int g = 0; g < G; g++) S[g] = 0.f;
+  if (L.n_src == 0) return;
+  if (!((L.srcmask[cell >> 5] >> (cell & 31)) & 1u)) return;
+  int lo = 0, hi = L.n_src - 1;                                       // sorted list, the cell is in it
+  const int key = (int)cell;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (L.src_cell[mid] < key) lo = mid + 1; else hi = mid;
+  }
+#pragma unroll
+  for (int g = 0; g < G; g++) S[g] = L.src_S[(size_t)lo * G + g];
+}
+
+template <int G>
+__device__ __forceinline__ void load_cell(const LevelDev& L, long long cell, const float4* __restrict__ U,
+                                          long long ustride, long long ucell, CellState<G>& c)
+{
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float4 u = U[(size_t)g * ustride + ucell];
+    c.N[g] = u.x; c.px[g] = u.y; c.py[g] = u.z; c.pz[g] = u.w;
+  }
+  c.n0 = L.n0[cell];
+  c.eps = L.eps[cell];
+  decode_x(L.xs[cell], c.x, c.y);
+  load_sources<G>(L, cell, c.S);
+}
+
+template <int G>
+__device__ __forceinline__ bool finite_cell(const CellState<G>& c)
+{
+  float s = fabsf(c.eps) + fabsf(c.x);
+#pragma unroll
+  for (int g = 0; g < G; g++) s += fabsf(c.N[g]) + fabsf(c.px[g]) + fabsf(c.py[g]) + fabsf(c.pz[g]);
+  return s < FINF;
+}
+
+template <int G>
+__device__ __forceinline__ void store_cell(const LevelDev& L, long long cell, float4* __restrict__ U, long long ustride,
+                                           const CellState<G>& c, const CellTally& tl, int record)
+{
+#pragma unroll
+  for (int g = 0; g < G; g++) U[(size_t)g * ustride + cell] = make_float4(c.N[g], c.px[g], c.py[g], c.pz[g]);
+  L.xs[cell] = encode_x(c.x, c.y);
+  L.eps[cell] = c.eps;
+  if (record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// level 0, pass 1: every unrefined coarse cell gets one attempt with dtau = dt (HBM-bound)
+// ------------------------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(256)
+chem_main_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, long long ncell,
+                 int* __restrict__ queue, unsigned int* __restrict__ qcount, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const int lane = threadIdx.x & 31;
+  for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += (long long)gridDim.x * blockDim.x) {
+    const long long cell = base + threadIdx.x;
+    bool valid = cell < ncell;
+    if (valid && L.refined) valid = !((L.refined[cell >> 5] >> (cell & 31)) & 1u);   // split cells: CRTA kernels
+    bool defer = false;
+    if (valid) {
+      CellState<G> c;
+      load_cell<G>(L, cell, U, ncell, cell, c);
+      CellTally tl;
+      float dmin = FINF;
+      // fast path == the first trip of the sub-cycle loop when it covers the whole step
+      const float T = c.eps * frcp(KB15 * (1.f + c.x));
+      const Rates r = rates_at(T, cp.otsa, c.x, c.n0);
+      bool go = true;
+      if (cp.thermal) {
+        float hsum = 0.f;
+#pragma unroll
+        for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
+        const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
+        const float guess = (d == 0.f) ? cp.dt : fabsf(c.eps / d);
+        go = guess >= cp.dt;
+        if (go) dmin = guess;
+      }
+      float N1[G], iden[G], x1, y1, eps1;
+      if (go) go = attempt<G>(cp, c, r, cp.dt, N1, iden, x1, y1, eps1);
+      if (go) {
+        const float k = c.y * c.n0 * cp.dt;
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);
+          tl.injected = fmaf(c.S[g], cp.dt, tl.injected);
+          c.N[g] = N1[g];
+          c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);
+        }
+        tl.recomb = r.rec * cp.dt;
+        c.x = x1; c.y = y1; c.eps = eps1;
+        tl.nsub = 1;
+        store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
+        fold(acc, tl, c.N, G, L.dV);
+        acc.dtau_min = fminf(acc.dtau_min, dmin);
+        if (!finite_cell<G>(c)) acc.nonfinite++;
+      } else {
+        defer = true;
+      }
+    }
+    // warp-aggregated append of the deferred cells (north_star item 3: warp-level work compaction)
+    const unsigned m = __ballot_sync(0xffffffffu, defer);
+    if (m) {
+      const int leader = __ffs(m) - 1;
+      unsigned b = 0;
+      if (lane == leader) b = atomicAdd(qcount, (unsigned)__popc(m));
+      b = __shfl_sync(0xffffffffu, b, leader);
+      if (defer) {
+        queue[b + __popc(m & ((1u << lane) - 1u))] = (int)cell;
+        acc.ndefer++;
+      }
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// level 0, pass 2: persistent warps over the compacted queue of cells that need real sub-cycling
+// ------------------------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(128)
+chem_tail_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, long long ncell,
+                 const int* __restrict__ queue, const unsigned int* __restrict__ qcount,
+                 unsigned int* __restrict__ qhead, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const unsigned nq = *qcount;
+  const int lane = threadIdx.x & 31;
+  CellState<G> c;
+  CellTally tl;
+  float rem = 0.f, dmin = FINF;
+  long long cell = -1;
+  bool has = false, exhausted = false;
+  for (;;) {
+    // refill idle lanes
+    const unsigned want = __ballot_sync(0xffffffffu, !has && !exhausted);
+    if (want) {
+      const int leader = __ffs(want) - 1;
+      unsigned b = 0;
+      if (lane == leader) b = atomicAdd(qhead, (unsigned)__popc(want));
+      b = __shfl_sync(0xffffffffu, b, leader);
+      if (!has && !exhausted) {
+        const unsigned idx = b + __popc(want & ((1u << lane) - 1u));
+        if (idx < nq) {
+          cell = queue[idx];
+          load_cell<G>(L, cell, U, ncell, cell, c);
+          tl = CellTally();
+          rem = cp.dt; dmin = FINF;
+          has = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(0xffffffffu, has)) break;
+    if (has) {
+      const bool ok = substep<G>(cp, c, rem, tl, dmin);
+      if (!ok) acc.err |= 1u;
+      if (!ok || rem <= 0.f) {
+        store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
+        fold(acc, tl, c.N, G, L.dV);
+        acc.dtau_min = fminf(acc.dtau_min, dmin);
+        if (!finite_cell<G>(c)) acc.nonfinite++;
+        has = false;
+      }
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// refined level l >= 1 (CRTA): inject -> leaf chemistry -> restriction to the parent, one thread per cell,
+// 8 consecutive lanes = one oct.  Deepest level first; level 1 writes the coarse cell in place.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float oct_sum(float v)
+{
+  // pairwise along x, then y, then z: (((c0+c1)+(c2+c3))+((c4+c5)+(c6+c7)))   (A14)
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  return v;
+}
+
+template <int G>
+__global__ void __launch_bounds__(128)
+chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow, const float4* __restrict__ Ut_above,
+                    long long nocts_above, float4* __restrict__ U0, long long ncell0, int level,
+                    Partial* __restrict__ parts)
+{
+  Acc acc;
+  const long long ncell = L.ncell;                                    // multiple of 8
+  for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += (long long)gridDim.x * blockDim.x) {
+    const long long cell = base + threadIdx.x;
+    const bool valid = cell < ncell;                                  // uniform per 8-lane group
+    CellState<G> c;
+    float e_den = 0.f;                                                // energy per volume for the restriction
+#pragma unroll
+    for (int g = 0; g < G; g++) { c.N[g] = c.px[g] = c.py[g] = c.pz[g] = 0.f; }
+    c.x = c.y = c.eps = c.n0 = 0.f;
+    long long oct = 0;
+    if (valid) {
+      oct = cell >> 3;
+      const int ch = L.child ? L.child[cell] : -1;
+      if (ch < 0) {
+        // leaf: starts from the coarse ancestor's post-transport radiation (piecewise-constant injection)
+        load_cell<G>(L, cell, U0, ncell0, (long long)L.anc0[oct], c);
+        CellTally tl;
+        float rem = cp.dt, dmin = FINF;
+        bool ok = true;
+        while (ok && rem > 0.f) ok = substep<G>(cp, c, rem, tl, dmin);
+        if (!ok) acc.err |= 1u;
+        L.xs[cell] = encode_x(c.x, c.y);
+        L.eps[cell] = c.eps;
+        if (cp.record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
+        fold(acc, tl, c.N, G, L.dV);
+        acc.dtau_min = fminf(acc.dtau_min, dmin);
+        if (!finite_cell<G>(c)) acc.nonfinite++;
+      } else {
+        // split cell: restricted values were written by the kernel of the level above
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 u = Ut_above[(size_t)g * nocts_above + ch];
+          c.N[g] = u.x; c.px[g] = u.y; c.py[g] = u.z; c.pz[g] = u.w;
+        }
+        c.n0 = L.n0[cell]; c.eps = L.eps[cell];
+        decode_x(L.xs[cell], c.x, c.y);
+        if (cp.record) L.subc[cell] = 0;
+      }
+      e_den = c.eps * c.n0;
+    }
+    // restriction: mean of the 8 children (A14)
+    float4 m[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      m[g].x = 0.125f * oct_sum(c.N[g]); m[g].y = 0.125f * oct_sum(c.px[g]);
+      m[g].z = 0.125f * oct_sum(c.py[g]); m[g].w = 0.125f * oct_sum(c.pz[g]);
+    }
+    const float xm = 0.125f * oct_sum(c.x), ym = 0.125f * oct_sum(c.y), em = 0.125f * oct_sum(e_den);
+    if (valid && (cell & 7) == 0) {
+      const long long pc = L.parent[oct];                             // split cell on the level below
+      if (level == 1) {
+#pragma unroll
+        for (int g = 0; g < G; g++) U0[(size_t)g * ncell0 + pc] = m[g];
+      } else {
+#pragma unroll
+        for (int g = 0; g < G; g++) L.Ut[(size_t)g * L.nocts + oct] = m[g];
+      }
+      Lbelow.xs[pc] = encode_x(xm, ym);
+      Lbelow.eps[pc] = em / Lbelow.n0[pc];
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// chemistry off: Eq. 43 degenerates to N += S dt in the source cells (A9); sources are folded to the coarse level
+template <int G>
+__global__ void inject_kernel(const LevelDev L, float dt, float4* __restrict__ U, long long ncell, Partial* parts)
+{
+  Acc acc;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < L.n_src; i += gridDim.x * blockDim.x) {
+    const long long cell = L.src_cell[i];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      const float add = L.src_S[(size_t)i * G + g] * dt;
+      U[(size_t)g * ncell + cell].x += add;
+      acc.injected += (double)add * L.dV;
+      acc.total += (double)add * L.dV;
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// children mean of n0, x, e at init (bottom-up), 8 lanes per oct
+__global__ void restrict_init_kernel(const LevelDev L, const LevelDev Lbelow)
+{
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = cell < L.ncell;
+  float n0 = 0.f, x = 0.f, y = 0.f, e = 0.f;
+  if (valid) {
+    n0 = L.n0[cell];
+    decode_x(L.xs[cell], x, y);
+    e = L.eps[cell] * n0;
+  }
+  const float nm = 0.125f * oct_sum(n0), xm = 0.125f * oct_sum(x), ym = 0.125f * oct_sum(y), em = 0.125f * oct_sum(e);
+  if (valid && (cell & 7) == 0) {
+    const long long pc = L.parent[cell >> 3];
+    Lbelow.n0[pc] = nm;
+    Lbelow.xs[pc] = encode_x(xm, ym);
+    Lbelow.eps[pc] = em / nm;
+  }
+}
+
+template <int G>
+int chem_level0_G(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue, unsigned int* qcount,
+                  Partial* parts, int* n_parts, int sm_count, cudaStream_t st, Profiler* pf)
+{
+  long long want = (ncell + 255) / 256;
+  int nb = (int)(want < (long long)sm_count * 8 ? want : (long long)sm_count * 8);
+  if (nb > MAX_PART_BLOCKS) nb = MAX_PART_BLOCKS;
+  pf->begin(EMMA_RT_K_CHEM_MAIN);
+  chem_main_kernel<G><<<nb, 256, 0, st>>>(cp, L0, U, ncell, queue, qcount, parts);
+  pf->end();
+  *n_parts = nb;
+  if (!cp.thermal) return 1;                                          // isothermal mode never defers
+  int nt = sm_count * 8;
+  if (nt > MAX_PART_BLOCKS) nt = MAX_PART_BLOCKS;
+  pf->begin(EMMA_RT_K_CHEM_TAIL);
+  chem_tail_kernel<G><<<nt, 128, 0, st>>>(cp, L0, U, ncell, queue, qcount, qcount + 1, parts + nb);
+  pf->end();
+  *n_parts = nb + nt;
+  return 2;
+}
+
+}  // namespace
+
+int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
+                       unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, cudaStream_t st, Profiler* pf)
+{
+  switch (cp.G) {
+    case 1: return chem_level0_G<1>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
+    case 2: return chem_level0_G<2>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
+    case 3: return chem_level0_G<3>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
+    default: return chem_level0_G<4>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
+  }
+}
+
+int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U, long long ncell0,
+                        Partial* parts, int* n_parts, cudaStream_t st)
+{
+  const LevelDev& L = lv[level];
+  if (L.ncell == 0) { *n_parts = 0; return 0; }
+  long long want = (L.ncell + 127) / 128;
+  int nb = (int)(want < MAX_PART_BLOCKS ? want : MAX_PART_BLOCKS);
+  const float4* Ut_above = (level < n_levels) ? lv[level + 1].Ut : nullptr;
+  const long long nocts_above = (level < n_levels) ? lv[level + 1].nocts : 0;
+  switch (cp.G) {
+    case 1: chem_refined_kernel<1><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
+    case 2: chem_refined_kernel<2><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
+    case 3: chem_refined_kernel<3><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
+    default: chem_refined_kernel<4><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
+  }
+  *n_parts = nb;
+  return 1;
+}
+
+int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts, int* n_parts,
+                          cudaStream_t st)
+{
+  if (L0.n_src == 0) { *n_parts = 0; return 0; }
+  int nb = (L0.n_src + 127) / 128;
+  if (nb > 64) nb = 64;
+  switch (G) {
+    case 1: inject_kernel<1><<<nb, 128, 0, st>>>(L0, dt, U, ncell0, parts); break;
+    case 2: inject_kernel<2><<<nb, 128, 0, st>>>(L0, dt, U, ncell0, parts); break;
+    case 3: inject_kernel<3><<<nb, 128, 0, st>>>(L0, dt, U, ncell0, parts); break;
+    default: inject_kernel<4><<<nb, 128, 0, st>>>(L0, dt, U, ncell0, parts); break;
+  }
+  *n_parts = nb;
+  return 1;
+}
+
+int launch_restrict_init(const LevelDev* lv, int level, cudaStream_t st)
+{
+  const LevelDev& L = lv[level];
+  if (L.ncell == 0) return 0;
+  const int nb = (int)((L.ncell + 127) / 128);
+  restrict_init_kernel<<<nb, 128, 0, st>>>(L, lv[level - 1]);
+  return 1;
+}
+
+}  // namespace emma

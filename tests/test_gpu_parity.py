@@ -1,0 +1,351 @@
+"""T2: CUDA path vs the fp64 oracle through the C-ABI, element by element, on the same seeded inputs.
+
+Tolerances are north_star's: N, F <= 1e-5 after one step (A17 norms); x_HII, T <= 1e-4 after the configured number of
+coupled steps; photon budget <= 1e-6 relative.  Run on the B200 box with `-m gpu`.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as O
+import paper_1508_07888_b200 as E
+from workloads import CGS, make_config
+
+from .helpers import groups, tiny_workload
+from .parity import absorption_condition, budget_residual, compare, run_pair, stencil_scale
+
+pytestmark = pytest.mark.gpu
+
+TOL_NF, TOL_XT, TOL_BUDGET = 1e-5, 1e-4, 1e-6
+C_RED = 0.1 * CGS.c
+
+
+def _random_U(rng, G, nc, c, fmax=1.0, lo=-6.0, hi=-2.0):
+    U0 = np.zeros((G, nc, 4))
+    for g in range(G):
+        N = 10 ** rng.uniform(lo, hi, nc)
+        d = rng.standard_normal((nc, 3))
+        d /= np.linalg.norm(d, axis=1)[:, None]
+        U0[g, :, 0] = N
+        U0[g, :, 1:] = (rng.uniform(0, fmax, nc) * c * N)[:, None] * d
+    return U0.astype(np.float32)
+
+
+BCS = [(4, 1, (0,) * 6), (8, 3, (0,) * 6), (20, 2, (1, 2, 0, 0, 2, 1)), (33, 1, (2, 2, 1, 1, 0, 0)),
+       (40, 3, (0,) * 6), (50, 1, (1, 1, 1, 1, 1, 1)), (64, 2, (0, 0, 2, 1, 0, 0))]
+
+
+# ------------------------------------------------------------------------------------------- transport only
+@pytest.mark.parametrize("n,G,bc", BCS)
+def test_transport_one_step_config_like_state(n, G, bc):
+    """Closure + GLF + update, several tiles and z chunks, ragged tails (n not a multiple of the 32x16 tile), every
+    boundary type.  State shaped like config 5b: N log-uniform over 5 decades cell to cell, f uniform in [0, 0.9],
+    isotropic directions.  north_star tolerance with the A17 norms."""
+    rng = np.random.default_rng(n * 10 + G)
+    w = tiny_workload(n, G, bc=bc, chemistry=0, U0=_random_U(rng, G, n ** 3, C_RED, fmax=0.9, lo=-7, hi=-2), courant=0.9)
+    orc, gpu, _, diags = run_pair(w, 1, track_signatures=False)
+    rep = compare(orc, gpu, w)
+    assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
+    do, dg = diags[0]
+    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+    assert abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-6 * do["photons_total"]
+
+
+@pytest.mark.parametrize("n,G,bc", BCS[2:])
+def test_transport_one_step_adversarial_state(n, G, bc):
+    """Unphysical reduced fluxes up to f = 1.2 (exercises the clip of A2) at Courant number 1 (the own-cell weight
+    1 - 3 nu vanishes): the update can cancel to far below its terms, so the error is measured against the magnitude
+    of what is summed -- the 7-point stencil maximum of N -- which is what bounds an fp32 evaluation."""
+    rng = np.random.default_rng(n * 10 + G + 1)
+    U0 = _random_U(rng, G, n ** 3, C_RED, fmax=1.2)
+    w = tiny_workload(n, G, bc=bc, chemistry=0, U0=U0, courant=1.0)
+    orc, gpu, _, _ = run_pair(w, 1, track_signatures=False)
+    for g in range(G):
+        sc = stencil_scale(U0[g], n, bc)
+        Uo = orc.read(O.F_U, 0, g)
+        Ug = gpu.read(E.FIELD_U, 0, g).astype(np.float64)
+        assert (np.abs(Ug[:, 0] - Uo[:, 0]) / sc).max() <= 2e-6
+        assert (np.abs(Ug[:, 1:] - Uo[:, 1:]).max(axis=1) / (C_RED * sc)).max() <= 2e-6
+
+
+def test_transport_many_steps_chunks_and_wrap():
+    """20 steps on 48^3 (z chunks, periodic wrap across tile and chunk borders): a hot corner cell and a free-streaming
+    beam cell spread into vacuum.  Upstream of the beam the exact solution cancels to ~1e-13 of the peak while fp32
+    leaves its cancellation residue (measured: ~2e-10 of the peak), so the error floor is 1e-4 of the peak here."""
+    n = 48
+    U0 = np.zeros((1, n, n, n, 4), np.float32)
+    U0[0, 0, n - 1, 0, 0] = 1.0
+    U0[0, 24, 17, 33, :] = (0.5, 0.5 * C_RED * 0.6, 0.0, -0.5 * C_RED * 0.8)
+    w = tiny_workload(n, 1, chemistry=0, U0=U0.reshape(1, -1, 4))
+    orc, gpu, _, diags = run_pair(w, 20, track_signatures=False, block=20)
+    rep = compare(orc, gpu, w, nf_floor=1e-4)
+    assert rep["N"] <= 2e-5 and rep["F"] <= 2e-5, rep
+    do, dg = diags[-1]
+    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)    # conservative to rounding
+
+
+def test_P2_single_cell_example_on_gpu():
+    n, N0 = 7, 2.0
+    c = n // 2
+    U0 = np.zeros((1, n, n, n, 4), np.float32)
+    U0[0, c, c, c, 0] = N0
+    w = tiny_workload(n, 1, U0=U0.reshape(1, -1, 4), chemistry=0, courant=0.6)
+    gpu = E.EmmaRT(w)
+    rc, d = gpu.step(w.dt, 1)
+    assert rc == E.OK
+    U = gpu.read(E.FIELD_U).reshape(n, n, n, 4).astype(np.float64)
+    nu = 0.2
+    assert U[c, c, c, 0] == pytest.approx((1 - 3 * nu) * N0, rel=1e-6)
+    assert U[c, c, c + 1, 0] == pytest.approx(nu * N0 / 2, rel=1e-6)
+    assert U[c, c, c + 1, 1] == pytest.approx(nu * w.c_red * N0 / 6, rel=1e-6)
+    assert U[c - 1, c, c, 3] == pytest.approx(-nu * w.c_red * N0 / 6, rel=1e-6)
+    assert U[..., 0].sum() == pytest.approx(N0, rel=1e-6)
+
+
+def test_P3_free_streaming_beam_on_gpu():
+    """chi = 1 branch on the device: a plane beam F = c N x^ stays free-streaming and moves at c~ (binomial form)."""
+    from math import comb
+    n, k = 16, 6
+    prof = np.zeros(n)
+    prof[3:6] = [1.0, 2.5, 0.5]
+    U0 = np.zeros((1, n, n, n, 4), np.float32)
+    U0[0, ..., 0] = prof[None, None, :]
+    U0[0, ..., 1] = U0[0, ..., 0] * np.float32(2.0 ** 31)
+    w = tiny_workload(n, 1, c_red=2.0 ** 31, chemistry=0, courant=0.75, U0=U0.reshape(1, -1, 4))
+    gpu = E.EmmaRT(w)
+    gpu.step(w.dt, k)
+    U = gpu.read(E.FIELD_U).reshape(n, n, n, 4).astype(np.float64)
+    nu = 0.25
+    exp = np.array([sum(comb(k, j) * nu ** j * (1 - nu) ** (k - j) * prof[(i - j) % n] for j in range(k + 1)) for i in range(n)])
+    assert np.allclose(U[5, 7, :, 0], exp, rtol=0, atol=2e-6 * exp.max())
+    assert np.allclose(U[..., 1], w.c_red * U[..., 0], rtol=0, atol=2e-6 * w.c_red * exp.max())
+
+
+def test_P1_uniform_field_invariant_on_gpu():
+    n = 36
+    U0 = np.zeros((2, n ** 3, 4), np.float32)
+    U0[:, :, 0] = 3.25e-4
+    w = tiny_workload(n, 2, U0=U0, chemistry=0)
+    gpu = E.EmmaRT(w)
+    gpu.step(w.dt, 10)
+    U = gpu.read(E.FIELD_U, 0, 1)
+    assert np.allclose(U[:, 0], 3.25e-4, rtol=2e-6) and np.abs(U[:, 1:]).max() <= 1e-6 * w.c_red * 3.25e-4
+
+
+def test_dark_cells_with_denormal_photon_density_stay_finite():
+    """Light reaching a dark cell passes through the fp32 denormal range; the closure must treat it as N = 0."""
+    n = 12
+    U0 = np.zeros((1, n ** 3, 4), np.float32)
+    U0[0, :, 0] = 1e-42
+    U0[0, :, 1] = 1e-42 * 0.5 * C_RED
+    U0[0, 7, 0] = 1e-3
+    w = tiny_workload(n, 1, U0=U0, chemistry=0)
+    gpu = E.EmmaRT(w)
+    rc, d = gpu.step(w.dt, 30)
+    assert rc == E.OK and d["n_nonfinite"] == 0
+    assert np.isfinite(gpu.read(E.FIELD_U)).all()
+
+
+def test_chemistry_off_sources_add_S_dt():
+    w = make_config(3, n=16, n_src=3)
+    orc, gpu, _, diags = run_pair(w, 3, chemistry=0, track_signatures=False)
+    rep = compare(orc, gpu, w)
+    assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
+    for do, dg in diags:
+        assert dg["photons_injected"] == pytest.approx(do["photons_injected"], rel=1e-6)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+
+
+# ------------------------------------------------------------------------------------------- coupled, one step
+@pytest.mark.parametrize("n,G,otsa", [(8, 1, 1), (24, 3, 1), (24, 3, 0), (40, 2, 1)])
+def test_coupled_one_step_random_state(n, G, otsa):
+    """One coupled step from random (x, T, N, F, n0): every rate, both sides of x = 1/2, sources, sub-cycling."""
+    rng = np.random.default_rng(7 * n + G + otsa)
+    nc = n ** 3
+    n0 = (10 ** rng.uniform(-5, -1, nc)).astype(np.float32)
+    x = np.minimum(10 ** rng.uniform(-4, 0, nc), 0.999999).astype(np.float32)
+    T = (10 ** rng.uniform(2, 4.7, nc)).astype(np.float32)
+    pos = rng.random((4, 3))
+    Q = 10 ** rng.uniform(47, 49, (4, G))
+    w = tiny_workload(n, G, n0=n0, x=x, T=T, U0=_random_U(rng, G, nc, C_RED, fmax=0.9, lo=-7, hi=-2), otsa=otsa,
+                      src_pos=pos, src_Q=Q)
+    orc, gpu, flips, diags = run_pair(w, 1)
+    rep = compare(orc, gpu, w, flips, 1)
+    do, dg = diags[0]
+    assert rep["flips"] <= max(2, 1e-4 * rep["cells"]), rep
+    assert do["subcycles_max"] > 1 and dg["n_deferred"] > 0           # the divergent branch is exercised
+    assert rep["x"] <= TOL_XT and rep["T"] <= TOL_XT and rep["xn"] <= TOL_XT, rep
+    # N, F: this state is harsher than any config (T up to 5e4 K at n0 up to 0.1: hundreds of sub-steps per cell,
+    # each rounding N once), so 5e-5 here; the north_star 1e-5 is asserted on the config states below
+    assert rep["N"] <= 5e-5 and rep["F"] <= 5e-5, rep
+    # diagnostics agree with the oracle's
+    for k in ("photons_total", "photons_injected", "photons_absorbed"):
+        assert dg[k] == pytest.approx(do[k], rel=2e-5), k
+    if not otsa:
+        assert dg["photons_recomb_emitted"] == pytest.approx(do["photons_recomb_emitted"], rel=1e-4)
+    assert abs(dg["subcycles_total"] - do["subcycles_total"]) <= 1e-3 * do["subcycles_total"]
+    assert dg["subcycles_max"] == do["subcycles_max"] or rep["flips"] > 0
+    assert dg["dtau_min"] == pytest.approx(do["dtau_min"], rel=1e-3)
+
+
+def test_isothermal_mode_and_equilibrium_on_gpu():
+    """thermal = 0: one backward-Euler sub-step per cell; with uniform S the state relaxes to the closed form P7."""
+    gr = groups(1)
+    T, n0 = 1.0e4, 1.0e-2
+    r = O.rates(T)
+    a, b = r["alphaB"], r["beta"]
+    S = 0.4 * a * n0 * n0
+    xeq = (b * n0 ** 2 + math.sqrt(b ** 2 * n0 ** 4 + 4 * (a + b) * n0 ** 2 * S)) / (2 * (a + b) * n0 ** 2)
+    n = 4
+    nc = n ** 3
+    pos = (np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / n
+    # dx = 1e23 cm so that one step is ~3 % of the relaxation time: an fp32 state stops moving once its increment
+    # falls under half an ulp, i.e. within eps32/(dt G) of equilibrium ("resolution")
+    w = tiny_workload(n, 1, L=n * 1e23, n0=n0, x=0.1, T=T, thermal=0, src_pos=pos, src_Q=np.full((nc, 1), S * 1e69))
+    gpu = E.EmmaRT(w)
+    dt = w.dx / (3 * w.c_red)
+    t_rec = 1.0 / (a * n0)
+    d = None
+    for _ in range(int(25 * t_rec / (50 * dt)) + 1):
+        rc, d = gpu.step(dt, 50, diag=True)
+        assert rc == E.OK
+    x = gpu.read(E.FIELD_X).astype(np.float64)
+    N = gpu.read(E.FIELD_N).astype(np.float64)
+    Tg = gpu.read(E.FIELD_T).astype(np.float64)
+    assert np.allclose(x, xeq, rtol=2e-5)
+    assert np.allclose(N, S / (w.c_red * gr["sigma_N"][0] * (1 - xeq) * n0), rtol=5e-5)
+    assert np.allclose(Tg, T, rtol=1e-4)
+    assert d["subcycles_max"] == 1 and d["n_deferred"] == 0
+
+
+# ------------------------------------------------------------------------------------------- the BASELINE configs
+def _run_config(w, n_steps, max_flip_frac=1e-4):
+    orc, gpu, flips, diags = run_pair(w, n_steps)
+    rep = compare(orc, gpu, w, flips, n_steps)
+    prev_g = None
+    worst_budget = 0.0
+    for do, dg in diags:
+        if prev_g is not None:
+            worst_budget = max(worst_budget, budget_residual(dg, prev_g))
+        prev_g = dg["photons_total"]
+    rep["budget"] = worst_budget
+    rep["sub_max"] = max(dg["subcycles_max"] for _, dg in diags)
+    print(w.name, n_steps, {k: (float("%.3g" % v) if isinstance(v, float) else v) for k, v in rep.items()})
+    assert rep["flips"] <= max(1, max_flip_frac * rep["cells"]), rep
+    assert rep["x"] <= TOL_XT and rep["T"] <= TOL_XT, rep
+    assert rep["x_near"] <= 2e-2 and rep["T_near"] <= 2e-2, rep       # flipped cells: both branches are valid results
+    assert rep["budget"] <= TOL_BUDGET, rep
+    return rep, diags
+
+
+def test_config1_stromgren_100_steps():
+    w = make_config(1)
+    rep, diags = _run_config(w, w.n_steps)
+    assert rep["N"] <= 1e-4 and rep["F"] <= 1e-4, rep                 # 100 steps of fp32 transport + chemistry
+    assert rep["sub_max"] > 10                                        # cells near the source really sub-cycle
+
+
+def test_config2_lognormal64_200_steps():
+    w = make_config(2)
+    _run_config(w, w.n_steps)
+
+
+def test_config3_three_groups_scaled():
+    _run_config(make_config(3, n=48), 100)
+
+
+def test_config3_three_groups_full_128():
+    w = make_config(3)                                                # 128^3, G = 3, fp32 fields, 256 sources
+    _run_config(w, w.n_steps)
+
+
+def test_config4_crta_scaled():
+    w = make_config(4, n=48, n_src=8)
+    assert w.n_levels == 2 and len(w.parent[1]) > 0
+    _run_config(w, 100, max_flip_frac=1e-3)
+
+
+@pytest.mark.parametrize("k,n", [(1, 32), (2, 64), (3, 64), (4, 32), (5, 64)])
+def test_configs_one_step_N_F(k, n):
+    """north_star: relative error <= 1e-5 on N and F after ONE coupled step, on the seeded inputs of every config
+    (configs 1-4 start dark, so they are first advanced 10 steps by the oracle-checked GPU path to get a field)."""
+    w = make_config(k, n=n)
+    warm = 0 if k == 5 else 10
+    orc, gpu, flips, diags = run_pair(w, warm + 1)
+    if warm:
+        # restart both sides from the GPU state after the warm-up so that exactly one step separates them
+        for g in range(w.G):
+            U = gpu.read(E.FIELD_U, 0, g)
+            w.U0 = (w.U0 or [None] * w.G)
+            w.U0[g] = U
+        for l in range(w.n_levels + 1):
+            w.x[l] = gpu.read(E.FIELD_X, l)
+            w.T[l] = gpu.read(E.FIELD_T, l)
+        orc, gpu, flips, diags = run_pair(w, 1)
+    rep = compare(orc, gpu, w, flips, 1, nf_cond=absorption_condition(w, w.dt))
+    print(w.name, "one step", {kk: (float("%.3g" % v) if isinstance(v, float) else v) for kk, v in rep.items()})
+    assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
+    assert rep["x"] <= TOL_NF and rep["T"] <= TOL_NF, rep
+    # the transport step alone (the M1 update whose outputs ARE N and F): plain A17 norms, no conditioning factor
+    orc, gpu, _, _ = run_pair(w, 1, chemistry=0, track_signatures=False)
+    rep = compare(orc, gpu, w)
+    print(w.name, "one transport step", {kk: float("%.3g" % rep[kk]) for kk in ("N", "F")})
+    assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
+
+
+def test_config5_sweep_scaled():
+    w = make_config(5, n=48)
+    _run_config(w, 50, max_flip_frac=1e-3)
+
+
+# ------------------------------------------------------------------------------------------- boundary behaviour
+def test_error_codes_and_api_contract():
+    w = make_config(1, n=8)
+    gpu = E.EmmaRT(w, record_subcycles=0)
+    dtmax = E.emma_rt_dt_cfl(gpu.h, 1.0)
+    assert dtmax == pytest.approx(w.dx / (3 * w.c_red))
+    x_before = gpu.read(E.FIELD_X).copy()
+    rc, _ = gpu.step(1.01 * dtmax, 1)
+    assert rc == E.ECFL and "A4" in gpu.last_error()
+    assert np.array_equal(gpu.read(E.FIELD_X), x_before)             # state untouched
+    assert gpu.set_sources([[1.0, 0.5, 0.5]], [[1e48]]) == E.EINVAL
+    assert gpu.set_sources([[0.5, 0.5, 0.5]], [[-1.0]]) == E.EINVAL
+    out = np.empty(8 ** 3, np.uint32)
+    assert gpu.read_into(E.FIELD_SUBCYCLES, 0, 0, out) == E.ESTATE    # record_subcycles not set
+    bad = np.empty(7, np.float32)
+    assert gpu.read_into(E.FIELD_X, 0, 0, bad) == E.EINVAL
+    assert gpu.read_into(E.FIELD_N, 0, 3, np.empty(8 ** 3, np.float32)) == E.EINVAL
+    # read is idempotent; set_sources replaces the list
+    a = gpu.read(E.FIELD_T)
+    assert np.array_equal(a, gpu.read(E.FIELD_T))
+    assert gpu.set_sources(np.zeros((0, 3)), np.zeros((0, 1))) == E.OK
+    rc, d = gpu.step(w.dt, 2)
+    assert rc == E.OK and d["photons_injected"] == 0.0
+    assert gpu.kernel_launches() > 0
+    # non-finite input is reported, the step still completes
+    Ubad = np.zeros((8 ** 3, 4), np.float32)
+    Ubad[5, 0] = np.inf
+    assert gpu.write(E.FIELD_U, 0, 0, Ubad) == E.OK
+    rc, d = gpu.step(w.dt, 1)
+    assert rc == E.ENONFINITE and d["n_nonfinite"] > 0
+
+
+def test_write_read_roundtrip_and_device_buffers():
+    import torch
+    w = make_config(5, n=12)
+    gpu = E.EmmaRT(w)
+    for g in range(3):
+        U = gpu.read(E.FIELD_U, 0, g)
+        assert np.allclose(U, w.U0[g], rtol=3e-7, atol=0)             # F <-> F/c conversion: <= 2 ulp
+    assert np.array_equal(gpu.read(E.FIELD_X), w.x[0])
+    assert np.allclose(gpu.read(E.FIELD_XNEUTRAL), 1.0 - w.x[0].astype(np.float64), rtol=1e-7)
+    assert np.allclose(gpu.read(E.FIELD_T), w.T[0], rtol=3e-7)
+    assert np.array_equal(gpu.read(E.FIELD_N0), w.n0[0])
+    t = torch.empty(12 ** 3, dtype=torch.float32, device="cuda")
+    assert gpu.read_into(E.FIELD_T, 0, 0, t) == E.OK
+    torch.cuda.synchronize()
+    assert np.allclose(t.cpu().numpy(), w.T[0], rtol=3e-7)
+    t2 = (t * 2).contiguous()
+    assert gpu.write(E.FIELD_T, 0, 0, t2) == E.OK
+    assert np.allclose(gpu.read(E.FIELD_T), 2 * w.T[0], rtol=5e-7)
