@@ -13,29 +13,57 @@
 // shared memory next to U; the paper's own stencil-array design recomputes it for every neighbour.
 //
 // Kernel shape: 2.5-D streaming.  A CTA owns a TX x TY column of cells and marches along z through a chunk of
-// planes; z-neighbours live in registers, x/y-neighbours come from a double-buffered shared-memory plane
-// (one barrier per plane).  Loads of plane k+2 are issued while plane k is computed.  HBM traffic is the
-// algorithmic 16 B read + 16 B write per cell-group plus the tile-edge halo (served from L2).
+// planes; every thread owns CY = 2 cells adjacent in y.  z-neighbours (and the y-neighbour inside the pair) live in
+// registers, the other x/y-neighbours come from a double-buffered shared-memory plane (one barrier per plane).
+// Loads of plane k+2 are issued while plane k is computed.  HBM traffic is the algorithmic 16 B read + 16 B write
+// per cell-group plus the tile-edge halo (served from L2).
+//
+// The first version of this kernel was issue-bound (ncu: 82 % issue slots busy, 291 instructions per cell-group,
+// profiles/r1a_*): this one is written for instruction count -- packed fp32 (FFMA2 on the (N,phi_x) and
+// (phi_y,phi_z) register pairs of the float4), pointer increments instead of 64-bit index arithmetic, diagnostics
+// compiled in only where a configuration needs them.
 #include "emma_rt_internal.cuh"
 
 namespace emma {
 
 namespace {
 
-constexpr int TX = 32, TY = 16;
+constexpr int TX = 32;                         // tile width = one warp along x
+constexpr int TYT = 8;                         // thread rows
+constexpr int CY = 2;                          // cells per thread along y
+constexpr int TY = TYT * CY;
+constexpr int NT = TX * TYT;
 constexpr int SW = TX + 2;                     // shared plane width incl. halo
 constexpr int SH = TY + 2;
 
-__device__ __forceinline__ void closure_ab(float N, float px, float py, float pz, float& a, float& b)
+// packed fp32 (sm_100a FFMA2 / FADD2): d = a * b + c on a register pair
+__device__ __forceinline__ void fma2(float& dx, float& dy, float ax, float ay, float bx, float by, float cx, float cy)
+{
+  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\t"
+      "mov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(dx), "=f"(dy)
+      : "f"(ax), "f"(ay), "f"(bx), "f"(by), "f"(cx), "f"(cy));
+}
+__device__ __forceinline__ void mul2(float& dx, float& dy, float ax, float ay, float bx, float by)
+{
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\t"
+      "mov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "mul.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(dx), "=f"(dy)
+      : "f"(ax), "f"(ay), "f"(bx), "f"(by));
+}
+
+__device__ __forceinline__ void closure_ab(const float4& U, float& a, float& b)
 {
   // A2: N <= 0 -> f = 0.  A denormal N (light that has just reached a dark cell) counts as 0: rcp.ftz of it is inf.
-  float rN = (N >= 1.1754944e-38f) ? frcp(N) : 0.f;
-  float rx = px * rN, ry = py * rN, rz = pz * rN;
-  float f2raw = rx * rx + ry * ry + rz * rz;
-  float f2 = fminf(f2raw, 1.f);                // A2: f clipped to [0,1]
-  float s = fsqrt(4.f - 3.f * f2);
-  float q = f2 * frcp(2.f + s);
-  a = N * (0.33333334f - q);
+  const float rN = (U.x >= 1.1754944e-38f) ? frcp(U.x) : 0.f;
+  const float rx = U.y * rN, ry = U.z * rN, rz = U.w * rN;
+  const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
+  const float f2 = fminf(f2raw, 1.f);          // A2: f clipped to [0,1]
+  const float s = fsqrt(fmaf(-3.f, f2, 4.f));
+  const float q = f2 * frcp(2.f + s);
+  a = fmaf(-U.x, q, 0.33333334f * U.x);
   // A1: |F| = 0 -> no n(x)n term; below f^2 = 1e-30 the term (<= f^2 N) is far under fp32 resolution of a
   b = (f2raw > 1e-30f) ? 3.f * q * rN * frcp(f2raw) : 0.f;
 }
@@ -57,37 +85,65 @@ __device__ __forceinline__ int bc_map(int i, int n, int bc_lo, int bc_hi, bool& 
   return i;
 }
 
-// contribution of the neighbour on the + side of direction d:  U - G_d
+template <int D>
+__device__ __forceinline__ float comp(const float4& U) { return (D == 0) ? U.y : (D == 1) ? U.z : U.w; }
+
+// contribution of the neighbour on the + side of direction d:  U - G_d = (N - phi_d, phi (1 - b phi_d) - a e_d)
 template <int D>
 __device__ __forceinline__ void add_plus(float4& acc, const float4& U, float a, float b)
 {
-  float pd = (D == 0) ? U.y : (D == 1) ? U.z : U.w;
-  float u = 1.f - b * pd;
-  acc.x += U.x - pd;
-  acc.y = fmaf(U.y, u, acc.y);
-  acc.z = fmaf(U.z, u, acc.z);
-  acc.w = fmaf(U.w, u, acc.w);
+  const float pd = comp<D>(U);
+  const float u = fmaf(-b, pd, 1.f);
+  fma2(acc.x, acc.y, U.x, U.y, 1.f, u, acc.x, acc.y);
+  fma2(acc.z, acc.w, U.z, U.w, u, u, acc.z, acc.w);
+  acc.x -= pd;
   if (D == 0) acc.y -= a; else if (D == 1) acc.z -= a; else acc.w -= a;
 }
 // neighbour on the - side:  U + G_d
 template <int D>
 __device__ __forceinline__ void add_minus(float4& acc, const float4& U, float a, float b)
 {
-  float pd = (D == 0) ? U.y : (D == 1) ? U.z : U.w;
-  float u = 1.f + b * pd;
-  acc.x += U.x + pd;
-  acc.y = fmaf(U.y, u, acc.y);
-  acc.z = fmaf(U.z, u, acc.z);
-  acc.w = fmaf(U.w, u, acc.w);
+  const float pd = comp<D>(U);
+  const float u = fmaf(b, pd, 1.f);
+  fma2(acc.x, acc.y, U.x, U.y, 1.f, u, acc.x, acc.y);
+  fma2(acc.z, acc.w, U.z, U.w, u, u, acc.z, acc.w);
+  acc.x += pd;
   if (D == 0) acc.y += a; else if (D == 1) acc.z += a; else acc.w += a;
 }
+// the same, starting a fresh accumulator (no add of the old value)
+__device__ __forceinline__ float4 below_z(const float4& U, float a, float b)
+{
+  const float u = fmaf(b, U.w, 1.f);
+  float4 r;
+  r.x = U.x + U.w;
+  r.y = U.y * u;
+  mul2(r.z, r.w, U.z, U.w, u, u);
+  r.w += a;
+  return r;
+}
 
-__global__ void __launch_bounds__(TX* TY, 2)
+
+// One plane of the z pipeline held in registers: my two cells (raw U and closure) and my halo cell.
+struct Slot {
+  float4 u0, u1, h;
+  float a0, b0, a1, b1;
+};
+
+struct Tile {                                  // per-thread constants of the march
+  int tx, ly, hsx, hsy;
+  bool act0, act1, pair, hduty;
+  float hsgn_y, hsgn_z;
+};
+
+// DIAG: chemistry is off, so this pass owns the step's photon total and non-finite scan.
+// OPEN: some face is transmissive, so the pass sums the outflow of A15.
+template <bool DIAG, bool OPEN>
+__global__ void __launch_bounds__(NT, 2)
 transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4* __restrict__ Uout,
                  Partial* __restrict__ parts)
 {
-  __shared__ float4 sU[2][SH][SW];
-  __shared__ float2 sAB[2][SH][SW];
+  __shared__ float4 sU[3][SH][SW];
+  __shared__ float2 sAB[3][SH][SW];
 
   const int n = p.n;
   // block -> (tile x, tile y, z chunk, group), tile x fastest so that concurrently resident CTAs are neighbours
@@ -96,147 +152,204 @@ transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4
   const int tiy = bid % p.tiles_y; bid /= p.tiles_y;
   const int izc = bid % p.nzc;     bid /= p.nzc;
   const int g = bid;
-  const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
   const int x0 = tix * TX, y0 = tiy * TY;
   const int wx = min(TX, n - x0), wy = min(TY, n - y0);
   const int z0 = izc * p.zchunk, z1 = min(n, z0 + p.zchunk);
-  const bool active = (tx < wx) && (ty < wy);
-  const int x = x0 + tx, y = y0 + ty;
+  Tile T;
+  T.tx = threadIdx.x % TX;
+  T.ly = CY * (threadIdx.x / TX);              // first of my two rows inside the tile
+  T.pair = T.ly + 1 < wy;                      // warp-uniform: both of my rows are inside the tile
+  T.act0 = (T.tx < wx) && (T.ly < wy);
+  T.act1 = (T.tx < wx) && T.pair;
+  const int x = x0 + T.tx, y = y0 + T.ly;
   const size_t plane = (size_t)n * n;
   const float4* __restrict__ Ug = Uin + (size_t)g * plane * n;
-  float4* __restrict__ Vg = Uout + (size_t)g * plane * n;
-  const size_t col = active ? ((size_t)y * n + x) : 0;
+  const size_t col0 = T.act0 ? ((size_t)y * n + x) : 0;
+  const size_t col1 = T.act1 ? col0 + n : col0;
 
   // halo duty: thread t < 2*wy + 2*wx also stages one halo cell per plane
   const int t = threadIdx.x;
-  const bool hduty = t < 2 * wy + 2 * wx;
-  int hsx = 0, hsy = 0, hflipc = 0;            // shared coords of my halo cell; component to flip (1..2) or 0
+  T.hduty = t < 2 * wy + 2 * wx;
+  T.hsx = 0; T.hsy = 0;
+  int hflipc = 0;                              // component of the halo cell to flip (1..2) or 0
   size_t hcol = 0;
-  if (hduty) {
+  if (T.hduty) {
     bool fl;
     if (t < 2 * wy) {                          // left / right columns
       const int r = (t < wy) ? t : t - wy;
       const int gx = bc_map((t < wy) ? x0 - 1 : x0 + wx, n, p.bc[0], p.bc[1], fl);
-      hsx = (t < wy) ? 0 : wx + 1; hsy = r + 1;
+      T.hsx = (t < wy) ? 0 : wx + 1; T.hsy = r + 1;
       hcol = (size_t)(y0 + r) * n + gx;
       hflipc = fl ? 1 : 0;
     } else {                                   // bottom / top rows
       const int q = t - 2 * wy;
       const int r = (q < wx) ? q : q - wx;
       const int gy = bc_map((q < wx) ? y0 - 1 : y0 + wy, n, p.bc[2], p.bc[3], fl);
-      hsx = r + 1; hsy = (q < wx) ? 0 : wy + 1;
+      T.hsx = r + 1; T.hsy = (q < wx) ? 0 : wy + 1;
       hcol = (size_t)gy * n + (x0 + r);
       hflipc = fl ? 2 : 0;
     }
   }
+  T.hsgn_y = (hflipc == 1) ? -1.f : 1.f;
+  T.hsgn_z = (hflipc == 2) ? -1.f : 1.f;
 
-  const float nu = p.nu, c0 = p.c0, c1 = p.c1;
+  const float c0 = p.c0, c1 = p.c1;
   Acc acc_d;
 
-  // ---- prologue: planes z0-1 (-> Wm), z0 (-> cur), z0+1 (-> raw next); halo of z0, z0+1
-  bool flz;
-  float4 Wm = make_float4(0, 0, 0, 0);
-  float4 cur = make_float4(0, 0, 0, 0), nxt = make_float4(0, 0, 0, 0), hcur = make_float4(0, 0, 0, 0),
-         hnxt = make_float4(0, 0, 0, 0);
-  float ca = 0, cb = 0;
-  bool nxt_flip = false;
+  // ---- prologue: planes z0-1 (-> W), z0 (-> slot A), z0+1 (-> slot B, raw); halo of z0, z0+1
+  bool flz, fltop;
+  const int zm = bc_map(z0 - 1, n, p.bc[4], p.bc[5], flz);
+  const int ztop = bc_map(z1, n, p.bc[4], p.bc[5], fltop);      // the plane above the chunk (mapped)
+  const float sgtop = fltop ? -1.f : 1.f;
+  const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  Slot A, B, C;
+  A.u0 = A.u1 = A.h = B.u0 = B.u1 = B.h = C.u0 = C.u1 = C.h = zero4;
+  A.a0 = A.b0 = A.a1 = A.b1 = B.a0 = B.b0 = B.a1 = B.b1 = C.a0 = C.b0 = C.a1 = C.b1 = 0.f;
+  float4 W0, W1;
   {
-    const int zm = bc_map(z0 - 1, n, p.bc[4], p.bc[5], flz);
-    if (active) {
-      float4 pm = __ldg(Ug + (size_t)zm * plane + col);
-      if (flz) pm.w = -pm.w;
-      float a, b;
-      closure_ab(pm.x, pm.y, pm.z, pm.w, a, b);
-      add_minus<2>(Wm, pm, a, b);              // Wm = U + G_z of the plane below
-      cur = __ldg(Ug + (size_t)z0 * plane + col);
-      closure_ab(cur.x, cur.y, cur.z, cur.w, ca, cb);
+    const float4* pm = Ug + (size_t)zm * plane;
+    const float4* pc = Ug + (size_t)z0 * plane;
+    const float4* pn = Ug + (size_t)((z0 + 1 < z1) ? z0 + 1 : ztop) * plane;
+    float4 m0 = zero4, m1 = zero4;
+    if (T.act0) { m0 = __ldg(pm + col0); A.u0 = __ldg(pc + col0); B.u0 = __ldg(pn + col0); }
+    if (T.act1) { m1 = __ldg(pm + col1); A.u1 = __ldg(pc + col1); B.u1 = __ldg(pn + col1); }
+    if (T.hduty) {
+      A.h = __ldg(pc + hcol);
+      if (z0 + 1 < z1) B.h = __ldg(pn + hcol);
     }
-    if (hduty) hcur = __ldg(Ug + (size_t)z0 * plane + hcol);
-    const int zn = bc_map(z0 + 1, n, p.bc[4], p.bc[5], nxt_flip);
-    if (active) nxt = __ldg(Ug + (size_t)zn * plane + col);
-    if (hduty && z0 + 1 < z1) hnxt = __ldg(Ug + (size_t)(z0 + 1) * plane + hcol);
+    if (flz) { m0.w = -m0.w; m1.w = -m1.w; }
+    float a, b;
+    closure_ab(m0, a, b); W0 = below_z(m0, a, b);
+    closure_ab(m1, a, b); W1 = below_z(m1, a, b);
+    closure_ab(A.u0, A.a0, A.b0);
+    closure_ab(A.u1, A.a1, A.b1);
   }
+  // running pointers (own column 0): loads of plane z+2, stores of plane z
+  const float4* pld = Ug + (size_t)(z0 + 2) * plane + col0;
+  const float4* ptop = Ug + (size_t)ztop * plane + col0;
+  float4* pst = Uout + (size_t)g * plane * n + (size_t)z0 * plane + col0;
+  const ptrdiff_t d1 = (ptrdiff_t)(col1 - col0), dh = (ptrdiff_t)hcol - (ptrdiff_t)col0;
+  float sg_nxt = (z0 + 1 == z1) ? sgtop : 1.f;                  // sign of phi_z of the plane held in the next slot
+  int z = z0;
 
-  for (int z = z0; z < z1; z++) {
-    const int buf = z & 1;
-    // (a) stage this plane: own cell and halo cell, each with its closure
-    if (active) {
-      sU[buf][ty + 1][tx + 1] = cur;
-      sAB[buf][ty + 1][tx + 1] = make_float2(ca, cb);
-    }
-    if (hduty) {
-      float4 h = hcur;
-      if (hflipc == 1) h.y = -h.y; else if (hflipc == 2) h.z = -h.z;
+  // one plane: CUR is staged and updated, NXT (already loaded) gets its closure, NEW receives the loads of z+2
+  auto body = [&](Slot& CUR, Slot& NXT, Slot& NEW, const int buf) {
+    // (a) stage this plane: own cells and halo cell, each with its closure
+    if (T.act0) { sU[buf][T.ly + 1][T.tx + 1] = CUR.u0; sAB[buf][T.ly + 1][T.tx + 1] = make_float2(CUR.a0, CUR.b0); }
+    if (T.act1) { sU[buf][T.ly + 2][T.tx + 1] = CUR.u1; sAB[buf][T.ly + 2][T.tx + 1] = make_float2(CUR.a1, CUR.b1); }
+    if (T.hduty) {
+      float4 h = CUR.h;
+      h.y *= T.hsgn_y; h.z *= T.hsgn_z;
       float a, b;
-      closure_ab(h.x, h.y, h.z, h.w, a, b);
-      sU[buf][hsy][hsx] = h;
-      sAB[buf][hsy][hsx] = make_float2(a, b);
+      closure_ab(h, a, b);
+      sU[buf][T.hsy][T.hsx] = h;
+      sAB[buf][T.hsy][T.hsx] = make_float2(a, b);
     }
-    // (b) issue the loads of plane z+2 (consumed two iterations from now)
-    float4 nn = make_float4(0, 0, 0, 0), hnn = make_float4(0, 0, 0, 0);
-    bool nn_flip = false;
+    // (b) issue the loads of plane z+2 (consumed one iteration from now)
+    const bool last2 = (z + 2 >= z1);                           // plane z+2 is the (mapped) plane above the chunk
     if (z + 1 < z1) {
-      const int z2 = bc_map(z + 2, n, p.bc[4], p.bc[5], nn_flip);
-      if (active) nn = __ldg(Ug + (size_t)z2 * plane + col);
-      if (hduty && z + 2 < z1) hnn = __ldg(Ug + (size_t)(z + 2) * plane + hcol);
+      const float4* q = last2 ? ptop : pld;
+      if (T.act0) NEW.u0 = __ldg(q);
+      if (T.act1) NEW.u1 = __ldg(q + d1);
+      if (T.hduty && !last2) NEW.h = __ldg(q + dh);
     }
     // (c) closure of the plane above and its contribution U - G_z
-    float4 acc = Wm;
-    float na = 0, nb = 0;
-    float4 nx = nxt;
-    if (active) {
-      if (nxt_flip) nx.w = -nx.w;
-      closure_ab(nx.x, nx.y, nx.z, nx.w, na, nb);
-      add_plus<2>(acc, nx, na, nb);
-    }
+    float4 acc0 = W0, acc1 = W1;
+    NXT.u0.w *= sg_nxt; NXT.u1.w *= sg_nxt;
+    closure_ab(NXT.u0, NXT.a0, NXT.b0);
+    closure_ab(NXT.u1, NXT.a1, NXT.b1);
+    add_plus<2>(acc0, NXT.u0, NXT.a0, NXT.b0);
+    add_plus<2>(acc1, NXT.u1, NXT.a1, NXT.b1);
+    // the y-neighbour inside the pair
+    if (T.pair) add_plus<1>(acc0, CUR.u1, CUR.a1, CUR.b1);
+    add_minus<1>(acc1, CUR.u0, CUR.a0, CUR.b0);
     __syncthreads();
-    // (d) x / y neighbours from shared memory
-    if (active) {
-      {
-        const float4 u = sU[buf][ty + 1][tx]; const float2 ab = sAB[buf][ty + 1][tx];
-        add_minus<0>(acc, u, ab.x, ab.y);
-      }
-      {
-        const float4 u = sU[buf][ty + 1][tx + 2]; const float2 ab = sAB[buf][ty + 1][tx + 2];
-        add_plus<0>(acc, u, ab.x, ab.y);
-      }
-      {
-        const float4 u = sU[buf][ty][tx + 1]; const float2 ab = sAB[buf][ty][tx + 1];
-        add_minus<1>(acc, u, ab.x, ab.y);
-      }
-      {
-        const float4 u = sU[buf][ty + 2][tx + 1]; const float2 ab = sAB[buf][ty + 2][tx + 1];
-        add_plus<1>(acc, u, ab.x, ab.y);
-      }
-      float4 o;
-      o.x = fmaf(c1, acc.x, c0 * cur.x);
-      o.y = fmaf(c1, acc.y, c0 * cur.y);
-      o.z = fmaf(c1, acc.z, c0 * cur.z);
-      o.w = fmaf(c1, acc.w, c0 * cur.w);
-      Vg[(size_t)z * plane + col] = o;
-      // diagnostics: non-finite scan; N dV total when chemistry is off; outflow through open faces (A15):
-      // transmissive face flux = own F_d (ghost copies the cell), reflective face flux = 0
-      if (!(fabsf(o.x) + fabsf(o.y) + fabsf(o.z) + fabsf(o.w) < __int_as_float(0x7f800000))) acc_d.nonfinite++;
-      if (p.want_total) acc_d.total += (double)o.x;
-      if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cur.y;
-      if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cur.y;
-      if (y == 0 && p.bc[2] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cur.z;
-      if (y == n - 1 && p.bc[3] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cur.z;
-      if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cur.w;
-      if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cur.w;
-      // (e) rotate the z pipeline: this plane becomes the one below
-      Wm = make_float4(0, 0, 0, 0);
-      add_minus<2>(Wm, cur, ca, cb);
-      cur = nx; ca = na; cb = nb;
+    // (d) the other x / y neighbours from shared memory
+    if (!T.pair) {                             // ragged tile: my second row is the halo row
+      const float4 u = sU[buf][T.ly + 2][T.tx + 1]; const float2 ab = sAB[buf][T.ly + 2][T.tx + 1];
+      add_plus<1>(acc0, u, ab.x, ab.y);
     }
-    nxt = nn; nxt_flip = nn_flip;
-    hcur = hnxt; hnxt = hnn;
+    {
+      const float4 u = sU[buf][T.ly + 1][T.tx]; const float2 ab = sAB[buf][T.ly + 1][T.tx];
+      add_minus<0>(acc0, u, ab.x, ab.y);
+    }
+    {
+      const float4 u = sU[buf][T.ly + 1][T.tx + 2]; const float2 ab = sAB[buf][T.ly + 1][T.tx + 2];
+      add_plus<0>(acc0, u, ab.x, ab.y);
+    }
+    {
+      const float4 u = sU[buf][T.ly][T.tx + 1]; const float2 ab = sAB[buf][T.ly][T.tx + 1];
+      add_minus<1>(acc0, u, ab.x, ab.y);
+    }
+    {
+      const float4 u = sU[buf][T.ly + 2][T.tx]; const float2 ab = sAB[buf][T.ly + 2][T.tx];
+      add_minus<0>(acc1, u, ab.x, ab.y);
+    }
+    {
+      const float4 u = sU[buf][T.ly + 2][T.tx + 2]; const float2 ab = sAB[buf][T.ly + 2][T.tx + 2];
+      add_plus<0>(acc1, u, ab.x, ab.y);
+    }
+    {
+      const float4 u = sU[buf][T.ly + 3][T.tx + 1]; const float2 ab = sAB[buf][T.ly + 3][T.tx + 1];
+      add_plus<1>(acc1, u, ab.x, ab.y);
+    }
+    float4 o0, o1;
+    mul2(o0.x, o0.y, CUR.u0.x, CUR.u0.y, c0, c0); mul2(o0.z, o0.w, CUR.u0.z, CUR.u0.w, c0, c0);
+    mul2(o1.x, o1.y, CUR.u1.x, CUR.u1.y, c0, c0); mul2(o1.z, o1.w, CUR.u1.z, CUR.u1.w, c0, c0);
+    fma2(o0.x, o0.y, acc0.x, acc0.y, c1, c1, o0.x, o0.y); fma2(o0.z, o0.w, acc0.z, acc0.w, c1, c1, o0.z, o0.w);
+    fma2(o1.x, o1.y, acc1.x, acc1.y, c1, c1, o1.x, o1.y); fma2(o1.z, o1.w, acc1.z, acc1.w, c1, c1, o1.z, o1.w);
+    if (T.act0) pst[0] = o0;
+    if (T.act1) pst[d1] = o1;
+    if (DIAG) {
+      // non-finite scan and N dV total (chemistry off: no later kernel looks at the field)
+      if (T.act0) {
+        if (!(fabsf(o0.x) + fabsf(o0.y) + fabsf(o0.z) + fabsf(o0.w) < __int_as_float(0x7f800000))) acc_d.nonfinite++;
+        acc_d.total += (double)o0.x;
+      }
+      if (T.act1) {
+        if (!(fabsf(o1.x) + fabsf(o1.y) + fabsf(o1.z) + fabsf(o1.w) < __int_as_float(0x7f800000))) acc_d.nonfinite++;
+        acc_d.total += (double)o1.x;
+      }
+    }
+    if (OPEN) {
+      // outflow through open faces (A15): transmissive face flux = own F_d (ghost copies the cell), reflective = 0
+      if (T.act0) {
+        if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u0.y;
+        if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u0.y;
+        if (y == 0 && p.bc[2] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u0.z;
+        if (y == n - 1 && p.bc[3] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u0.z;
+        if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u0.w;
+        if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u0.w;
+      }
+      if (T.act1) {
+        if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u1.y;
+        if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u1.y;
+        if (y + 1 == n - 1 && p.bc[3] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u1.z;
+        if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u1.w;
+        if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u1.w;
+      }
+    }
+    // (e) this plane becomes the one below
+    W0 = below_z(CUR.u0, CUR.a0, CUR.b0);
+    W1 = below_z(CUR.u1, CUR.a1, CUR.b1);
+    sg_nxt = last2 ? sgtop : 1.f;
+    pld += plane; pst += plane;
+    z++;
+  };
+
+  // the three register slots rotate roles, so the march is unrolled by three (no register moves, static buffers)
+  for (;;) {
+    body(A, B, C, 0); if (z >= z1) break;
+    body(B, C, A, 1); if (z >= z1) break;
+    body(C, A, B, 2); if (z >= z1) break;
   }
 
-  // photons: sums are in units of N; scale by nu dV (outflow = c phi dt dx^2 = nu phi dV) resp. dV
-  acc_d.outflow *= (double)nu * p.dV;
-  acc_d.total *= p.dV;
-  block_reduce_store(acc_d, parts + blockIdx.x);
+  if (DIAG || OPEN) {
+    // photons: sums are in units of N; scale by nu dV (outflow = c phi dt dx^2 = nu phi dV) resp. dV
+    acc_d.outflow *= (double)p.nu * p.dV;
+    acc_d.total *= p.dV;
+    block_reduce_store(acc_d, parts + blockIdx.x);
+  }
 }
 
 }  // namespace
@@ -245,8 +358,14 @@ int launch_transport(const TransportParams& p, const float4* Uin, float4* Uout, 
                      cudaStream_t st)
 {
   const int nblk = p.tiles_x * p.tiles_y * p.nzc * p.G;
-  transport_kernel<<<nblk, TX * TY, 0, st>>>(p, Uin, Uout, parts);
-  *n_parts = nblk;
+  bool open = false;
+  for (int f = 0; f < 6; f++) open = open || (p.bc[f] == EMMA_RT_BC_TRANSMISSIVE);
+  const bool diag = p.want_total != 0;
+  if (diag && open) transport_kernel<true, true><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);
+  else if (diag) transport_kernel<true, false><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);
+  else if (open) transport_kernel<false, true><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);
+  else transport_kernel<false, false><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);
+  *n_parts = (diag || open) ? nblk : 0;
   return 1;
 }
 
