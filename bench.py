@@ -29,6 +29,7 @@ if ROOT not in sys.path:
 METRIC = "cell_group_updates_per_s"
 UNIT = "cell-group updates/s"
 ORACLE_SAMPLE_N = 128
+ORACLE_SAMPLE_STEPS = 16          # ~10-20 s of host time at 128^3 x 3 groups
 
 
 def log(*a):
@@ -43,6 +44,23 @@ def measured_peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(kernel, n):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full summary
+    (profiles/traffic.csv; captured at 512^3) -- None for any other grid size or if no capture is recorded."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if n != 512 or not os.path.exists(p):
+        return None
+    try:
+        import csv
+        val = None
+        for row in csv.DictReader(open(p)):
+            if row["kernel"] == kernel:
+                val = float(row["dram_bytes_per_launch"])          # the last row of a kernel is the current capture
+        return val
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -197,12 +215,7 @@ def run_ours(args):
     roofline = {"kernel": dominant, "bound": "hbm", "achieved": kern[dominant]["GBps"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dominant]["frac"], "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg[dominant]}
-    tfile = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tfile):
-        try:
-            roofline["traffic"] = json.load(open(tfile)).get(dominant)
-        except Exception:
-            pass
+    roofline["traffic"] = ncu_traffic(dominant, n)
 
     # ---------------- transport-only throughput (chemistry = 0), same grid, K steps
     tr = None
@@ -264,10 +277,10 @@ def run_ours(args):
     # ---------------- oracle on the host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.skip_cpu_baseline:
-        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N, 3, 0, args.variant)
+        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N, ORACLE_SAMPLE_STEPS, 0, args.variant)
         cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
-               "sample": "config 5%s recipe at %d^3 x 3 groups, 3 coupled steps from the initial state, fp64 C oracle, "
-                         "OpenMP on all host cores" % (args.variant, ORACLE_SAMPLE_N)}
+               "sample": "config 5%s recipe at %d^3 x 3 groups, %d coupled steps from the initial state, fp64 C oracle, "
+                         "OpenMP on all host cores" % (args.variant, ORACLE_SAMPLE_N, ORACLE_SAMPLE_STEPS)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
