@@ -353,14 +353,27 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   for (int f = 0; f < 6; f++) tp.bc[f] = h->cfg.bc[f];
   tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
   {
-    // z chunks: enough CTAs for ~8 per SM (two waves at 2 CTAs/SM x 4), chunks of at least 8 planes
+    // z chunks.  Every CTA costs (its planes + ~3 planes of prologue) and the SMs hold 2 CTAs each, so the launch
+    // takes ceil(blocks / (2 SMs)) rounds of (zchunk + 3) plane-times: pick the chunk count that minimises that
+    // (at 512^3 x 3 one chunk per column is 1536 CTAs = 5.19 rounds, i.e. 14 % of the last round idle).
     const int per = tp.tiles_x * tp.tiles_y * s.G;
-    int nzc = (h->sm_count * 8 + per - 1) / per;
-    nzc = std::max(1, std::min(nzc, std::max(1, s.n / 8)));
-    while (nzc > 1 && (long long)per * nzc > TRANSPORT_MAX_BLOCKS) nzc--;
-    tp.zchunk = (s.n + nzc - 1) / nzc;
+    const long long slots = 2LL * h->sm_count;
+    int best = 1; double best_cost = 1e300;
+    const int env_nzc = getenv("EMMA_RT_TUNE_NZC") ? atoi(getenv("EMMA_RT_TUNE_NZC")) : 0;
+    for (int nzc = 1; nzc <= std::max(1, s.n / 8); nzc++) {
+      const int zc = (s.n + nzc - 1) / nzc;
+      const int nz = (s.n + zc - 1) / zc;
+      if (nz != nzc) continue;
+      const long long blocks = (long long)per * nz;
+      if (blocks > TRANSPORT_MAX_BLOCKS) break;
+      const double cost = (double)((blocks + slots - 1) / slots) * (zc + 3);
+      if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = nzc; }
+    }
+    if (env_nzc > 0) best = env_nzc;
+    tp.zchunk = (s.n + best - 1) / best;
     tp.nzc = (s.n + tp.zchunk - 1) / tp.zchunk;
     if ((long long)per * tp.nzc > TRANSPORT_MAX_BLOCKS) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+    tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
   }
   tp.want_total = h->cfg.chemistry ? 0 : 1;
   tp.nu = (float)(c * dt / h->dx);

@@ -68,6 +68,7 @@ struct TransportParams {
   int n, G;
   int bc[6];
   int zchunk, nzc, tiles_x, tiles_y;
+  int pf;                  // planes ahead of the march that are prefetched into L2 (0 = off)
   int want_total;          // 1 when chemistry is off: the transport pass also sums N dV
   float nu;                // c_red dt / dx
   float c0, c1;            // 1 - 3 nu and nu / 2, rounded once from fp64
