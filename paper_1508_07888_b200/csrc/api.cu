@@ -113,6 +113,7 @@ struct emma_rt {
   long long launches;
   DiagDev* diag_pinned;
   Profiler prof;
+  TransportMaps tmaps[2];                      // TMA descriptors of U[0], U[1]
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
@@ -212,6 +213,10 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   CUDA_TRY(h, cudaGetDeviceProperties(&prop, cfg->device));
   h->sm_count = prop.multiProcessorCount;
   CUDA_TRY(h, cudaMallocHost((void**)&h->diag_pinned, sizeof(DiagDev)));
+  for (int b = 0; b < 2; b++) {
+    const int r = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps[b]);
+    if (r != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", r);
+  }
 
   // ---- AMR index arrays (a-0: per-level oct arrays with parent / coarse-ancestor / child indices)
   std::vector<std::vector<int>> parent_h(s.nl + 1), child_h(s.nl + 1);
@@ -373,8 +378,10 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
     tp.zchunk = (s.n + best - 1) / best;
     tp.nzc = (s.n + tp.zchunk - 1) / tp.zchunk;
     if ((long long)per * tp.nzc > TRANSPORT_MAX_BLOCKS) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+    tp.nst = getenv("EMMA_RT_TUNE_NST") ? atoi(getenv("EMMA_RT_TUNE_NST")) : 6;
     tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
   }
+  const bool use_tma = getenv("EMMA_RT_TUNE_TMA") ? atoi(getenv("EMMA_RT_TUNE_TMA")) != 0 : true;
   tp.want_total = h->cfg.chemistry ? 0 : 1;
   tp.nu = (float)(c * dt / h->dx);
   tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
@@ -396,7 +403,13 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
     Partial* P = h->parts();
     // 1. coarse transport, old buffer -> new buffer (Jacobi)
     h->prof.begin(EMMA_RT_K_TRANSPORT);
-    h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
+    if (use_tma) {
+      const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+      if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      h->launches += k;
+    } else {
+      h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
+    }
     h->prof.end();
     off += np;
     h->cur = 1 - h->cur;

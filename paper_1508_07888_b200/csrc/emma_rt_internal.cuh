@@ -7,6 +7,7 @@
 //     fraction y = 1-x = -xs (x > 1/2).  Both ends keep full fp32 relative precision;
 //   * energy: eps = e / n0  [erg per hydrogen atom], so T = eps / (1.5 k_B (1+x)).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -68,11 +69,18 @@ struct TransportParams {
   int n, G;
   int bc[6];
   int zchunk, nzc, tiles_x, tiles_y;
+  int nst;                 // stages of the TMA ring (transport_tma.cu)
   int pf;                  // planes ahead of the march that are prefetched into L2 (0 = off)
   int want_total;          // 1 when chemistry is off: the transport pass also sums N dV
   float nu;                // c_red dt / dx
   float c0, c1;            // 1 - 3 nu and nu / 2, rounded once from fp64
   double dV;
+};
+
+// TMA descriptors of one radiation buffer (transport_tma.cu): the tile's own 32 x 16 box, a 32 x 1 halo row, a
+// 1 x 16 halo column
+struct TransportMaps {
+  CUtensorMap main, row, col;
 };
 
 // Optional per-kernel device timing: CUDA events recorded on the handle's stream around every launch of a step.
@@ -105,6 +113,9 @@ struct Profiler {
 // ---- launchers (each returns the number of kernels it launched) ---------------------------------------------
 int launch_transport(const TransportParams& p, const float4* Uin, float4* Uout, Partial* parts, int* n_parts,
                      cudaStream_t st);
+int make_transport_maps(const float4* U, int n, int G, TransportMaps* out);
+int launch_transport_tma(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
+                         int* n_parts, cudaStream_t st);
 int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
                        unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, cudaStream_t st,
                        Profiler* pf);

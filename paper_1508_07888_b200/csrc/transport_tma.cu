@@ -49,14 +49,14 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}"
-      :: "r"(bar), "r"(parity) : "memory");
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
 }
 // one box of a rank-3 tensor (x in floats, y, z' = group * n + z) -> shared memory, completion on an mbarrier
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int cx, int cy, int cz)
@@ -296,3 +296,100 @@ transport_tma_kernel(const TransportParams p, const __grid_constant__ TransportM
     block_reduce_store(acc_d, parts + blockIdx.x);
   }
 }
+
+// ---- host side ---------------------------------------------------------------------------------------------------
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled()
+{
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+constexpr int NST_DEFAULT = 6;
+
+template <int NST>
+size_t smem_bytes() { return (size_t)NST * STAGE_BYTES + 2 * AB_BYTES + 8 * NST; }
+
+template <int NST, bool DIAG, bool BCGEN>
+cudaError_t launch_variant(const TransportParams& p, const TransportMaps& maps, float4* Uout, Partial* parts, int nblk,
+                           cudaStream_t st)
+{
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(transport_tma_kernel<NST, DIAG, BCGEN>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>());
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  transport_tma_kernel<NST, DIAG, BCGEN><<<nblk, NT, smem_bytes<NST>(), st>>>(p, maps, Uout, parts);
+  return cudaSuccess;
+}
+
+template <int NST>
+cudaError_t launch_nst(const TransportParams& p, const TransportMaps& maps, float4* Uout, Partial* parts, int nblk,
+                       bool diag, bool bcgen, cudaStream_t st)
+{
+  if (diag && bcgen) return launch_variant<NST, true, true>(p, maps, Uout, parts, nblk, st);
+  if (diag) return launch_variant<NST, true, false>(p, maps, Uout, parts, nblk, st);
+  if (bcgen) return launch_variant<NST, false, true>(p, maps, Uout, parts, nblk, st);
+  return launch_variant<NST, false, false>(p, maps, Uout, parts, nblk, st);
+}
+
+}  // namespace
+
+// Tensor maps of one radiation buffer U[G][n][n][n] float4, seen as a rank-3 fp32 tensor (4n, n, G n).
+// Returns 0 on success, the CUresult (or -1 when the driver entry point is missing) otherwise.
+int make_transport_maps(const float4* U, int n, int G, TransportMaps* out)
+{
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc) return -1;
+  const cuuint64_t gdim[3] = {(cuuint64_t)4 * n, (cuuint64_t)n, (cuuint64_t)n * G};
+  const cuuint64_t gstr[2] = {(cuuint64_t)16 * n, (cuuint64_t)16 * n * n};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const cuuint32_t box_main[3] = {4 * TX, TY, 1}, box_row[3] = {4 * TX, 1, 1}, box_col[3] = {4, TY, 1};
+  CUresult r;
+  r = enc(&out->main, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)U, gdim, gstr, box_main, estr,
+          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return (int)r;
+  r = enc(&out->row, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)U, gdim, gstr, box_row, estr,
+          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return (int)r;
+  r = enc(&out->col, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)U, gdim, gstr, box_col, estr,
+          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return (int)r;
+}
+
+int launch_transport_tma(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
+                         int* n_parts, cudaStream_t st)
+{
+  const int nblk = p.tiles_x * p.tiles_y * p.nzc * p.G;
+  bool bcgen = false;
+  for (int f = 0; f < 6; f++) bcgen = bcgen || (p.bc[f] != EMMA_RT_BC_PERIODIC);
+  const bool diag = p.want_total != 0;
+  cudaError_t e;
+  switch (p.nst) {
+    case 4: e = launch_nst<4>(p, maps_in, Uout, parts, nblk, diag, bcgen, st); break;
+    case 8: e = launch_nst<8>(p, maps_in, Uout, parts, nblk, diag, bcgen, st); break;
+    default: e = launch_nst<NST_DEFAULT>(p, maps_in, Uout, parts, nblk, diag, bcgen, st); break;
+  }
+  *n_parts = (diag || bcgen) ? nblk : 0;
+  return e == cudaSuccess ? 1 : 0;
+}
+
+}  // namespace emma
