@@ -17,6 +17,8 @@
 // rule, are appended to a queue with one warp-aggregated atomic and left untouched.  `chem_tail_kernel` then runs
 // persistent warps over that (compacted) queue: each lane owns one queued cell, advances it one accepted sub-step
 // per loop trip and refills from the queue as soon as its cell is done, so lanes stay busy while any work is left.
+#include <stdlib.h>
+
 #include "emma_rt_internal.cuh"
 
 namespace emma {
@@ -314,6 +316,160 @@ chem_main_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, 
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// level 0, pass 1, bulk-async variant: the same arithmetic, but the inputs of a chunk of 256 cells (G float4 runs of
+// 4 KB and the n0, xs, eps runs of 1 KB) are brought into a ring of shared-memory stages by cp.async.bulk copies that
+// complete on mbarriers, NSTC-1 chunks ahead of the compute and at no register cost.  chem_main_kernel keeps ~60 B per
+// thread in flight and waits on long-scoreboard stalls (profiles/r1b_summary.md: 14 of 18.5 cycles per issue).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int CH = 256;                                               // cells per chunk = threads per CTA
+constexpr int NSTC = 4;                                               // stages of the ring
+template <int G> constexpr int chem_stage_bytes() { return CH * 16 * G + CH * 4 * 3; }
+template <int G> constexpr int chem_smem_bytes() { return NSTC * chem_stage_bytes<G>() + 8 * NSTC; }
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar)
+{
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+template <int G>
+__global__ void __launch_bounds__(CH)
+chem_main_bulk_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, long long ncell,
+                      int* __restrict__ queue, unsigned int* __restrict__ qcount, Partial* __restrict__ parts)
+{
+  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr int SB = chem_stage_bytes<G>();
+  const unsigned stage0 = (unsigned)__cvta_generic_to_shared(smem);
+  const unsigned bar0 = stage0 + NSTC * SB;
+  const int t = threadIdx.x, lane = t & 31;
+  const long long nchunks = (ncell + CH - 1) / CH;
+
+  // chunk i of this CTA -> stage s (arrays are 256-byte padded in the arena, so a ragged last run may be rounded
+  // up to the 16-byte granularity of the copy)
+  auto issue = [&](long long i, int s) {
+    const long long chunk = blockIdx.x + i * gridDim.x;
+    if (chunk >= nchunks) return;
+    const long long base = chunk * CH;
+    const unsigned cnt = (unsigned)min((long long)CH, ncell - base);
+    const unsigned bU = cnt * 16u, bF = (cnt * 4u + 15u) & ~15u;
+    const unsigned dst = stage0 + s * SB, bar = bar0 + 8 * s;
+    mbar_expect_tx(bar, G * bU + 3 * bF);
+#pragma unroll
+    for (int g = 0; g < G; g++) bulk_load(dst + g * CH * 16, U + (size_t)g * ncell + base, bU, bar);
+    bulk_load(dst + G * CH * 16, L.n0 + base, bF, bar);
+    bulk_load(dst + G * CH * 16 + CH * 4, L.xs + base, bF, bar);
+    bulk_load(dst + G * CH * 16 + CH * 8, L.eps + base, bF, bar);
+  };
+  if (t == 0) {
+    for (int s = 0; s < NSTC; s++) mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (t == 0)
+    for (int s = 0; s < NSTC; s++) issue(s, s);
+
+  Acc acc;
+  int s = 0;
+  unsigned par = 0;
+  for (long long i = 0;; i++) {
+    const long long chunk = blockIdx.x + i * gridDim.x;
+    if (chunk >= nchunks) break;
+    const long long cell = chunk * CH + t;
+    bool valid = cell < ncell;
+    if (valid && L.refined) valid = !((L.refined[cell >> 5] >> (cell & 31)) & 1u);   // split cells: CRTA kernels
+    mbar_wait(bar0 + 8 * s, par);
+    CellState<G> c;
+    {
+      const unsigned char* st = smem + s * SB;
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        const float4 u = *(const float4*)(st + g * CH * 16 + t * 16);
+        c.N[g] = u.x; c.px[g] = u.y; c.py[g] = u.z; c.pz[g] = u.w;
+      }
+      c.n0 = *(const float*)(st + G * CH * 16 + t * 4);
+      decode_x(*(const float*)(st + G * CH * 16 + CH * 4 + t * 4), c.x, c.y);
+      c.eps = *(const float*)(st + G * CH * 16 + CH * 8 + t * 4);
+    }
+    __syncthreads();                                                  // every thread has taken its cell: refill
+    if (t == 0) issue(i + NSTC, s);
+    if (++s == NSTC) { s = 0; par ^= 1u; }
+    bool defer = false;
+    if (valid) {
+      load_sources<G>(L, cell, c.S);
+      CellTally tl;
+      float dmin = FINF;
+      // fast path == the first trip of the sub-cycle loop when it covers the whole step
+      const float T = c.eps * frcp(KB15 * (1.f + c.x));
+      const Rates r = rates_at(T, cp.otsa, c.x, c.n0);
+      bool go = true;
+      if (cp.thermal) {
+        float hsum = 0.f;
+#pragma unroll
+        for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
+        const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
+        const float guess = (d == 0.f) ? cp.dt : fabsf(c.eps / d);
+        go = guess >= cp.dt;
+        if (go) dmin = guess;
+      }
+      float N1[G], iden[G], x1, y1, eps1;
+      if (go) go = attempt<G>(cp, c, r, cp.dt, N1, iden, x1, y1, eps1);
+      if (go) {
+        const float k = c.y * c.n0 * cp.dt;
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);
+          tl.injected = fmaf(c.S[g], cp.dt, tl.injected);
+          c.N[g] = N1[g];
+          c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);
+        }
+        tl.recomb = r.rec * cp.dt;
+        c.x = x1; c.y = y1; c.eps = eps1;
+        tl.nsub = 1;
+        store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
+        fold(acc, tl, c.N, G, L.dV);
+        acc.dtau_min = fminf(acc.dtau_min, dmin);
+        if (!finite_cell<G>(c)) acc.nonfinite++;
+      } else {
+        defer = true;
+      }
+    }
+    // warp-aggregated append of the deferred cells (north_star item 3: warp-level work compaction)
+    const unsigned m = __ballot_sync(0xffffffffu, defer);
+    if (m) {
+      const int leader = __ffs(m) - 1;
+      unsigned b = 0;
+      if (lane == leader) b = atomicAdd(qcount, (unsigned)__popc(m));
+      b = __shfl_sync(0xffffffffu, b, leader);
+      if (defer) {
+        queue[b + __popc(m & ((1u << lane) - 1u))] = (int)cell;
+        acc.ndefer++;
+      }
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // level 0, pass 2: persistent warps over the compacted queue of cells that need real sub-cycling
 // ------------------------------------------------------------------------------------------------------------
 template <int G>
@@ -496,9 +652,26 @@ int chem_level0_G(const ChemParams& cp, const LevelDev& L0, float4* U, long long
   long long want = (ncell + 255) / 256;
   int nb = (int)(want < (long long)sm_count * 8 ? want : (long long)sm_count * 8);
   if (nb > MAX_PART_BLOCKS) nb = MAX_PART_BLOCKS;
-  pf->begin(EMMA_RT_K_CHEM_MAIN);
-  chem_main_kernel<G><<<nb, 256, 0, st>>>(cp, L0, U, ncell, queue, qcount, parts);
-  pf->end();
+  const bool bulk = getenv("EMMA_RT_TUNE_CHEMBULK") ? atoi(getenv("EMMA_RT_TUNE_CHEMBULK")) != 0 : true;
+  if (bulk) {
+    static bool configured = false;
+    if (!configured) {
+      if (cudaFuncSetAttribute(chem_main_bulk_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               chem_smem_bytes<G>()) != cudaSuccess) return 0;
+      configured = true;
+    }
+    static int occ = 0;                                               // persistent CTAs: as many as fit per SM
+    if (!occ && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, chem_main_bulk_kernel<G>, CH, chem_smem_bytes<G>()) != cudaSuccess) return 0;
+    const int per_sm = getenv("EMMA_RT_TUNE_CHEMCTAS") ? atoi(getenv("EMMA_RT_TUNE_CHEMCTAS")) : (occ > 0 ? occ : 1);
+    nb = (int)(want < (long long)sm_count * per_sm ? want : (long long)sm_count * per_sm);
+    pf->begin(EMMA_RT_K_CHEM_MAIN);
+    chem_main_bulk_kernel<G><<<nb, CH, chem_smem_bytes<G>(), st>>>(cp, L0, U, ncell, queue, qcount, parts);
+    pf->end();
+  } else {
+    pf->begin(EMMA_RT_K_CHEM_MAIN);
+    chem_main_kernel<G><<<nb, 256, 0, st>>>(cp, L0, U, ncell, queue, qcount, parts);
+    pf->end();
+  }
   *n_parts = nb;
   if (!cp.thermal) return 1;                                          // isothermal mode never defers
   int nt = sm_count * 8;
