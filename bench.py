@@ -5,8 +5,8 @@
 
 Workload: BASELINE.json config 5 ("throughput sweep"): 512^3 coarse grid x 3 photon groups, lognormal density,
 4096 sources, random x and T, seeded background radiation (variant b, so that transport does not move zeros) --
-`workloads.make_config(5)`.  A "step" is one pass of the whole hot path (transport -> chemistry main -> chemistry
-tail -> diagnostics) over all cells.  `value` = cell-group updates per second, inputs resident in HBM.
+`workloads.make_config(5)`.  A "step" is one pass of the whole hot path (fused transport + chemistry pass -> chemistry
+tail -> diagnostics; with --unfused: transport -> chemistry main -> tail -> diagnostics) over all cells.  `value` = cell-group updates per second, inputs resident in HBM.
 `e2e` = the same metric through the C-ABI with HOST buffers: every step uploads (U, x, T) from pinned host memory
 and reads (U, x, T) back.  N > 1 GPUs: independent replicas, one process per GPU.
 
@@ -166,7 +166,7 @@ def run_ours(args):
     ncell = n ** 3
     log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
 
-    gpu = E.EmmaRT(w, device=dev)
+    gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
     dt = w.dt
     units_per_step = ncell * G
 
@@ -203,7 +203,8 @@ def run_ours(args):
     # per-kernel roofline (algorithmic bytes of DESIGN.md section 7 / live CUDA-event durations)
     peak, peak_src = measured_peaks()
     alg = {"transport": 32.0 * ncell * G,                    # 16 B read + 16 B write per cell-group
-           "chem_main": (32.0 * G + 20.0) * ncell}           # U in/out + n0, x, e in + x, e out per cell
+           "chem_main": (32.0 * G + 20.0) * ncell,           # U in/out + n0, x, e in + x, e out per cell
+           "fused": (32.0 * G + 20.0) * ncell}               # single pass: U in, U out, n0, x, e in, x, e out
     kern = {}
     for k, (kms, cnt) in prof.items():
         if cnt:
@@ -236,7 +237,7 @@ def run_ours(args):
         tr["frac"] = tr["GBps"] / peak
         g2.close()
         torch.cuda.empty_cache()
-        gpu = E.EmmaRT(w, device=dev)
+        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
 
     # ---------------- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
     Ke = max(1, min(K, args.e2e_steps))
@@ -289,6 +290,7 @@ def run_ours(args):
                 "config": {"workload": "BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
                                        "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)),
                            "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
+                           "schedule": "unfused" if args.unfused else "fused",
                            "parallelism": "replicas" if world > 1 else "single"},
                 "roofline": roofline, "kernels": kern, "transport_only": tr, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": int(launches), "clocks": clk,
@@ -308,6 +310,7 @@ def main():
     ap.add_argument("--n", type=int, default=512)
     ap.add_argument("--variant", default="b", choices=["a", "b"])
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--unfused", action="store_true", help="separate transport and chemistry passes")
     ap.add_argument("--skip-transport-only", action="store_true")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -157,8 +157,13 @@ EMMA_RT_API int64_t emma_rt_kernel_launches(const emma_rt* h);                 /
  * nullable) the summed CUDA-event durations and launch counts of the emma_rt_step kernels recorded since the last
  * call, clears them, and switches recording on (enable != 0) or off for the steps that follow.  Off by default. */
 enum { EMMA_RT_K_TRANSPORT = 0, EMMA_RT_K_CHEM_MAIN = 1, EMMA_RT_K_CHEM_TAIL = 2, EMMA_RT_K_CHEM_REFINED = 3,
-       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_COUNT = 6 };
+       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_FUSED = 6, EMMA_RT_K_COUNT = 7 };
 EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out);
+/* Schedule of the coupled step on the unrefined coarse cells (same result up to fp32 rounding order of nothing: both
+ * schedules run the same arithmetic).  fused = 1 (default): ONE pass does the transport update (Eq. 30, 32) and the
+ * first trip of the sub-cycle loop (Eq. 43-48), so the radiation field crosses HBM once per step; fused = 0: a
+ * transport pass followed by a chemistry pass.  Ignored when chemistry = 0.  Returns EMMA_RT_OK or EINVAL. */
+EMMA_RT_API int emma_rt_set_schedule(emma_rt* h, int32_t fused);
 EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */
 EMMA_RT_API void emma_rt_free(emma_rt* h);                                     /* does not free the arena                    */
 

@@ -18,8 +18,8 @@ _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYC
 
 EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources", "emma_rt_dt_cfl", "emma_rt_step",
                     "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
-                    "emma_rt_profile", "emma_rt_last_error", "emma_rt_free"]
-KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other"]
+                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_last_error", "emma_rt_free"]
+KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused"]
 
 
 class EmmaRTError(RuntimeError):
@@ -93,6 +93,8 @@ def lib():
     L.emma_rt_kernel_launches.argtypes = [C.c_void_p]
     L.emma_rt_profile.restype = C.c_int
     L.emma_rt_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    L.emma_rt_set_schedule.restype = C.c_int
+    L.emma_rt_set_schedule.argtypes = [C.c_void_p, C.c_int32]
     L.emma_rt_last_error.restype = C.c_char_p
     L.emma_rt_last_error.argtypes = [C.c_void_p]
     L.emma_rt_free.restype = None
@@ -195,7 +197,7 @@ class EmmaRT:
     """Owns the torch arena and the handle.  `w` is any object with the attributes of workloads.Workload."""
 
     def __init__(self, w, device=0, record_subcycles=0, chemistry=None, thermal=None, otsa=None, bc=None,
-                 max_source_cells=0, stream=None):
+                 max_source_cells=0, stream=None, fused=None):
         import torch
         if not torch.cuda.is_available():
             raise EmmaRTError(ECUDA, "no CUDA device: this library has no CPU fallback")
@@ -218,6 +220,8 @@ class EmmaRT:
         ptr = (self.arena.data_ptr() + 255) // 256 * 256
         rc, self.h = emma_rt_init(self.cfg, w.parent, w.U0, w.n0, w.x, w.T, ptr, nbytes)
         self._check(rc)
+        if fused is not None:
+            self.set_schedule(fused)
         if w.src_pos is not None and len(w.src_pos):
             self._check(emma_rt_set_sources(self.h, w.src_pos, w.src_Q))
 
@@ -240,6 +244,10 @@ class EmmaRT:
 
     def kernel_launches(self):
         return lib().emma_rt_kernel_launches(self.h)
+
+    def set_schedule(self, fused):
+        """fused=1 (default): single-pass transport + chemistry; 0: separate passes."""
+        self._check(lib().emma_rt_set_schedule(self.h, int(fused)))
 
     def profile(self, enable):
         """Per-kernel CUDA-event times [ms] and launch counts since the last call; then switch recording on/off."""

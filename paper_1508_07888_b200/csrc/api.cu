@@ -114,6 +114,7 @@ struct emma_rt {
   DiagDev* diag_pinned;
   Profiler prof;
   TransportMaps tmaps[2];                      // TMA descriptors of U[0], U[1]
+  int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
@@ -203,7 +204,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   make_layout(s, h->lay);
   h->arena = (char*)arena_dev;
   h->st = (cudaStream_t)cfg->stream;
-  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr;
+  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr; h->fused = 1;
   h->prof.st = h->st;
   h->dx = cfg->box_len_cm / s.n;
   *out = h;                                    // returned even on failure so the caller can read last_error
@@ -357,12 +358,11 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   tp.n = s.n; tp.G = s.G;
   for (int f = 0; f < 6; f++) tp.bc[f] = h->cfg.bc[f];
   tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
-  {
-    // z chunks.  Every CTA costs (its planes + ~3 planes of prologue) and the SMs hold 2 CTAs each, so the launch
-    // takes ceil(blocks / (2 SMs)) rounds of (zchunk + 3) plane-times: pick the chunk count that minimises that
-    // (at 512^3 x 3 one chunk per column is 1536 CTAs = 5.19 rounds, i.e. 14 % of the last round idle).
-    const int per = tp.tiles_x * tp.tiles_y * s.G;
-    const long long slots = 2LL * h->sm_count;
+  // z chunks.  Every CTA costs (its planes + ~3 planes of prologue) and the SMs hold `per_sm` CTAs each, so a launch
+  // takes ceil(blocks / (per_sm SMs)) rounds of (zchunk + 3) plane-times: pick the chunk count that minimises that
+  // (at 512^3 x 3 one chunk per column is 1536 CTAs = 5.19 rounds, i.e. 14 % of the last round idle).
+  auto pick_zchunks = [&](TransportParams& q, int per, int per_sm) -> bool {
+    const long long slots = (long long)per_sm * h->sm_count;
     int best = 1; double best_cost = 1e300;
     const int env_nzc = getenv("EMMA_RT_TUNE_NZC") ? atoi(getenv("EMMA_RT_TUNE_NZC")) : 0;
     for (int nzc = 1; nzc <= std::max(1, s.n / 8); nzc++) {
@@ -375,12 +375,13 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
       if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = nzc; }
     }
     if (env_nzc > 0) best = env_nzc;
-    tp.zchunk = (s.n + best - 1) / best;
-    tp.nzc = (s.n + tp.zchunk - 1) / tp.zchunk;
-    if ((long long)per * tp.nzc > TRANSPORT_MAX_BLOCKS) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
-    tp.nst = getenv("EMMA_RT_TUNE_NST") ? atoi(getenv("EMMA_RT_TUNE_NST")) : 6;
-    tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
-  }
+    q.zchunk = (s.n + best - 1) / best;
+    q.nzc = (s.n + q.zchunk - 1) / q.zchunk;
+    return (long long)per * q.nzc <= TRANSPORT_MAX_BLOCKS;
+  };
+  if (!pick_zchunks(tp, tp.tiles_x * tp.tiles_y * s.G, 2)) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+  tp.nst = getenv("EMMA_RT_TUNE_NST") ? atoi(getenv("EMMA_RT_TUNE_NST")) : 6;
+  tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
   const bool use_tma = getenv("EMMA_RT_TUNE_TMA") ? atoi(getenv("EMMA_RT_TUNE_TMA")) != 0 : true;
   tp.want_total = h->cfg.chemistry ? 0 : 1;
   tp.nu = (float)(c * dt / h->dx);
@@ -398,9 +399,40 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
     cp.csigE[g] = (float)(c * (h->cfg.sigma_E[g] * h->cfg.E_mean[g] - h->cfg.sigma_N[g] * E_HI_ERG));
   }
 
+  // fused schedule (fused.cu): all G groups of a tile in one CTA, one CTA per SM
+  const bool fused = h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
+  TransportParams fp = tp;
+  if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+
   for (int step = 0; step < n_steps; step++) {
     int off = 0, np = 0;
     Partial* P = h->parts();
+    if (fused) {
+      // 1+3. transport and the first chemistry trip of every unrefined coarse cell in one pass; then the compacted
+      // tail, then CRTA on the refined cells (they read the U* this pass wrote into their coarse ancestors)
+      float4* U = h->U(1 - h->cur);
+      h->prof.begin(EMMA_RT_K_FUSED);
+      const int k = launch_fused(fp, h->tmaps[h->cur], U, cp, h->lv[0], (int*)(h->arena + h->lay.queue), h->qcount(), P + off, &np, h->st);
+      if (!k) return fail(h, EMMA_RT_ECUDA, "fused launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      h->prof.end();
+      h->launches += k;
+      off += np;
+      h->cur = 1 - h->cur;
+      h->launches += launch_chem_tail(cp, h->lv[0], U, s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(), P + off, &np,
+                                      h->sm_count, h->st, &h->prof);
+      off += np;
+      for (int l = s.nl; l >= 1; l--) {
+        h->prof.begin(EMMA_RT_K_CHEM_REFINED);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->st);
+        h->prof.end();
+        off += np;
+      }
+      h->t_sim += dt;
+      h->prof.begin(EMMA_RT_K_FINALIZE);
+      h->launches += launch_finalize(P, off, h->diag(), h->qcount(), h->t_sim, h->st);
+      h->prof.end();
+      continue;
+    }
     // 1. coarse transport, old buffer -> new buffer (Jacobi)
     h->prof.begin(EMMA_RT_K_TRANSPORT);
     if (use_tma) {
@@ -533,6 +565,14 @@ int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launche
   }
   h->prof.reset();
   h->prof.on = enable != 0;
+  return EMMA_RT_OK;
+}
+
+int emma_rt_set_schedule(emma_rt* h, int32_t fused)
+{
+  if (!h) return EMMA_RT_EINVAL;
+  if (fused != 0 && fused != 1) return fail(h, EMMA_RT_EINVAL, "fused must be 0 or 1");
+  h->fused = fused;
   return EMMA_RT_OK;
 }
 

@@ -9,7 +9,7 @@ _GR = {}
 
 def groups(G):
     if G not in _GR:
-        _GR[G] = blackbody_groups(1.0e5, (13.6, 1000.0) if G == 1 else (13.6, 24.6, 54.4, 1000.0), n_quad=20001)
+        _GR[G] = blackbody_groups(1.0e5, (13.6, 1000.0) if G == 1 else (13.6, 24.6, 54.4, 100.0, 1000.0) if G == 4 else (13.6, 24.6, 54.4, 1000.0), n_quad=20001)
     return _GR[G]
 
 
