@@ -22,6 +22,11 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
 }
+// plain arrive (release): one count of the current phase
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
   unsigned done;

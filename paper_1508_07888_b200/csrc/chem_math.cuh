@@ -190,6 +190,23 @@ __device__ __forceinline__ void load_sources(const LevelDev& L, long long cell, 
   for (int g = 0; g < G; g++) S[g] = L.src_S[(size_t)lo * G + g];
 }
 
+// the same with the cell's word of the source bitmap already loaded
+template <int G>
+__device__ __forceinline__ void load_sources_word(const LevelDev& L, long long cell, unsigned word, float (&S)[G])
+{
+#pragma unroll
+  for (int g = 0; g < G; g++) S[g] = 0.f;
+  if (!((word >> (cell & 31)) & 1u)) return;
+  int lo = 0, hi = L.n_src - 1;
+  const int key = (int)cell;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (L.src_cell[mid] < key) lo = mid + 1; else hi = mid;
+  }
+#pragma unroll
+  for (int g = 0; g < G; g++) S[g] = L.src_S[(size_t)lo * G + g];
+}
+
 template <int G>
 __device__ __forceinline__ void load_cell(const LevelDev& L, long long cell, const float4* __restrict__ U,
                                           long long ustride, long long ucell, CellState<G>& c)

@@ -43,7 +43,7 @@ constexpr int SG = STAGE_ROWS + 2 * COLB;      // one group's plane: what its fi
 constexpr int ABG = SG / 2;                    // its closure plane: float2 (a, b) at half the byte offset of the cell
 
 template <int G> constexpr int fused_nst() { return G == 1 ? 12 : G == 2 ? 8 : G == 3 ? 6 : 4; }
-template <int G> constexpr size_t fused_smem() { return (size_t)fused_nst<G>() * G * SG + 2 * G * ABG + 8 * fused_nst<G>(); }
+template <int G> constexpr size_t fused_smem() { return (size_t)fused_nst<G>() * G * SG + 2 * G * ABG + 8 * (fused_nst<G>() + 1); }
 
 template <int G, bool BCGEN>
 __global__ void __launch_bounds__(NT, 1)
@@ -57,6 +57,10 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   unsigned char* const sAB = smem + NST * STAGE;
   const unsigned bar0 = smem_u32(sAB + 2 * ABP);
   const unsigned stage0 = smem_u32(smem);
+  // "plane done" barrier: a warp arrives when its reads of planes j-1 / j and its closure writes of plane j+1 are
+  // complete; everyone waits for it at the top of the next plane (split-phase: the chemistry runs in between, so the
+  // warps do not have to finish a plane together)
+  const unsigned bar_pl = bar0 + 8 * NST;
 
   const int n = p.n;
   int bid = blockIdx.x;
@@ -116,6 +120,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
 
   if (t == 0) {
     for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 1);
+    mbar_init(bar_pl, NT / 32);
     mbar_fence_init();
   }
   __syncthreads();
@@ -148,19 +153,35 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   stage_closures(smem + STAGE, sAB + ABP, true);
   __syncthreads();
 
-  int s_blw = 0, s_cur = 1, s_nxt = 2 % NST;   // stages of planes j-1, j, j+1
+  int s_old = 0, s_blw = 0, s_cur = 1, s_nxt = 2 % NST;   // stages of planes j-2 (free), j-1, j, j+1
   unsigned par_nxt = (2 / NST) & 1;            // phase parity of plane j+1's stage
   int ab_blw = 0, ab_cur = 1;                  // closure planes of j-1 (reused for j+1) and j
+
+  unsigned pend_m = 0, pend_b = 0;             // deferred cells of the previous plane: ballot, queue base (in flight)
+  int pend_cell = 0;
+  auto flush_deferred = [&]() {
+    if (pend_m) {
+      const unsigned b = __shfl_sync(0xffffffffu, pend_b, __ffs(pend_m) - 1);
+      if ((pend_m >> lane) & 1u) queue[b + __popc(pend_m & ((1u << lane) - 1u))] = pend_cell;
+    }
+  };
 
   for (int j = 0; j < zc; j++) {
     const int z = z0 + j;
     const size_t cell = (size_t)z * plane + (act ? ((size_t)y * n + x) : 0);
     // chemistry inputs of my cell: in flight while the transport arithmetic runs
     float n0v = 1.f, xsv = 0.f, epsv = 1.f;
+    unsigned srcw = 0;
     bool chem = act;
     if (act) {
       n0v = L.n0[cell]; xsv = L.xs[cell]; epsv = L.eps[cell];
+      if (L.n_src) srcw = L.srcmask[cell >> 5];
       if (L.refined) chem = !((L.refined[cell >> 5] >> (cell & 31)) & 1u);            // split cells: CRTA kernels
+    }
+    if (j > 0) {
+      // every warp is done with plane j-2's stage and with the closure plane that now receives plane j+1
+      mbar_wait(bar_pl, (unsigned)(j - 1) & 1u);
+      if (t == 0 && j + NST - 2 <= zc) issue(j + NST - 2, s_old);
     }
     const unsigned char* sb = smem + s_blw * STAGE;
     const unsigned char* sc = smem + s_cur * STAGE;
@@ -217,6 +238,10 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       }
     }
 
+    // my part of planes j-1, j, j+1 is done (release: the closure writes above)
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_pl);
+
     // ---- chemistry: the first trip of the sub-cycle loop when it covers the whole step (as chem_main_kernel)
     bool defer = false;
     if (act) {
@@ -226,7 +251,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       if (chem) {
         c.n0 = n0v; c.eps = epsv;
         decode_x(xsv, c.x, c.y);
-        load_sources<G>(L, (long long)cell, c.S);
+        load_sources_word<G>(L, (long long)cell, srcw, c.S);
         const float T = c.eps * frcp(KB15 * (1.f + c.x));
         r = rates_at(T, cp.otsa, c.x, c.n0);
         if (cp.thermal) {
@@ -265,27 +290,22 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
         defer = chem;
       }
     }
-    // warp-aggregated append of the deferred cells (north_star item 3: warp-level work compaction)
-    const unsigned m = __ballot_sync(0xffffffffu, defer);
-    if (m) {
-      const int leader = __ffs(m) - 1;
-      unsigned b = 0;
-      if (lane == leader) b = atomicAdd(qcount, (unsigned)__popc(m));
-      b = __shfl_sync(0xffffffffu, b, leader);
-      if (defer) {
-        queue[b + __popc(m & ((1u << lane) - 1u))] = (int)cell;
-        acc_d.ndefer++;
-      }
+    // warp-aggregated append of the deferred cells (north_star item 3: warp-level work compaction).  The atomic that
+    // reserves the queue slots is issued here and its result consumed one plane later, off the critical path.
+    flush_deferred();
+    pend_m = __ballot_sync(0xffffffffu, defer);
+    if (pend_m) {
+      if (lane == __ffs(pend_m) - 1) pend_b = atomicAdd(qcount, (unsigned)__popc(pend_m));
+      pend_cell = (int)cell;
+      if (defer) acc_d.ndefer++;
     }
 
-    // plane j-1's stage is free once every thread has passed the barrier; its closure plane now holds plane j+1
-    __syncthreads();
-    if (t == 0 && j + NST - 1 <= zc) issue(j + NST - 1, s_blw);
-    s_blw = s_cur; s_cur = s_nxt;
+    s_old = s_blw; s_blw = s_cur; s_cur = s_nxt;
     if (++s_nxt == NST) { s_nxt = 0; par_nxt ^= 1u; }
     const int ab_nxt = ab_blw;
     ab_blw = ab_cur; ab_cur = ab_nxt;
   }
+  flush_deferred();
 
   acc_d.outflow *= (double)p.nu * p.dV;
   block_reduce_store(acc_d, parts + blockIdx.x);
