@@ -101,32 +101,33 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const int cyb = bc_map(y0 - 1, n, p.bc[2], p.bc[3], fl);
   const int cyt = bc_map(y0 + wy, n, p.bc[2], p.bc[3], fl);
 
-  // plane j (relative to z0; -1 = the plane below, zc = the plane above), all G groups -> stage s
+  // plane j (relative to z0; -1 = the plane below, zc = the plane above), all G groups -> stage s.  The 5 G boxes of a
+  // plane are issued by the first lanes of 5 G different warps (each arrives on the stage's mbarrier with its own
+  // byte count), so that no single warp carries the whole descriptor traffic on the critical path of the plane loop.
+  const int warp = t >> 5;
   auto issue = [&](int j, int s) {
+    if (lane != 0) return;
     const int zz = (j < 0) ? zm : (j >= zc) ? ztop : z0 + j;
     const unsigned bar = bar0 + 8 * s;
-    mbar_expect_tx(bar, STAGE);
-#pragma unroll
-    for (int g = 0; g < G; g++) {
+    for (int b = warp; b < 5 * G; b += NT / 32) {
+      const int g = b / 5, k = b - 5 * g;
       const unsigned dst = stage0 + s * STAGE + g * SG;
       const int zg = g * n + zz;
-      tma_load_3d(dst + ROWB, &maps.main, bar, 4 * x0, y0, zg);
-      tma_load_3d(dst, &maps.row, bar, 4 * x0, cyb, zg);
-      tma_load_3d(dst + TOPROW, &maps.row, bar, 4 * x0, cyt, zg);
-      tma_load_3d(dst + STAGE_ROWS, &maps.col, bar, cxl, y0, zg);
-      tma_load_3d(dst + STAGE_ROWS + COLB, &maps.col, bar, cxr, y0, zg);
+      if (k == 0) { mbar_expect_tx(bar, TY * ROWB); tma_load_3d(dst + ROWB, &maps.main, bar, 4 * x0, y0, zg); }
+      else if (k == 1) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst, &maps.row, bar, 4 * x0, cyb, zg); }
+      else if (k == 2) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst + TOPROW, &maps.row, bar, 4 * x0, cyt, zg); }
+      else if (k == 3) { mbar_expect_tx(bar, COLB); tma_load_3d(dst + STAGE_ROWS, &maps.col, bar, cxl, y0, zg); }
+      else { mbar_expect_tx(bar, COLB); tma_load_3d(dst + STAGE_ROWS + COLB, &maps.col, bar, cxr, y0, zg); }
     }
   };
 
   if (t == 0) {
-    for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 1);
+    for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 5 * G);
     mbar_init(bar_pl, NT / 32);
     mbar_fence_init();
   }
   __syncthreads();
-  if (t == 0) {
-    for (int j = -1; j < NST - 1 && j <= zc; j++) issue(j, j + 1);
-  }
+  for (int j = -1; j < NST - 1 && j <= zc; j++) issue(j, j + 1);
 
   const float c0 = p.c0, c1 = p.c1;
   const size_t plane = (size_t)n * n, ncell = plane * n;
@@ -181,7 +182,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
     if (j > 0) {
       // every warp is done with plane j-2's stage and with the closure plane that now receives plane j+1
       mbar_wait(bar_pl, (unsigned)(j - 1) & 1u);
-      if (t == 0 && j + NST - 2 <= zc) issue(j + NST - 2, s_old);
+      if (j + NST - 2 <= zc) issue(j + NST - 2, s_old);
     }
     const unsigned char* sb = smem + s_blw * STAGE;
     const unsigned char* sc = smem + s_cur * STAGE;

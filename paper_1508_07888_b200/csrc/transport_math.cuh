@@ -28,10 +28,19 @@ __device__ __forceinline__ void mul2(float& dx, float& dy, float ax, float ay, f
 // later, then hits L2 instead of waiting a full DRAM round trip
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
+// d = (x >= lo) ? v : 0 as a predicated select: keeps the closure branch-free (the compiler otherwise branches
+// around the MUFU ops, which chops the march into basic blocks and serialises the shared-memory latencies)
+__device__ __forceinline__ float sel_ge(float x, float lo, float v)
+{
+  float d;
+  asm("{\n\t.reg .pred p;\n\tsetp.ge.f32 p, %1, %2;\n\tselp.f32 %0, %3, 0f00000000, p;\n\t}" : "=f"(d) : "f"(x), "f"(lo), "f"(v));
+  return d;
+}
+
 __device__ __forceinline__ void closure_ab(const float4& U, float& a, float& b)
 {
   // A2: N <= 0 -> f = 0.  A denormal N (light that has just reached a dark cell) counts as 0: rcp.ftz of it is inf.
-  const float rN = (U.x >= 1.1754944e-38f) ? frcp(U.x) : 0.f;
+  const float rN = sel_ge(U.x, 1.1754944e-38f, frcp(U.x));
   const float rx = U.y * rN, ry = U.z * rN, rz = U.w * rN;
   const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
   const float f2 = fminf(f2raw, 1.f);          // A2: f clipped to [0,1]
@@ -39,7 +48,8 @@ __device__ __forceinline__ void closure_ab(const float4& U, float& a, float& b)
   const float q = f2 * frcp(2.f + s);
   a = fmaf(-U.x, q, 0.33333334f * U.x);
   // A1: |F| = 0 -> no n(x)n term; below f^2 = 1e-30 the term (<= f^2 N) is far under fp32 resolution of a
-  b = (f2raw > 1e-30f) ? 3.f * q * rN * frcp(f2raw) : 0.f;
+  // (f2raw is +inf or NaN only for non-finite inputs, which the diagnostics report)
+  b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
 }
 
 // map an index that may be one cell outside [0,n) through the boundary condition of that face (A13)
