@@ -82,9 +82,18 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const int oxp = (tx < wx - 1) ? own + 16 : STAGE_ROWS + COLB + ty * 16;
   const int oym = own - ROWB;
   const int oyp = (ty + 1 < wy) ? own + ROWB : TOPROW + tx * 16;
-  int hoff = -1;                               // halo cell whose closure I compute
-  if (t < 2 * wy) hoff = STAGE_ROWS + ((t < wy) ? t * 16 : COLB + (t - wy) * 16);
-  else if (t < 2 * wy + 2 * wx) { const int q = t - 2 * wy; hoff = (q < wx) ? q * 16 : TOPROW + (q - wx) * 16; }
+  // halo closures: the 2 wy + 2 wx halo cells of each of the G groups are dealt round-robin over the warps (task
+  // h -> warp h % 16, lane h / 16), at most one per thread, so that every warp carries the same extra work
+  int hoff = -1;                               // byte offset (inside a stage) of the halo cell whose closure I compute
+  {
+    const int nh = 2 * wy + 2 * wx, h = (t & 31) * (NT / 32) + (t >> 5);
+    if (h < nh * G) {
+      const int g = h / nh, q = h - g * nh;
+      const int o = (q < wy) ? STAGE_ROWS + q * 16 : (q < 2 * wy) ? STAGE_ROWS + COLB + (q - wy) * 16
+                  : (q < 2 * wy + wx) ? (q - 2 * wy) * 16 : TOPROW + (q - 2 * wy - wx) * 16;
+      hoff = g * SG + o;
+    }
+  }
   float sxm = 1.f, sxp = 1.f, sym = 1.f, syp = 1.f;     // reflective faces: sign of the face-normal flux (A13)
   if (BCGEN) {
     if (tx == 0 && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) sxm = -1.f;
@@ -140,10 +149,11 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       float a, b;
       closure_ab(*(const float4*)(st + g * SG + own), a, b);
       *(float2*)(ab + g * ABG + (own >> 1)) = make_float2(a, b);
-      if (halo && hoff >= 0) {
-        closure_ab(*(const float4*)(st + g * SG + hoff), a, b);
-        *(float2*)(ab + g * ABG + (hoff >> 1)) = make_float2(a, b);
-      }
+    }
+    if (halo && hoff >= 0) {
+      float a, b;
+      closure_ab(*(const float4*)(st + hoff), a, b);
+      *(float2*)(ab + (hoff >> 1)) = make_float2(a, b);
     }
   };
 
@@ -205,14 +215,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       }
       float na, nb;
       closure_ab(un, na, nb);
-      if (!top) {
-        *(float2*)(ABb + g * ABG + (own >> 1)) = make_float2(na, nb);
-        if (hoff >= 0) {
-          float a, b;
-          closure_ab(*(const float4*)(sn + g * SG + hoff), a, b);
-          *(float2*)(ABb + g * ABG + (hoff >> 1)) = make_float2(a, b);
-        }
-      }
+      if (!top) *(float2*)(ABb + g * ABG + (own >> 1)) = make_float2(na, nb);
       float4 acc = below_z(ub, abb.x, abb.y);
       add_plus<2>(acc, un, na, nb);
       // x / y neighbours from the stage of plane j and its closure plane
@@ -239,6 +242,11 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       }
     }
 
+    if (!top && hoff >= 0) {                   // my halo cell of plane j+1 (read by others one plane later)
+      float a, b;
+      closure_ab(*(const float4*)(sn + hoff), a, b);
+      *(float2*)(ABb + (hoff >> 1)) = make_float2(a, b);
+    }
     // my part of planes j-1, j, j+1 is done (release: the closure writes above)
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_pl);
