@@ -38,6 +38,21 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
   } while (!done);
 }
+// the same with a short sleep between polls: for waits on other warps (not on data), where a spinning warp would only
+// take issue slots from the warps it is waiting for
+__device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
+{
+  unsigned done;
+  for (;;) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (done) break;
+    __nanosleep(64);
+  }
+}
 // one box of a rank-3 tensor -> shared memory, completion (bytes) on an mbarrier
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int cx, int cy, int cz)
 {

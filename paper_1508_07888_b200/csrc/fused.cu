@@ -191,7 +191,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
     }
     if (j > 0) {
       // every warp is done with plane j-2's stage and with the closure plane that now receives plane j+1
-      mbar_wait(bar_pl, (unsigned)(j - 1) & 1u);
+      mbar_wait_relaxed(bar_pl, (unsigned)(j - 1) & 1u);
       if (j + NST - 2 <= zc) issue(j + NST - 2, s_old);
     }
     const unsigned char* sb = smem + s_blw * STAGE;
