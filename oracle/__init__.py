@@ -20,6 +20,7 @@ _LIB = os.path.join(_HERE, "libemma_rt_oracle.so")
 MAX_GROUPS = 4
 OK, EINVAL, ENOMEM, ENONFINITE, ECFL, ESUBCYCLE = 0, -1, -2, -4, -6, -7
 F_U, F_N, F_F, F_X, F_T, F_E, F_N0, F_SUBCYCLES, F_XNEUTRAL = range(9)
+FLUX_GLF, FLUX_HLL = 0, 1
 
 
 def build(force=False):
@@ -77,6 +78,12 @@ def lib():
     L.orc_transport_stencil.restype = None
     L.orc_transport_stencil.argtypes = [C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
     L.orc_chem_cell.restype = C.c_int
+    L.orc_transport_stencil_flux.restype = None
+    L.orc_transport_stencil_flux.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
+    L.orc_m1_wavespeeds.restype = None
+    L.orc_m1_wavespeeds.argtypes = [dp, C.c_double, C.c_int, dp, dp]
+    L.orc_set_flux.restype = C.c_int
+    L.orc_set_flux.argtypes = [C.c_void_p, C.c_int]
     L.orc_chem_cell.argtypes = [C.POINTER(Phys), C.c_double, C.c_double, dp, dp, dp, dp, C.POINTER(ChemOut)]
     L.orc_create.restype = C.c_void_p
     L.orc_create.argtypes = [C.c_int, C.POINTER(C.c_int), C.c_int, C.POINTER(Phys), C.c_double, C.c_int,
@@ -140,14 +147,26 @@ def energy(T, x, n0):
     return lib().orc_energy(float(T), float(x), float(n0))
 
 
-def transport_stencil(c, dt, dx, U0, Um, Up):
-    """One cell of Eq. 30+32 from its own state U0[4] and its -/+ neighbours Um[3,4], Up[3,4]."""
+def transport_stencil(c, dt, dx, U0, Um, Up, flux=None):
+    """One cell of Eq. 30+32 from its own state U0[4] and its -/+ neighbours Um[3,4], Up[3,4]
+    (flux = FLUX_HLL: the HLL interface flux of reading A19 instead of Eq. 32)."""
     U0 = np.ascontiguousarray(U0, np.float64)
     Um = np.ascontiguousarray(Um, np.float64)
     Up = np.ascontiguousarray(Up, np.float64)
     out = np.zeros(4)
-    lib().orc_transport_stencil(float(c), float(dt), float(dx), _dp(U0), _dp(Um), _dp(Up), _dp(out))
+    if flux is None:
+        lib().orc_transport_stencil(float(c), float(dt), float(dx), _dp(U0), _dp(Um), _dp(Up), _dp(out))
+    else:
+        lib().orc_transport_stencil_flux(int(flux), float(c), float(dt), float(dx), _dp(U0), _dp(Um), _dp(Up), _dp(out))
     return out
+
+
+def m1_wavespeeds(U, c, d):
+    """(lmin, lmax): extreme eigenvalues of dF~_d/dU of the M1 system in direction d (reading A19)."""
+    U = np.ascontiguousarray(U, np.float64)
+    lo, hi = np.zeros(1), np.zeros(1)
+    lib().orc_m1_wavespeeds(_dp(U), float(c), int(d), _dp(lo), _dp(hi))
+    return float(lo[0]), float(hi[0])
 
 
 def chem_cell(phys, dt, n0, x, e, U, S=None):
@@ -174,7 +193,7 @@ def _ptr_array(arrs):
 class Oracle:
     """Same call shape as the library: init(config, amr, fields) / set_sources / step / read."""
 
-    def __init__(self, w, chemistry=None, thermal=None, otsa=None, bc=None):
+    def __init__(self, w, chemistry=None, thermal=None, otsa=None, bc=None, flux=None):
         L = lib()
         self.w = w
         self.G = w.G
@@ -199,6 +218,8 @@ class Oracle:
                               _ptr_array(n0), _ptr_array(x), _ptr_array(T))
         if not self.h:
             raise ValueError("orc_create failed (invalid arguments or out of memory)")
+        if flux is not None and L.orc_set_flux(self.h, int(flux)) != OK:
+            raise ValueError("orc_set_flux: unknown flux %r" % (flux,))
         if w.src_pos is not None and len(w.src_pos):
             rc = self.set_sources(w.src_pos, w.src_Q)
             if rc != OK:

@@ -82,16 +82,63 @@ static void glf_flux(const double UL[4], const double UR[4], double c, int d, do
   for (int q = 0; q < 4; q++) Fh[q] = 0.5 * (FL[q] + FR[q]) - 0.5 * c * (UR[q] - UL[q]);
 }
 
+/* A19 -- HLL interface flux ("an implementation of the less diffusive HLL flux is also on the way";
+ * nothing else is printed).  Reading: the standard HLL formula on the same flux vectors F~ as Eq. 32,
+ *     F_{i+1/2} = [ l+ F~_L - l- F~_R + l+ l- (U_R - U_L) ] / (l+ - l-),
+ *     l+ = max(0, lmax(U_L), lmax(U_R)),   l- = min(0, lmin(U_L), lmin(U_R)),
+ * with lmin/lmax the extreme eigenvalues of dF~_d/dU for the M1 closure of Eq. 22-23 (A1, A2):
+ *     l(f, mu) = c [ mu f -/+ sqrt( (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) ) ] / xi,   xi = sqrt(4 - 3 f^2),
+ * f as in the closure (clipped to [0,1], N <= 0 -> f = 0), mu = F_d/|F| (0 if |F| = 0).  l+ = -l- = c gives back
+ * Eq. 32.  If l+ - l- = 0 (both cells free-streaming exactly along the face) the flux is (F~_L + F~_R)/2 (= 0 there).
+ * Pinned in tests against the eigenvalues of the finite-difference Jacobian of orc_closure. */
+void orc_m1_wavespeeds(const double U[4], double c, int d, double* lmin, double* lmax)
+{
+  double N = U[0];
+  double Fn = sqrt(U[1] * U[1] + U[2] * U[2] + U[3] * U[3]);
+  double f = 0.0;
+  if (N > 0.0) {
+    f = Fn / (c * N);
+    if (f > 1.0) f = 1.0;
+  }
+  double mu = (Fn > 0.0) ? U[1 + d] / Fn : 0.0;
+  double xi = sqrt(4.0 - 3.0 * f * f);
+  double rad = (2.0 / 3.0) * (xi * xi - xi) + 2.0 * mu * mu * (2.0 - f * f - xi);
+  if (rad < 0.0) rad = 0.0;
+  double r = sqrt(rad);
+  *lmin = c * (mu * f - r) / xi;
+  *lmax = c * (mu * f + r) / xi;
+}
+
+static void hll_flux(const double UL[4], const double UR[4], double c, int d, double Fh[4])
+{
+  double FL[4], FR[4], aL, bL, aR, bR;
+  flux_vector(UL, c, d, FL);
+  flux_vector(UR, c, d, FR);
+  orc_m1_wavespeeds(UL, c, d, &aL, &bL);
+  orc_m1_wavespeeds(UR, c, d, &aR, &bR);
+  double lp = fmax(0.0, fmax(bL, bR)), lm = fmin(0.0, fmin(aL, aR));
+  if (lp - lm <= 0.0) {
+    for (int q = 0; q < 4; q++) Fh[q] = 0.5 * (FL[q] + FR[q]);
+    return;
+  }
+  for (int q = 0; q < 4; q++) Fh[q] = (lp * FL[q] - lm * FR[q] + lp * lm * (UR[q] - UL[q])) / (lp - lm);
+}
+
+static void face_flux(int flux, const double UL[4], const double UR[4], double c, int d, double Fh[4])
+{
+  if (flux == ORC_FLUX_HLL) hll_flux(UL, UR, c, d, Fh); else glf_flux(UL, UR, c, d, Fh);
+}
+
 /* Eq. 30 summed over the three directions (A4: unsplit).  faceN[2d], faceN[2d+1] receive the N-component
  * of the flux through the -d and +d faces (used for the boundary-outflow diagnostic, A15). */
-static void transport_core(double c, double dt, double dx, const double U0[4], const double Um[3][4],
+static void transport_core(int flux, double c, double dt, double dx, const double U0[4], const double Um[3][4],
                            const double Up[3][4], double out[4], double faceN[6])
 {
   for (int q = 0; q < 4; q++) out[q] = U0[q];
   for (int d = 0; d < 3; d++) {
     double Fm[4], Fp[4];
-    glf_flux(Um[d], U0, c, d, Fm);     /* F_{i-1/2} */
-    glf_flux(U0, Up[d], c, d, Fp);     /* F_{i+1/2} */
+    face_flux(flux, Um[d], U0, c, d, Fm);     /* F_{i-1/2} */
+    face_flux(flux, U0, Up[d], c, d, Fp);     /* F_{i+1/2} */
     for (int q = 0; q < 4; q++) out[q] += (dt / dx) * (Fm[q] - Fp[q]);
     if (faceN) { faceN[2 * d] = Fm[0]; faceN[2 * d + 1] = Fp[0]; }
   }
@@ -100,7 +147,13 @@ static void transport_core(double c, double dt, double dx, const double U0[4], c
 void orc_transport_stencil(double c, double dt, double dx, const double U0[4], const double Um[3][4],
                            const double Up[3][4], double out[4])
 {
-  transport_core(c, dt, dx, U0, Um, Up, out, 0);
+  transport_core(ORC_FLUX_GLF, c, dt, dx, U0, Um, Up, out, 0);
+}
+
+void orc_transport_stencil_flux(int flux, double c, double dt, double dx, const double U0[4], const double Um[3][4],
+                                const double Up[3][4], double out[4])
+{
+  transport_core(flux, c, dt, dx, U0, Um, Up, out, 0);
 }
 
 /* ------------------------------------------------------------------------------------------------
@@ -241,6 +294,7 @@ int orc_chem_cell(const orc_phys* ph, double dt, double n0, double* x_io, double
  * ---------------------------------------------------------------------------------------------- */
 struct orc {
   int n, chemistry;
+  int flux;                        /* ORC_FLUX_GLF (Eq. 32) or ORC_FLUX_HLL (A19) */
   int bc[6];
   orc_phys ph;
   double L, dx;
@@ -259,6 +313,13 @@ struct orc {
   int64_t cnt_transport_cells[8];  /* cells swept by the transport engine, per level (CRTA: level 0 only) */
   int64_t cnt_chem_cells[8];       /* leaf cells swept by the chemistry engine, per level */
 };
+
+int orc_set_flux(orc* o, int flux)
+{
+  if (!o || (flux != ORC_FLUX_GLF && flux != ORC_FLUX_HLL)) return ORC_EINVAL;
+  o->flux = flux;
+  return ORC_OK;
+}
 
 int orc_threads(void)
 {
@@ -515,7 +576,7 @@ int orc_step(orc* o, double dt, int n_steps, orc_diag* diag)
               neighbour(o, Ug, i, j, k, d, -1, Um[d]);
               neighbour(o, Ug, i, j, k, d, +1, Up[d]);
             }
-            transport_core(c, dt, dx, Ug + 4 * id, Um, Up, Vg + 4 * id, faceN);
+            transport_core(o->flux, c, dt, dx, Ug + 4 * id, Um, Up, Vg + 4 * id, faceN);
             /* net photon flux through non-periodic box faces (A15) */
             int idx[3] = {i, j, k};
             for (int d = 0; d < 3; d++) {

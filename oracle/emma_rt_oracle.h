@@ -23,6 +23,7 @@ enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ENONFINITE = -4, ORC_EC
 enum { ORC_BC_PERIODIC = 0, ORC_BC_TRANSMISSIVE = 1, ORC_BC_REFLECTIVE = 2 };          /* PAPER.md:436 */
 enum { ORC_F_U = 0, ORC_F_N = 1, ORC_F_F = 2, ORC_F_X = 3, ORC_F_T = 4, ORC_F_E = 5, ORC_F_N0 = 6,
        ORC_F_SUBCYCLES = 7, ORC_F_XNEUTRAL = 8 };
+enum { ORC_FLUX_GLF = 0, ORC_FLUX_HLL = 1 };        /* Eq. 32 (PAPER.md:246) / reading A19 (PAPER.md:250) */
 #define ORC_MAX_SUBSTEPS 65535       /* accepted sub-steps per cell per step before ORC_ESUBCYCLE */
 
 /* physics parameters of the chemistry (PAPER.md:254-312) */
@@ -66,6 +67,11 @@ double orc_energy(double T, double x, double n0);
 /* Eq. 30 + 32, unsplit 3-D, for one cell from its six face neighbours (ghosts already applied) */
 void   orc_transport_stencil(double c, double dt, double dx, const double U0[4],
                              const double Um[3][4], const double Up[3][4], double out[4]);
+/* the same with the interface flux chosen: ORC_FLUX_GLF (Eq. 32) or ORC_FLUX_HLL (reading A19) */
+void   orc_transport_stencil_flux(int flux, double c, double dt, double dx, const double U0[4],
+                                  const double Um[3][4], const double Up[3][4], double out[4]);
+/* extreme eigenvalues of dF~_d/dU of the M1 system in direction d (reading A19) */
+void   orc_m1_wavespeeds(const double U[4], double c, int d, double* lmin, double* lmax);
 /* Eq. 43-48 sub-cycled over dt for one cell (reading A9).  U is [G][4], S is [G] (may be NULL). */
 int    orc_chem_cell(const orc_phys* ph, double dt, double n0, double* x, double* e, double* U,
                      const double* S, orc_chem_out* out);
@@ -75,6 +81,7 @@ orc* orc_create(int n, const int bc[6], int chemistry, const orc_phys* ph, doubl
                 int n_levels, const int64_t* n_octs, const int64_t* const* parent,
                 const float* const* U0, const float* const* n0, const float* const* x, const float* const* T);
 int  orc_set_sources(orc*, int64_t n_src, const double* pos_box, const double* Q);
+int  orc_set_flux(orc*, int flux);          /* interface flux of the transport sweep; default ORC_FLUX_GLF */
 int  orc_step(orc*, double dt, int n_steps, orc_diag* diag_last);
 int  orc_read(const orc*, int field, int level, int group, double* dst, int64_t n_dst);
 int64_t orc_level_cells(const orc*, int level);

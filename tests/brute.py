@@ -86,3 +86,40 @@ def chem_cell(U, n0, x, e, S, dt, c, sigN, sigE, Emean, otsa=1, e_tol=0.1):
         nacc += 1
         rem = 0.0 if dtau >= rem else rem - dtau
     return U, x, e, nacc, nhalv
+
+
+def wavespeeds(U, c, d):
+    """Extreme eigenvalues of the M1 flux Jacobian in direction d (reading A19), in the cancellation-free
+    form  l = c [r_d -/+ sqrt(R_d)] / xi,  r_d = F_d/(cN) (scaled by 1/f_raw if f_raw > 1),
+    R_d = 2 (1 - f^2) (xi - 3 r_d^2 / (2 + xi)) / (xi + 1)  -- algebraically the textbook radicand
+    (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) with mu f = r_d and (2 - xi)/f^2 = 3/(2 + xi)."""
+    N = U[..., 0]
+    F = U[..., 1:]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        r = np.where(N[..., None] > 0, F / (c * N[..., None]), 0.0)
+    fraw = np.sqrt((r ** 2).sum(-1))
+    r = r / np.maximum(fraw, 1.0)[..., None]
+    f2 = np.minimum(fraw, 1.0) ** 2
+    xi = np.sqrt(4 - 3 * f2)
+    rd = r[..., d]
+    R = np.maximum(2 * (1 - f2) * (xi - 3 * rd * rd / (2 + xi)) / (xi + 1), 0.0)
+    return c * (rd - np.sqrt(R)) / xi, c * (rd + np.sqrt(R)) / xi
+
+
+def transport_periodic_hll(U, c, dt, dx):
+    """U: [nz, ny, nx, 4] fp64, periodic; Eq. 30 with the HLL interface flux of reading A19, face by face."""
+    P = pressure(U, c)
+    out = U.copy()
+    for d, axis in ((0, 2), (1, 1), (2, 0)):
+        Ft = np.empty_like(U)
+        Ft[..., 0] = U[..., 1 + d]
+        Ft[..., 1:] = c * c * P[..., d, :]
+        lo, hi = wavespeeds(U, c, d)
+        up = lambda a: np.roll(a, -1, axis=axis)      # value of the right cell of the face i+1/2
+        lp = np.maximum(0.0, np.maximum(hi, up(hi)))[..., None]
+        lm = np.minimum(0.0, np.minimum(lo, up(lo)))[..., None]
+        den = lp - lm
+        with np.errstate(divide="ignore", invalid="ignore"):
+            Fh = np.where(den > 0, (lp * Ft - lm * up(Ft) + lp * lm * (up(U) - U)) / den, 0.5 * (Ft + up(Ft)))
+        out -= dt / dx * (Fh - np.roll(Fh, +1, axis=axis))
+    return out

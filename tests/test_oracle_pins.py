@@ -492,3 +492,176 @@ def test_thread_count_does_not_change_results(oracle_mod):
         outs.append(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True,
                                    cwd=os.path.dirname(os.path.dirname(__file__)), check=True).stdout)
     assert outs[0] == outs[1]
+
+
+# ------------------------------------------------------------------------------------------------------------
+# HLL interface flux (PAPER.md:250 names it, prints nothing: DESIGN.md reading A19)
+# ------------------------------------------------------------------------------------------------------------
+def _flux_vec(U, c, d):
+    P = O.closure(U, c)
+    return np.array([U[1 + d], c * c * P[d, 0], c * c * P[d, 1], c * c * P[d, 2]])
+
+
+def test_H1_wavespeeds_are_the_extreme_eigenvalues_of_the_flux_jacobian(oracle_mod):
+    """lmin/lmax of A19 against the eigenvalues of a central-difference Jacobian of F~_d(U) built from orc_closure:
+    the mathematics (the closure of Eq. 22-23) fixes them, whatever formula the oracle uses."""
+    rng = np.random.default_rng(19)
+    c = 1.0
+    worst = 0.0
+    for _ in range(300):
+        f = rng.uniform(0.0, 0.995)
+        dirn = rng.standard_normal(3)
+        dirn /= np.linalg.norm(dirn)
+        U = np.array([1.0, *(f * c * dirn)])
+        for d in range(3):
+            J = np.zeros((4, 4))
+            h = 1e-6
+            for k in range(4):
+                e = np.zeros(4)
+                e[k] = h
+                J[:, k] = (_flux_vec(U + e, c, d) - _flux_vec(U - e, c, d)) / (2 * h)
+            ev = np.linalg.eigvals(J)
+            assert np.abs(ev.imag).max() < 1e-6                       # hyperbolic
+            lo, hi = O.m1_wavespeeds(U, c, d)
+            worst = max(worst, abs(ev.real.min() - lo), abs(ev.real.max() - hi))
+    assert worst < 2e-7, worst
+
+
+def test_H2_wavespeed_limits_and_scaling(oracle_mod):
+    c = C_RED
+    lo, hi = O.m1_wavespeeds([2.0, 0, 0, 0], c, 1)
+    assert lo == pytest.approx(-c / math.sqrt(3), rel=1e-14) and hi == pytest.approx(c / math.sqrt(3), rel=1e-14)
+    assert O.m1_wavespeeds([1.0, c, 0, 0], c, 0) == pytest.approx((c, c), rel=1e-14)        # free streaming along d
+    assert O.m1_wavespeeds([1.0, c, 0, 0], c, 2) == pytest.approx((0.0, 0.0), abs=1e-9 * c)  # ... across d
+    assert O.m1_wavespeeds([1.0, -3 * c, 0, 0], c, 0) == pytest.approx((-c, -c), rel=1e-14)  # f clipped to 1
+    assert O.m1_wavespeeds([0.0, 1.0, 0, 0], c, 0) == pytest.approx((-c / math.sqrt(3), c / math.sqrt(3)))  # N<=0: f=0
+    # |l| <= c always, lmin <= lmax, and the pair agrees with the independent cancellation-free transcription
+    rng = np.random.default_rng(3)
+    U = np.concatenate([10 ** rng.uniform(-6, -2, (500, 1)), np.zeros((500, 3))], axis=1)
+    dirn = rng.standard_normal((500, 3))
+    dirn /= np.linalg.norm(dirn, axis=1)[:, None]
+    U[:, 1:] = rng.uniform(0, 1.2, (500, 1)) * c * U[:, :1] * dirn
+    for d in range(3):
+        blo, bhi = brute.wavespeeds(U, c, d)
+        for i in range(500):
+            lo, hi = O.m1_wavespeeds(U[i], c, d)
+            assert -c * (1 + 1e-12) <= lo <= hi <= c * (1 + 1e-12)
+            assert lo == pytest.approx(blo[i], abs=2e-8 * c) and hi == pytest.approx(bhi[i], abs=2e-8 * c)
+
+
+def test_H3_hll_single_cell_worked_example(oracle_mod):
+    """One hot cell in the dark, F = 0: every state has f = 0, so l = -/+ c/sqrt(3) and HLL is Eq. 32 with c/sqrt(3)
+    as its dissipation speed: centre (1 - sqrt(3) nu) N0, face neighbours nu N0/(2 sqrt 3), outward flux nu c N0/6."""
+    n, c = 8, C_RED
+    U0 = np.zeros((1, n ** 3, 4), np.float32)
+    ctr = 3 + n * (4 + n * 2)
+    U0[0, ctr, 0] = 1.0
+    w = tiny_workload(n, 1, U0=U0, chemistry=0)
+    o = O.Oracle(w, flux=O.FLUX_HLL)
+    rc, _ = o.step(w.dt, 1)
+    assert rc == O.OK
+    U = o.read(O.F_U).reshape(n, n, n, 4)
+    nu = c * w.dt / w.dx
+    assert U[2, 4, 3, 0] == pytest.approx(1 - math.sqrt(3) * nu, rel=1e-13)
+    for (dz, dy, dx_), comp in (((0, 0, 1), 1), ((0, 0, -1), 1), ((0, 1, 0), 2), ((0, -1, 0), 2), ((1, 0, 0), 3), ((-1, 0, 0), 3)):
+        v = U[2 + dz, 4 + dy, 3 + dx_]
+        sgn = dz + dy + dx_
+        assert v[0] == pytest.approx(nu / (2 * math.sqrt(3)), rel=1e-13)
+        assert v[comp] == pytest.approx(sgn * nu * c / 6, rel=1e-13)
+        assert np.abs(np.delete(v[1:], comp - 1)).max() == 0.0
+    assert U[..., 0].sum() == pytest.approx(1.0, rel=1e-13)
+
+
+def test_H4_hll_free_streaming_beam_is_exact_upwind(oracle_mod):
+    """F = c N x^ (f = 1 along x): l+ = c, l- = 0, so HLL is first-order upwind: the binomial closed form of P3, F = cN
+    kept, and NOTHING leaks through the transverse faces (l = 0 there)."""
+    n, c, k = 16, 2.0 ** 31, 6                  # power-of-two speed: c N is exact in fp32, so f = 1 exactly (as in P3)
+    rng = np.random.default_rng(5)
+    prof = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    U0 = np.zeros((1, n, n, n, 4), np.float32)
+    U0[0, ..., 0] = prof[None, None, :]
+    U0[0, ..., 1] = np.float32(c) * prof[None, None, :]
+    U0 = U0.reshape(1, n ** 3, 4)
+    w = tiny_workload(n, 1, U0=U0, c_red=c, chemistry=0, courant=0.75)
+    o = O.Oracle(w, flux=O.FLUX_HLL)
+    rc, _ = o.step(w.dt, k)
+    assert rc == O.OK
+    nu = c * w.dt / w.dx
+    p0 = prof.astype(np.float64)
+    expect = sum(comb(k, m) * nu ** m * (1 - nu) ** (k - m) * np.roll(p0, m) for m in range(k + 1))
+    U = o.read(O.F_U).reshape(n, n, n, 4)
+    assert np.allclose(U[3, 7, :, 0], expect, rtol=1e-12)
+    assert np.allclose(U[..., 1], c * U[..., 0], rtol=1e-12) and np.abs(U[..., 2:]).max() == 0.0
+
+
+@pytest.mark.parametrize("n,G,seed", [(4, 1, 0), (6, 3, 1), (8, 2, 2)])
+def test_H5_hll_bruteforce_transcription_and_conservation(oracle_mod, n, G, seed):
+    """Oracle HLL transport vs the independent numpy transcription (tests/brute.py), random states incl. f > 1 and dark
+    cells, 3 steps; sum N conserved to rounding on the periodic box."""
+    rng = np.random.default_rng(200 + seed)
+    nc, c = n ** 3, C_RED
+    U0 = np.zeros((G, nc, 4))
+    for g in range(G):
+        N = 10 ** rng.uniform(-6, -2, nc)
+        N[rng.random(nc) < 0.1] = 0.0
+        d = rng.standard_normal((nc, 3))
+        d /= np.linalg.norm(d, axis=1)[:, None]
+        U0[g, :, 0] = N
+        U0[g, :, 1:] = (rng.uniform(0, 1.1, nc) * c * N)[:, None] * d
+    U0 = U0.astype(np.float32)
+    w = tiny_workload(n, G, U0=U0, chemistry=0)
+    o = O.Oracle(w, flux=O.FLUX_HLL)
+    Ub = U0.astype(np.float64).reshape(G, n, n, n, 4)
+    for _ in range(3):
+        Ub = np.stack([brute.transport_periodic_hll(Ub[g], c, w.dt, w.dx) for g in range(G)])
+    rc, _ = o.step(w.dt, 3)
+    assert rc == O.OK
+    for g in range(G):
+        U = o.read(O.F_U, 0, g).reshape(n, n, n, 4)
+        scale = np.abs(Ub[g][..., 0]).max()
+        assert np.abs(U[..., 0] - Ub[g][..., 0]).max() <= 1e-10 * scale
+        assert np.abs(U[..., 1:] - Ub[g][..., 1:]).max() <= 1e-10 * c * scale
+        assert U[..., 0].sum() == pytest.approx(U0[g, :, 0].astype(np.float64).sum(), rel=1e-12)
+
+
+def test_H6_hll_is_less_diffusive_than_glf(oracle_mod):
+    """HLL is 'less diffusive' than GLF, whose weak shadows come from light leaking sideways.  A beam
+    of finite width along x: after 10 steps the photons found outside the beam's own rows are far fewer with HLL."""
+    n, c = 16, C_RED
+    U0 = np.zeros((1, n, n, n, 4))
+    U0[0, 6:10, 6:10, :, 0] = 1.0
+    U0[0, 6:10, 6:10, :, 1] = c
+    U0 = U0.reshape(1, n ** 3, 4).astype(np.float32)
+    w = tiny_workload(n, 1, U0=U0, chemistry=0)
+    leak = {}
+    for name, fl in (("glf", O.FLUX_GLF), ("hll", O.FLUX_HLL)):
+        o = O.Oracle(w, flux=fl)
+        rc, _ = o.step(w.dt, 10)
+        assert rc == O.OK
+        N = o.read(O.F_N).reshape(n, n, n)
+        inside = N[6:10, 6:10, :].sum()
+        leak[name] = 1.0 - inside / N.sum()
+        assert N.sum() == pytest.approx(16.0 * n, rel=1e-12)
+    assert leak["hll"] < 0.6 * leak["glf"], leak
+
+
+def test_H7_hll_budget_with_open_and_reflective_faces(oracle_mod):
+    """A15 with the HLL flux: photons_total changes by injected - outflow (chemistry off), transmissive + reflective."""
+    n = 8
+    rng = np.random.default_rng(11)
+    U0 = np.zeros((1, n ** 3, 4))
+    U0[0, :, 0] = 10 ** rng.uniform(-5, -3, n ** 3)
+    d = rng.standard_normal((n ** 3, 3))
+    d /= np.linalg.norm(d, axis=1)[:, None]
+    U0[0, :, 1:] = (rng.uniform(0, 0.9, n ** 3) * C_RED * U0[0, :, 0])[:, None] * d
+    w = tiny_workload(n, 1, U0=U0.astype(np.float32), chemistry=0, bc=(1, 1, 2, 2, 1, 2),
+                      src_pos=[[0.5, 0.5, 0.5]], src_Q=[[1e48]])
+    o = O.Oracle(w, flux=O.FLUX_HLL)
+    prev = o.step(w.dt, 0)[1]["photons_total"] if False else float(U0[0, :, 0].astype(np.float32).astype(np.float64).sum() * w.dx ** 3)
+    for _ in range(5):
+        rc, dg = o.step(w.dt, 1)
+        assert rc == O.OK
+        resid = dg["photons_total"] - prev - dg["photons_injected"] + dg["photons_outflow"]
+        assert abs(resid) <= 1e-12 * dg["photons_total"]
+        assert dg["photons_outflow"] != 0.0
+        prev = dg["photons_total"]
