@@ -164,6 +164,13 @@ EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int6
  * first trip of the sub-cycle loop (Eq. 43-48), so the radiation field crosses HBM once per step; fused = 0: a
  * transport pass followed by a chemistry pass.  Ignored when chemistry = 0.  Returns EMMA_RT_OK or EINVAL. */
 EMMA_RT_API int emma_rt_set_schedule(emma_rt* h, int32_t fused);
+/* Interface flux of the transport update (Eq. 30).  EMMA_RT_FLUX_GLF (default): the Lax-Friedrichs / GLF flux of Eq. 32
+ * (PAPER.md:246).  EMMA_RT_FLUX_HLL: the HLL flux the paper names as its less diffusive successor (
+ * DESIGN.md reading A19):  F = [l+ F~_L - l- F~_R + l+ l- (U_R - U_L)] / (l+ - l-),  l+ = max(0, lmax_L, lmax_R),
+ * l- = min(0, lmin_L, lmin_R), lmin/lmax the extreme eigenvalues of the M1 flux Jacobian in the face direction.
+ * With HLL the coupled step runs the two-pass schedule (the fused pass implements Eq. 32 only).  Returns OK / EINVAL. */
+enum { EMMA_RT_FLUX_GLF = 0, EMMA_RT_FLUX_HLL = 1 };
+EMMA_RT_API int emma_rt_set_flux(emma_rt* h, int32_t flux);
 EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */
 EMMA_RT_API void emma_rt_free(emma_rt* h);                                     /* does not free the arena                    */
 

@@ -18,7 +18,8 @@ _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYC
 
 EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources", "emma_rt_dt_cfl", "emma_rt_step",
                     "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
-                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_last_error", "emma_rt_free"]
+                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_last_error", "emma_rt_free"]
+FLUX_GLF, FLUX_HLL = 0, 1
 KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused"]
 
 
@@ -95,6 +96,8 @@ def lib():
     L.emma_rt_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.emma_rt_set_schedule.restype = C.c_int
     L.emma_rt_set_schedule.argtypes = [C.c_void_p, C.c_int32]
+    L.emma_rt_set_flux.restype = C.c_int
+    L.emma_rt_set_flux.argtypes = [C.c_void_p, C.c_int32]
     L.emma_rt_last_error.restype = C.c_char_p
     L.emma_rt_last_error.argtypes = [C.c_void_p]
     L.emma_rt_free.restype = None
@@ -197,7 +200,7 @@ class EmmaRT:
     """Owns the torch arena and the handle.  `w` is any object with the attributes of workloads.Workload."""
 
     def __init__(self, w, device=0, record_subcycles=0, chemistry=None, thermal=None, otsa=None, bc=None,
-                 max_source_cells=0, stream=None, fused=None):
+                 max_source_cells=0, stream=None, fused=None, flux=None):
         import torch
         if not torch.cuda.is_available():
             raise EmmaRTError(ECUDA, "no CUDA device: this library has no CPU fallback")
@@ -222,6 +225,8 @@ class EmmaRT:
         self._check(rc)
         if fused is not None:
             self.set_schedule(fused)
+        if flux is not None:
+            self._check(lib().emma_rt_set_flux(self.h, int(flux)))
         if w.src_pos is not None and len(w.src_pos):
             self._check(emma_rt_set_sources(self.h, w.src_pos, w.src_Q))
 

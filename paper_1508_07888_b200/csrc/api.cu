@@ -115,6 +115,7 @@ struct emma_rt {
   Profiler prof;
   TransportMaps tmaps[2];                      // TMA descriptors of U[0], U[1]
   int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
+  int flux;                                    // interface flux of the transport update (emma_rt_set_flux)
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
@@ -204,7 +205,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   make_layout(s, h->lay);
   h->arena = (char*)arena_dev;
   h->st = (cudaStream_t)cfg->stream;
-  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr; h->fused = 1;
+  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr; h->fused = 1; h->flux = EMMA_RT_FLUX_GLF;
   h->prof.st = h->st;
   h->dx = cfg->box_len_cm / s.n;
   *out = h;                                    // returned even on failure so the caller can read last_error
@@ -400,7 +401,10 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   }
 
   // fused schedule (fused.cu): all G groups of a tile in one CTA, one CTA per SM
-  const bool fused = h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
+  const bool hll = h->flux == EMMA_RT_FLUX_HLL;
+  TransportParams hp = tp;                     // HLL pass (transport_hll.cu): one group per CTA, one CTA per SM
+  if (hll && !pick_zchunks(hp, hp.tiles_x * hp.tiles_y * s.G, hll_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+  const bool fused = !hll && h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
   TransportParams fp = tp;
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
 
@@ -435,7 +439,11 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
     }
     // 1. coarse transport, old buffer -> new buffer (Jacobi)
     h->prof.begin(EMMA_RT_K_TRANSPORT);
-    if (use_tma) {
+    if (hll) {
+      const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+      if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      h->launches += k;
+    } else if (use_tma) {
       const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
       if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
       h->launches += k;
@@ -573,6 +581,14 @@ int emma_rt_set_schedule(emma_rt* h, int32_t fused)
   if (!h) return EMMA_RT_EINVAL;
   if (fused != 0 && fused != 1) return fail(h, EMMA_RT_EINVAL, "fused must be 0 or 1");
   h->fused = fused;
+  return EMMA_RT_OK;
+}
+
+int emma_rt_set_flux(emma_rt* h, int32_t flux)
+{
+  if (!h) return EMMA_RT_EINVAL;
+  if (flux != EMMA_RT_FLUX_GLF && flux != EMMA_RT_FLUX_HLL) return fail(h, EMMA_RT_EINVAL, "unknown flux %d", (int)flux);
+  h->flux = flux;
   return EMMA_RT_OK;
 }
 

@@ -124,6 +124,9 @@ int launch_chem_tail(const ChemParams& cp, const LevelDev& L0, float4* U, long l
 int launch_fused(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, const ChemParams& cp,
                  const LevelDev& L0, int* queue, unsigned int* qcount, Partial* parts, int* n_parts, cudaStream_t st);
 int fused_ctas_per_sm();
+int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
+                         int* n_parts, cudaStream_t st);
+int hll_ctas_per_sm();
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U,
                         long long ncell0, Partial* parts, int* n_parts, cudaStream_t st);
 int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts,

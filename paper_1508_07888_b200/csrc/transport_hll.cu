@@ -1,0 +1,327 @@
+// transport_hll.cu -- explicit M1 transport with the HLL interface flux.
+//
+// PAPER.md:250 names the HLL flux as the less diffusive successor of the GLF flux of Eq. 32 and prints nothing else;
+// DESIGN.md reading A19 fixes it:  Eq. 30 with
+//     H_{i+1/2} = [ l+ G_L - l- G_R + l+ l- (U_R - U_L) ] / (l+ - l-),   l+ = max(0, lmax_L, lmax_R),  l- = min(0, lmin_L, lmin_R),
+// G_d = (phi_d, Pi_d.) the flux vector in the internal variables phi = F/c (units of N), l the extreme eigenvalues of
+// dG_d/dU in units of c:
+//     l(-/+) = [ r_d -/+ sqrt(R_d) ] / xi,   r = phi/N (scaled to |r| = 1 if f > 1),  xi = sqrt(4 - 3 f^2),
+//     R_d = 2 (1 - f^2) (xi - 3 r_d^2 / (2 + xi)) / (xi + 1)
+// -- algebraically the textbook radicand (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) with mu f = r_d and
+// (2 - xi)/f^2 = 3/(2 + xi); this form has no cancellation at f -> 1 and no 0/0 at f -> 0.  l+ = -l- = 1 gives Eq. 32.
+// The update is U' = U - nu sum_d (H_{d+1/2} - H_{d-1/2}).  If l+ = l- (= 0: both cells stream exactly along the face)
+// the flux vectors vanish too and H = 0.
+//
+// Shape: as fused.cu with one group per CTA -- 512 threads own a 32 x 16 column, one cell each, and march along z
+// through a TMA-fed ring of planes (j-1, j, j+1 resident, the rest in flight).  Per cell the closure (a, b) and the six
+// wave speeds are computed ONCE, when its plane lands, and staged in shared memory (32 B per cell); the x/y face
+// fluxes are evaluated from both sides (once per adjacent cell), the z face flux is carried to the next plane.
+#include <cuda.h>
+
+#include "async_copy.cuh"
+#include "emma_rt_internal.cuh"
+#include "transport_math.cuh"
+
+namespace emma {
+
+namespace {
+
+using namespace acp;
+
+constexpr int TX = 32, TY = 16, NT = TX * TY;
+constexpr int ROWB = TX * 16;
+constexpr int TOPROW = (TY + 1) * ROWB;
+constexpr int STAGE_ROWS = (TY + 2) * ROWB;
+constexpr int COLB = TY * 16;
+constexpr int SG = STAGE_ROWS + 2 * COLB;      // bytes of one plane (own 32 x 16 box, 2 halo rows, 2 halo columns)
+constexpr int NST = 8;                         // stages of the ring
+constexpr int AUXB = 2 * SG;                   // aux plane: two float4 per cell at twice the byte offset of the cell
+constexpr size_t SMEM = (size_t)NST * SG + 2 * AUXB + 8 * (NST + 1);
+
+struct Aux {                                   // closure and wave speeds of one cell
+  float a, b;                                  // Pi = a I + b phi (x) phi
+  float lm[3], lp[3];                          // lmin, lmax per direction, in units of c
+};
+
+__device__ __forceinline__ Aux make_aux(const float4& U)
+{
+  Aux A;
+  const float rN = sel_ge(U.x, 1.1754944e-38f, frcp(U.x));           // A2: N <= 0 (or denormal) -> f = 0
+  float rx = U.y * rN, ry = U.z * rN, rz = U.w * rN;
+  const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
+  const float f2 = fminf(f2raw, 1.f);
+  const float xi = fsqrt(fmaf(-3.f, f2, 4.f));
+  const float i2 = frcp(2.f + xi);
+  const float q = f2 * i2;
+  A.a = fmaf(-U.x, q, 0.33333334f * U.x);
+  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
+  if (f2raw > 1.f) { const float s = rsqrtf(f2raw); rx *= s; ry *= s; rz *= s; }   // f clipped to 1: r -> unit vector
+  const float k = 2.f * (1.f - f2) * frcp(xi + 1.f), ixi = frcp(xi), t3 = 3.f * i2;
+  const float sx = fsqrt(fmaxf(k * fmaf(-t3 * rx, rx, xi), 0.f));
+  const float sy = fsqrt(fmaxf(k * fmaf(-t3 * ry, ry, xi), 0.f));
+  const float sz = fsqrt(fmaxf(k * fmaf(-t3 * rz, rz, xi), 0.f));
+  A.lm[0] = (rx - sx) * ixi; A.lp[0] = (rx + sx) * ixi;
+  A.lm[1] = (ry - sy) * ixi; A.lp[1] = (ry + sy) * ixi;
+  A.lm[2] = (rz - sz) * ixi; A.lp[2] = (rz + sz) * ixi;
+  return A;
+}
+
+__device__ __forceinline__ void store_aux(unsigned char* plane, int off, const Aux& A)
+{
+  float4* q = (float4*)(plane + 2 * off);
+  q[0] = make_float4(A.a, A.b, A.lm[0], A.lp[0]);
+  q[1] = make_float4(A.lm[1], A.lp[1], A.lm[2], A.lp[2]);
+}
+
+// flux vector G_d of a cell and the HLL combination for the face between L (towards -d) and R (towards +d)
+template <int D>
+__device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL, float lmL, float lpL,
+                                           const float4& UR, float aR, float bR, float lmR, float lpR)
+{
+  const float pL = comp<D>(UL), pR = comp<D>(UR);
+  const float uL = bL * pL, uR = bR * pR;
+  float4 GL = make_float4(pL, uL * UL.y, uL * UL.z, uL * UL.w);
+  float4 GR = make_float4(pR, uR * UR.y, uR * UR.z, uR * UR.w);
+  if (D == 0) { GL.y += aL; GR.y += aR; } else if (D == 1) { GL.z += aL; GR.z += aR; } else { GL.w += aL; GR.w += aR; }
+  const float lp = fmaxf(0.f, fmaxf(lpL, lpR)), lm = fminf(0.f, fminf(lmL, lmR));
+  const float den = lp - lm;
+  const float inv = (den > 0.f) ? frcp(den) : 0.f;
+  const float wl = lp * inv, wr = -lm * inv, wd = lp * lm * inv;
+  float4 H;
+  H.x = fmaf(wl, GL.x, fmaf(wr, GR.x, wd * (UR.x - UL.x)));
+  H.y = fmaf(wl, GL.y, fmaf(wr, GR.y, wd * (UR.y - UL.y)));
+  H.z = fmaf(wl, GL.z, fmaf(wr, GR.z, wd * (UR.z - UL.z)));
+  H.w = fmaf(wl, GL.w, fmaf(wr, GR.w, wd * (UR.w - UL.w)));
+  return H;
+}
+
+// DIAG: chemistry is off, so this pass owns the step's photon total and non-finite scan.
+// BCGEN: some face is not periodic (outflow sums and the reflective signs are compiled in).
+template <bool DIAG, bool BCGEN>
+__global__ void __launch_bounds__(NT, 1)
+transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps, float4* __restrict__ Uout,
+                     Partial* __restrict__ parts)
+{
+  extern __shared__ __align__(128) unsigned char smem[];
+  unsigned char* const sAUX = smem + NST * SG;
+  const unsigned bar0 = smem_u32(sAUX + 2 * AUXB);
+  const unsigned bar_pl = bar0 + 8 * NST;      // split-phase "plane done" barrier (see fused.cu)
+  const unsigned stage0 = smem_u32(smem);
+
+  const int n = p.n;
+  int bid = blockIdx.x;
+  const int tix = bid % p.tiles_x; bid /= p.tiles_x;
+  const int tiy = bid % p.tiles_y; bid /= p.tiles_y;
+  const int izc = bid % p.nzc;     bid /= p.nzc;
+  const int g = bid;
+  const int x0 = tix * TX, y0 = tiy * TY;
+  const int wx = min(TX, n - x0), wy = min(TY, n - y0);
+  const int z0 = izc * p.zchunk, z1 = min(n, z0 + p.zchunk);
+  const int zc = z1 - z0;
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int tx = t % TX, ty = t / TX;
+  const int x = x0 + tx, y = y0 + ty;
+  const bool act = (tx < wx) && (ty < wy);
+
+  const int own = (ty + 1) * ROWB + tx * 16;
+  const int oxm = (tx > 0) ? own - 16 : STAGE_ROWS + ty * 16;
+  const int oxp = (tx < wx - 1) ? own + 16 : STAGE_ROWS + COLB + ty * 16;
+  const int oym = own - ROWB;
+  const int oyp = (ty + 1 < wy) ? own + ROWB : TOPROW + tx * 16;
+  float sxm = 1.f, sxp = 1.f, sym = 1.f, syp = 1.f;     // reflective faces: sign of the face-normal flux (A13)
+  if (BCGEN) {
+    if (tx == 0 && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) sxm = -1.f;
+    if (tx == wx - 1 && x0 + wx == n && p.bc[1] == EMMA_RT_BC_REFLECTIVE) sxp = -1.f;
+    if (ty == 0 && y0 == 0 && p.bc[2] == EMMA_RT_BC_REFLECTIVE) sym = -1.f;
+    if (ty == wy - 1 && y0 + wy == n && p.bc[3] == EMMA_RT_BC_REFLECTIVE) syp = -1.f;
+  }
+  // halo cells: dealt round-robin over the warps, at most one per thread; a reflective ghost gets its aux from the
+  // mirrored state (face-normal component negated)
+  int hoff = -1;
+  float hsx = 1.f, hsy = 1.f;
+  {
+    const int nh = 2 * wy + 2 * wx, h = lane * (NT / 32) + warp;
+    if (h < nh) {
+      if (h < wy) { hoff = STAGE_ROWS + h * 16; if (BCGEN && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) hsx = -1.f; }
+      else if (h < 2 * wy) { hoff = STAGE_ROWS + COLB + (h - wy) * 16; if (BCGEN && x0 + wx == n && p.bc[1] == EMMA_RT_BC_REFLECTIVE) hsx = -1.f; }
+      else if (h < 2 * wy + wx) { hoff = (h - 2 * wy) * 16; if (BCGEN && y0 == 0 && p.bc[2] == EMMA_RT_BC_REFLECTIVE) hsy = -1.f; }
+      else { hoff = TOPROW + (h - 2 * wy - wx) * 16; if (BCGEN && y0 + wy == n && p.bc[3] == EMMA_RT_BC_REFLECTIVE) hsy = -1.f; }
+    }
+  }
+
+  bool flz, fltop, fl;
+  const int zm = bc_map(z0 - 1, n, p.bc[4], p.bc[5], flz);
+  const int ztop = bc_map(z1, n, p.bc[4], p.bc[5], fltop);
+  const int cxl = 4 * bc_map(x0 - 1, n, p.bc[0], p.bc[1], fl);
+  const int cxr = 4 * bc_map(x0 + wx, n, p.bc[0], p.bc[1], fl);
+  const int cyb = bc_map(y0 - 1, n, p.bc[2], p.bc[3], fl);
+  const int cyt = bc_map(y0 + wy, n, p.bc[2], p.bc[3], fl);
+
+  auto issue = [&](int j, int s) {             // the five boxes of plane j, each by the first lane of a different warp
+    if (lane != 0 || warp >= 5) return;
+    const int zg = g * n + ((j < 0) ? zm : (j >= zc) ? ztop : z0 + j);
+    const unsigned bar = bar0 + 8 * s, dst = stage0 + s * SG;
+    if (warp == 0) { mbar_expect_tx(bar, TY * ROWB); tma_load_3d(dst + ROWB, &maps.main, bar, 4 * x0, y0, zg); }
+    else if (warp == 1) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst, &maps.row, bar, 4 * x0, cyb, zg); }
+    else if (warp == 2) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst + TOPROW, &maps.row, bar, 4 * x0, cyt, zg); }
+    else if (warp == 3) { mbar_expect_tx(bar, COLB); tma_load_3d(dst + STAGE_ROWS, &maps.col, bar, cxl, y0, zg); }
+    else { mbar_expect_tx(bar, COLB); tma_load_3d(dst + STAGE_ROWS + COLB, &maps.col, bar, cxr, y0, zg); }
+  };
+
+  if (t == 0) {
+    for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 5);
+    mbar_init(bar_pl, NT / 32);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  for (int j = -1; j < NST - 1 && j <= zc; j++) issue(j, j + 1);
+
+  const float nu = p.nu;
+  const size_t plane = (size_t)n * n;
+  float4* pst = Uout + ((size_t)g * n + z0) * plane + (act ? ((size_t)y * n + x) : 0);
+  Acc acc_d;
+
+  auto halo_aux = [&](const unsigned char* st, unsigned char* aux) {
+    if (hoff >= 0) {
+      float4 h = *(const float4*)(st + hoff);
+      if (BCGEN) { h.y *= hsx; h.z *= hsy; }
+      store_aux(aux, hoff, make_aux(h));
+    }
+  };
+
+  // ---- prologue: aux of plane -1 (own cells only: it is only ever a z-neighbour) and of plane 0
+  {
+    mbar_wait(bar0, 0);
+    float4 m = *(const float4*)(smem + own);
+    if (BCGEN && flz) m.w = -m.w;
+    store_aux(sAUX, own, make_aux(m));
+    mbar_wait(bar0 + 8, 0);
+    store_aux(sAUX + AUXB, own, make_aux(*(const float4*)(smem + SG + own)));
+    halo_aux(smem + SG, sAUX + AUXB);
+  }
+  __syncthreads();
+
+  int s_old = 0, s_blw = 0, s_cur = 1, s_nxt = 2 % NST;
+  unsigned par_nxt = (2 / NST) & 1;
+  int ab_blw = 0, ab_cur = 1;
+  float4 Hzm = make_float4(0.f, 0.f, 0.f, 0.f);
+
+  for (int j = 0; j < zc; j++) {
+    if (j > 0) {
+      mbar_wait_relaxed(bar_pl, (unsigned)(j - 1) & 1u);
+      if (j + NST - 2 <= zc) issue(j + NST - 2, s_old);
+    }
+    const unsigned char* sb = smem + s_blw * SG;
+    const unsigned char* sc = smem + s_cur * SG;
+    const unsigned char* sn = smem + s_nxt * SG;
+    unsigned char* AXb = sAUX + ab_blw * AUXB;                         // aux of plane j-1; receives plane j+1
+    const unsigned char* AXc = sAUX + ab_cur * AUXB;
+    mbar_wait(bar0 + 8 * s_nxt, par_nxt);
+    const bool top = (j + 1 == zc);
+
+    // my cell and its aux (staged by me one plane ago)
+    const float4 cu = *(const float4*)(sc + own);
+    const float4 c0 = *(const float4*)(AXc + 2 * own), c1 = *(const float4*)(AXc + 2 * own + 16);
+    // the plane above: aux now (kept for the z face, staged for the next plane)
+    float4 un = *(const float4*)(sn + own);
+    if (BCGEN && top && fltop) un.w = -un.w;
+    const Aux An = make_aux(un);
+    if (j == 0) {
+      // the face below the chunk: flux from the plane below (afterwards it is carried from plane to plane)
+      float4 ub = *(const float4*)(sb + own);
+      if (BCGEN && flz) ub.w = -ub.w;
+      const float4 b0 = *(const float4*)(AXb + 2 * own), b1 = *(const float4*)(AXb + 2 * own + 16);
+      Hzm = hll_face<2>(ub, b0.x, b0.y, b1.z, b1.w, cu, c0.x, c0.y, c1.z, c1.w);
+    }
+    if (!top) {
+      store_aux(AXb, own, An);
+      halo_aux(sn, AXb);
+    }
+    const float4 Hzp = hll_face<2>(cu, c0.x, c0.y, c1.z, c1.w, un, An.a, An.b, An.lm[2], An.lp[2]);
+    float4 u, q;
+    float2 r;
+    u = *(const float4*)(sc + oxm); q = *(const float4*)(AXc + 2 * oxm); if (BCGEN) u.y *= sxm;
+    const float4 Hxm = hll_face<0>(u, q.x, q.y, q.z, q.w, cu, c0.x, c0.y, c0.z, c0.w);
+    u = *(const float4*)(sc + oxp); q = *(const float4*)(AXc + 2 * oxp); if (BCGEN) u.y *= sxp;
+    const float4 Hxp = hll_face<0>(cu, c0.x, c0.y, c0.z, c0.w, u, q.x, q.y, q.z, q.w);
+    u = *(const float4*)(sc + oym); q = *(const float4*)(AXc + 2 * oym); r = *(const float2*)(AXc + 2 * oym + 16); if (BCGEN) u.z *= sym;
+    const float4 Hym = hll_face<1>(u, q.x, q.y, r.x, r.y, cu, c0.x, c0.y, c1.x, c1.y);
+    u = *(const float4*)(sc + oyp); q = *(const float4*)(AXc + 2 * oyp); r = *(const float2*)(AXc + 2 * oyp + 16); if (BCGEN) u.z *= syp;
+    const float4 Hyp = hll_face<1>(cu, c0.x, c0.y, c1.x, c1.y, u, q.x, q.y, r.x, r.y);
+    // my reads of planes j-1, j and my aux writes of plane j+1 are done
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_pl);
+
+    float4 o;                                                          // Eq. 30, unsplit (A4)
+    o.x = fmaf(-nu, (Hxp.x - Hxm.x) + (Hyp.x - Hym.x) + (Hzp.x - Hzm.x), cu.x);
+    o.y = fmaf(-nu, (Hxp.y - Hxm.y) + (Hyp.y - Hym.y) + (Hzp.y - Hzm.y), cu.y);
+    o.z = fmaf(-nu, (Hxp.z - Hxm.z) + (Hyp.z - Hym.z) + (Hzp.z - Hzm.z), cu.z);
+    o.w = fmaf(-nu, (Hxp.w - Hxm.w) + (Hyp.w - Hym.w) + (Hzp.w - Hzm.w), cu.w);
+    Hzm = Hzp;
+    if (act) {
+      *pst = o;
+      if (DIAG) {
+        if (!(fabsf(o.x) + fabsf(o.y) + fabsf(o.z) + fabsf(o.w) < __int_as_float(0x7f800000))) acc_d.nonfinite++;
+        acc_d.total += (double)o.x;
+      }
+      if (BCGEN) {
+        // outflow through open faces (A15): with ghost = own cell the HLL flux is the cell's own G_d, N-component
+        // phi_d; through a reflective face it is 0 (mirror states: l- = -l+, the phi_d cancel, N_R = N_L)
+        const int z = z0 + j;
+        if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.y;
+        if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.y;
+        if (y == 0 && p.bc[2] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.z;
+        if (y == n - 1 && p.bc[3] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.z;
+        if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.w;
+        if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.w;
+      }
+    }
+    pst += plane;
+    s_old = s_blw; s_blw = s_cur; s_cur = s_nxt;
+    if (++s_nxt == NST) { s_nxt = 0; par_nxt ^= 1u; }
+    const int ab_nxt = ab_blw;
+    ab_blw = ab_cur; ab_cur = ab_nxt;
+  }
+
+  if (DIAG || BCGEN) {
+    acc_d.outflow *= (double)p.nu * p.dV;
+    acc_d.total *= p.dV;
+    block_reduce_store(acc_d, parts + blockIdx.x);
+  }
+}
+
+template <bool DIAG, bool BCGEN>
+cudaError_t launch_variant(const TransportParams& p, const TransportMaps& maps, float4* Uout, Partial* parts, int nblk,
+                           cudaStream_t st)
+{
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(transport_hll_kernel<DIAG, BCGEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  transport_hll_kernel<DIAG, BCGEN><<<nblk, NT, SMEM, st>>>(p, maps, Uout, parts);
+  return cudaSuccess;
+}
+
+}  // namespace
+
+int hll_ctas_per_sm() { return 1; }
+
+int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
+                         int* n_parts, cudaStream_t st)
+{
+  const int nblk = p.tiles_x * p.tiles_y * p.nzc * p.G;
+  bool bcgen = false;
+  for (int f = 0; f < 6; f++) bcgen = bcgen || (p.bc[f] != EMMA_RT_BC_PERIODIC);
+  const bool diag = p.want_total != 0;
+  cudaError_t e;
+  if (diag && bcgen) e = launch_variant<true, true>(p, maps_in, Uout, parts, nblk, st);
+  else if (diag) e = launch_variant<true, false>(p, maps_in, Uout, parts, nblk, st);
+  else if (bcgen) e = launch_variant<false, true>(p, maps_in, Uout, parts, nblk, st);
+  else e = launch_variant<false, false>(p, maps_in, Uout, parts, nblk, st);
+  *n_parts = (diag || bcgen) ? nblk : 0;
+  return e == cudaSuccess ? 1 : 0;
+}
+
+}  // namespace emma

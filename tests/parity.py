@@ -28,12 +28,12 @@ def coarse_ancestors(w):
     return anc
 
 
-def run_pair(w, n_steps, track_signatures=True, chemistry=None, thermal=None, otsa=None, bc=None, block=1, fused=None):
+def run_pair(w, n_steps, track_signatures=True, chemistry=None, thermal=None, otsa=None, bc=None, block=1, fused=None, flux=None):
     """Advance the oracle and the CUDA library side by side.
     Returns (oracle, gpu, flips, diags); flips = list of (step, level, cell, coarse_cell)."""
     kw = dict(chemistry=chemistry, thermal=thermal, otsa=otsa, bc=bc)
-    orc = O.Oracle(w, **kw)
-    gpu = E.EmmaRT(w, record_subcycles=1 if track_signatures else 0, fused=fused, **kw)
+    orc = O.Oracle(w, flux=flux, **kw)
+    gpu = E.EmmaRT(w, record_subcycles=1 if track_signatures else 0, fused=fused, flux=flux, **kw)
     nl = w.n_levels
     chem_on = (w.chemistry if chemistry is None else chemistry) and (w.thermal if thermal is None else thermal)
     do_track = track_signatures and chem_on
