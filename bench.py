@@ -219,7 +219,7 @@ def run_ours(args):
     roofline["traffic"] = ncu_traffic(dominant, n)
 
     # ---------------- transport-only throughput (chemistry = 0), same grid, K steps
-    tr = None
+    tr = hll = None
     if not args.skip_transport_only:
         gpu.close()
         gpu = None
@@ -236,6 +236,20 @@ def run_ours(args):
               "GBps": 32.0 * units_per_step * K / (ms_t * 1e-3) / 1e9}
         tr["frac"] = tr["GBps"] / peak
         g2.close()
+        torch.cuda.empty_cache()
+        # the same with the HLL interface flux (emma_rt_set_flux)
+        g3 = E.EmmaRT(w, device=dev, chemistry=0, flux=E.FLUX_HLL)
+        g3.step(dt, W, diag=False)
+        barrier()
+        e0.record()
+        g3.step(dt, K, diag=False)
+        e1.record()
+        barrier()
+        ms_h = e0.elapsed_time(e1)
+        hll = {"value": units_per_step * K / (ms_h * 1e-3), "unit": UNIT, "ms_per_step": ms_h / K,
+               "GBps": 32.0 * units_per_step * K / (ms_h * 1e-3) / 1e9}
+        hll["frac"] = hll["GBps"] / peak
+        g3.close()
         torch.cuda.empty_cache()
         gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
 
@@ -292,7 +306,7 @@ def run_ours(args):
                            "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
                            "schedule": "unfused" if args.unfused else "fused",
                            "parallelism": "replicas" if world > 1 else "single"},
-                "roofline": roofline, "kernels": kern, "transport_only": tr, "e2e": e2e, "cpu_baseline": cpu,
+                "roofline": roofline, "kernels": kern, "transport_only": tr, "transport_only_hll": hll, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": int(launches), "clocks": clk,
                 "subcycles": {"mean_last_step": diag["subcycles_total"] / float(ncell), "max_last_step": diag["subcycles_max"],
                               "deferred_last_step": diag["n_deferred"]}}

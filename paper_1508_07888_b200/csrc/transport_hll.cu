@@ -34,7 +34,7 @@ constexpr int TOPROW = (TY + 1) * ROWB;
 constexpr int STAGE_ROWS = (TY + 2) * ROWB;
 constexpr int COLB = TY * 16;
 constexpr int SG = STAGE_ROWS + 2 * COLB;      // bytes of one plane (own 32 x 16 box, 2 halo rows, 2 halo columns)
-constexpr int NST = 8;                         // stages of the ring
+constexpr int NST = 6;                         // stages of the ring
 constexpr int AUXB = 2 * SG;                   // aux plane: two float4 per cell at twice the byte offset of the cell
 constexpr size_t SMEM = (size_t)NST * SG + 2 * AUXB + 8 * (NST + 1);
 
@@ -98,7 +98,7 @@ __device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL,
 // DIAG: chemistry is off, so this pass owns the step's photon total and non-finite scan.
 // BCGEN: some face is not periodic (outflow sums and the reflective signs are compiled in).
 template <bool DIAG, bool BCGEN>
-__global__ void __launch_bounds__(NT, 1)
+__global__ void __launch_bounds__(NT, 2)
 transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps, float4* __restrict__ Uout,
                      Partial* __restrict__ parts)
 {
@@ -306,7 +306,7 @@ cudaError_t launch_variant(const TransportParams& p, const TransportMaps& maps, 
 
 }  // namespace
 
-int hll_ctas_per_sm() { return 1; }
+int hll_ctas_per_sm() { return 2; }
 
 int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st)
