@@ -104,35 +104,43 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_oracle(n, steps, warmup, variant):
-    """The oracle as it stands on the host cores, on config 5 at n^3 (a bounded sample of the 512^3 workload)."""
+def time_oracle(n, steps, warmup, variant, config=5):
+    """The oracle as it stands on the host cores, on config `config` at n^3 (a bounded sample of the full workload)."""
     import oracle as O
     from workloads import make_config
-    w = make_config(5, n=n, variant=variant)
+    w = make_config(config, n=n, variant=variant)
     orc = O.Oracle(w)
     if warmup:
         orc.step(w.dt, warmup)
     t0 = time.perf_counter()
     rc, d = orc.step(w.dt, steps)
     dt = time.perf_counter() - t0
-    units = n ** 3 * w.G * steps
+    units = leaf_count(w) * w.G * steps
     return units / dt, dt, O.lib().orc_threads(), d
+
+
+def leaf_count(w):
+    """Cells that carry chemistry: every cell of every level minus the split ones (config 4; n^3 on a uniform grid)."""
+    cells = [w.n ** 3] + [8 * len(p) for p in w.parent]
+    split = [len(p) for p in w.parent] + [0]
+    return int(sum(c - s for c, s in zip(cells, split)))
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n = ORACLE_SAMPLE_N
+    n = ORACLE_SAMPLE_N if args.config == 5 else 96
     steps, warm = max(1, min(args.steps, 5)), min(args.warmup, 1)
     # per "step" of this arm: one oracle step on the n^3 sample; the whole run stays within a few minutes
-    val, secs, cores, d = time_oracle(n, steps, warm, args.variant)
-    sample = "config 5%s recipe at %d^3 x 3 groups (1/%d of the 512^3 cells), %d coupled steps, fp64 C oracle with OpenMP" % (
-        args.variant, n, (512 // n) ** 3, steps)
+    val, secs, cores, d = time_oracle(n, steps, warm, args.variant, args.config)
+    label = ("5" + args.variant) if args.config == 5 else "4 (CRTA, 2 refined levels)"
+    sample = "config %s recipe at %d^3 x 3 groups (a bounded sample of the full grid), %d coupled steps, fp64 C oracle with OpenMP" % (
+        label, n, steps)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE config 5%s sampled at %d^3 (oracle on host cores)" % (args.variant, n)},
+            "config": {"workload": "BASELINE config %s sampled at %d^3 (oracle on host cores)" % (label, n)},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -161,14 +169,19 @@ def run_ours(args):
 
     n, K, W = args.n, args.steps, args.warmup
     t0 = time.time()
-    w = make_config(5, n=n, variant=args.variant, seed=None if world == 1 else 150807893 + 1000 * rank)
+    if args.config == 4:
+        # BASELINE config 4: 256^3 coarse + 2 refined levels (CRTA); transport on the coarse level, chemistry on leaves
+        w = make_config(4, n=None if n == 512 else n, seed=None if world == 1 else 150807892 + 1000 * rank)
+        n = w.n
+    else:
+        w = make_config(5, n=n, variant=args.variant, seed=None if world == 1 else 150807893 + 1000 * rank)
     G = w.G
     ncell = n ** 3
     log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
 
     gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
     dt = w.dt
-    units_per_step = ncell * G
+    units_per_step = leaf_count(w) * G            # config 5: n^3 G; config 4: leaf cells x G
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -232,8 +245,8 @@ def run_ours(args):
         e1.record()
         barrier()
         ms_t = e0.elapsed_time(e1)
-        tr = {"value": units_per_step * K / (ms_t * 1e-3), "unit": UNIT, "ms_per_step": ms_t / K,
-              "GBps": 32.0 * units_per_step * K / (ms_t * 1e-3) / 1e9}
+        tr = {"value": ncell * G * K / (ms_t * 1e-3), "unit": UNIT, "ms_per_step": ms_t / K,       # coarse cells x G
+              "GBps": 32.0 * ncell * G * K / (ms_t * 1e-3) / 1e9}
         tr["frac"] = tr["GBps"] / peak
         g2.close()
         torch.cuda.empty_cache()
@@ -246,8 +259,8 @@ def run_ours(args):
         e1.record()
         barrier()
         ms_h = e0.elapsed_time(e1)
-        hll = {"value": units_per_step * K / (ms_h * 1e-3), "unit": UNIT, "ms_per_step": ms_h / K,
-               "GBps": 32.0 * units_per_step * K / (ms_h * 1e-3) / 1e9}
+        hll = {"value": ncell * G * K / (ms_h * 1e-3), "unit": UNIT, "ms_per_step": ms_h / K,
+               "GBps": 32.0 * ncell * G * K / (ms_h * 1e-3) / 1e9}
         hll["frac"] = hll["GBps"] / peak
         g3.close()
         torch.cuda.empty_cache()
@@ -292,23 +305,27 @@ def run_ours(args):
     # ---------------- oracle on the host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.skip_cpu_baseline:
-        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N, ORACLE_SAMPLE_STEPS, 0, args.variant)
+        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N if args.config == 5 else 96, ORACLE_SAMPLE_STEPS, 0, args.variant, args.config)
         cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
-               "sample": "config 5%s recipe at %d^3 x 3 groups, %d coupled steps from the initial state, fp64 C oracle, "
-                         "OpenMP on all host cores" % (args.variant, ORACLE_SAMPLE_N, ORACLE_SAMPLE_STEPS)}
+               "sample": "config %s recipe at %d^3 x 3 groups, %d coupled steps from the initial state, fp64 C oracle, "
+                         "OpenMP on all host cores" % ("5" + args.variant if args.config == 5 else "4 (CRTA, 2 levels)",
+                                                       ORACLE_SAMPLE_N if args.config == 5 else 96, ORACLE_SAMPLE_STEPS)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic",
-                "config": {"workload": "BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
-                                       "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)),
+                "config": {"workload": ("BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
+                                        "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)))
+                           if args.config == 5 else
+                           ("BASELINE config 4: %d^3 coarse + 2 refined levels (CRTA), %d groups, lognormal sigma_ln=1.5, "
+                            "%d leaves, %d sources; value counts leaf-cell-group updates" % (n, G, leaf_count(w), len(w.src_pos))),
                            "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
                            "schedule": "unfused" if args.unfused else "fused",
                            "parallelism": "replicas" if world > 1 else "single"},
                 "roofline": roofline, "kernels": kern, "transport_only": tr, "transport_only_hll": hll, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": int(launches), "clocks": clk,
-                "subcycles": {"mean_last_step": diag["subcycles_total"] / float(ncell), "max_last_step": diag["subcycles_max"],
+                "subcycles": {"mean_last_step": diag["subcycles_total"] / float(leaf_count(w)), "max_last_step": diag["subcycles_max"],
                               "deferred_last_step": diag["n_deferred"]}}
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -323,6 +340,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=512)
     ap.add_argument("--variant", default="b", choices=["a", "b"])
+    ap.add_argument("--config", type=int, default=5, choices=[4, 5], help="BASELINE config: 5 (default, the metric's) or 4 (CRTA)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--unfused", action="store_true", help="separate transport and chemistry passes")
     ap.add_argument("--skip-transport-only", action="store_true")
