@@ -319,7 +319,7 @@ __device__ __forceinline__ float oct_sum(float v)
 }
 
 template <int G>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 8)
 chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow, const float4* __restrict__ Ut_above,
                     long long nocts_above, float4* __restrict__ U0, long long ncell0, int level,
                     Partial* __restrict__ parts)
@@ -508,7 +508,10 @@ int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int
   const LevelDev& L = lv[level];
   if (L.ncell == 0) { *n_parts = 0; return 0; }
   long long want = (L.ncell + 127) / 128;
-  int nb = (int)(want < MAX_PART_BLOCKS ? want : MAX_PART_BLOCKS);
+  static int sms = 0;                                                 // persistent grid: whole waves of 8 CTAs per SM
+  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+  const long long cap = (sms > 0 && (long long)sms * 8 <= MAX_PART_BLOCKS) ? (long long)sms * 8 : MAX_PART_BLOCKS;
+  int nb = (int)(want < cap ? want : cap);
   const float4* Ut_above = (level < n_levels) ? lv[level + 1].Ut : nullptr;
   const long long nocts_above = (level < n_levels) ? lv[level + 1].nocts : 0;
   switch (cp.G) {
