@@ -114,6 +114,7 @@ struct emma_rt {
   DiagDev* diag_pinned;
   Profiler prof;
   TransportMaps tmaps[2];                      // TMA descriptors of U[0], U[1]
+  TransportMaps tmaps_f[2];                    // the same with the fused pass's tile height
   int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
   int flux;                                    // interface flux of the transport update (emma_rt_set_flux)
   char err[256];
@@ -218,6 +219,8 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   for (int b = 0; b < 2; b++) {
     const int r = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps[b]);
     if (r != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", r);
+    const int rf = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_f[b], fused_tile_y());
+    if (rf != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", rf);
   }
 
   // ---- AMR index arrays (a-0: per-level oct arrays with parent / coarse-ancestor / child indices)
@@ -406,6 +409,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   if (hll && !pick_zchunks(hp, hp.tiles_x * hp.tiles_y * s.G, hll_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
   const bool fused = !hll && h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
   TransportParams fp = tp;
+  fp.tiles_y = (s.n + fused_tile_y() - 1) / fused_tile_y();
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
 
   for (int step = 0; step < n_steps; step++) {
@@ -416,7 +420,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
       // tail, then CRTA on the refined cells (they read the U* this pass wrote into their coarse ancestors)
       float4* U = h->U(1 - h->cur);
       h->prof.begin(EMMA_RT_K_FUSED);
-      const int k = launch_fused(fp, h->tmaps[h->cur], U, cp, h->lv[0], (int*)(h->arena + h->lay.queue), h->qcount(), P + off, &np, h->st);
+      const int k = launch_fused(fp, h->tmaps_f[h->cur], U, cp, h->lv[0], (int*)(h->arena + h->lay.queue), h->qcount(), P + off, &np, h->st);
       if (!k) return fail(h, EMMA_RT_ECUDA, "fused launch failed: %s", cudaGetErrorString(cudaGetLastError()));
       h->prof.end();
       h->launches += k;

@@ -113,7 +113,7 @@ struct Profiler {
 // ---- launchers (each returns the number of kernels it launched) ---------------------------------------------
 int launch_transport(const TransportParams& p, const float4* Uin, float4* Uout, Partial* parts, int* n_parts,
                      cudaStream_t st);
-int make_transport_maps(const float4* U, int n, int G, TransportMaps* out);
+int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int tile_y = 16);
 int launch_transport_tma(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st);
 int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
@@ -124,6 +124,7 @@ int launch_chem_tail(const ChemParams& cp, const LevelDev& L0, float4* U, long l
 int launch_fused(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, const ChemParams& cp,
                  const LevelDev& L0, int* queue, unsigned int* qcount, Partial* parts, int* n_parts, cudaStream_t st);
 int fused_ctas_per_sm();
+int fused_tile_y();
 int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st);
 int hll_ctas_per_sm();

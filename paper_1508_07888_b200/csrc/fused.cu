@@ -33,7 +33,12 @@ namespace {
 using namespace acp;
 
 constexpr int TX = 32;                         // tile width = one warp along x
-constexpr int TY = 16;                         // tile height = warps per CTA
+#ifndef FUSED_TY
+#define FUSED_TY 16
+#endif
+constexpr int TY = FUSED_TY;                   // tile height = warps per CTA.  16: one CTA of 512 threads per SM (3.95 ms
+                                               // at 512^3 x 3); 8: two CTAs of 256 (measured slower: 4.19 ms, more halo work)
+constexpr int CTAS_PER_SM = 16 / TY;
 constexpr int NT = TX * TY;
 constexpr int ROWB = TX * 16;                  // bytes of one row of cells
 constexpr int TOPROW = (TY + 1) * ROWB;        // offset of the y-halo row above
@@ -42,11 +47,11 @@ constexpr int COLB = TY * 16;                  // bytes of one halo column
 constexpr int SG = STAGE_ROWS + 2 * COLB;      // one group's plane: what its five boxes deliver
 constexpr int ABG = SG / 2;                    // its closure plane: float2 (a, b) at half the byte offset of the cell
 
-template <int G> constexpr int fused_nst() { return G == 1 ? 12 : G == 2 ? 8 : G == 3 ? 6 : 4; }
+template <int G> constexpr int fused_nst() { return TY == 16 ? (G == 1 ? 12 : G == 2 ? 8 : G == 3 ? 6 : 4) : (G == 1 ? 10 : G == 2 ? 7 : G == 3 ? 5 : 4); }
 template <int G> constexpr size_t fused_smem() { return (size_t)fused_nst<G>() * G * SG + 2 * G * ABG + 8 * (fused_nst<G>() + 1); }
 
 template <int G, bool BCGEN>
-__global__ void __launch_bounds__(NT, 1)
+__global__ void __launch_bounds__(NT, CTAS_PER_SM)
 fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps, float4* __restrict__ Uout,
              const ChemParams cp, const LevelDev L, int* __restrict__ queue, unsigned int* __restrict__ qcount,
              Partial* __restrict__ parts)
@@ -84,16 +89,17 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const int oyp = (ty + 1 < wy) ? own + ROWB : TOPROW + tx * 16;
   // halo closures: the 2 wy + 2 wx halo cells of each of the G groups are dealt round-robin over the warps (task
   // h -> warp h % 16, lane h / 16), at most one per thread, so that every warp carries the same extra work
-  int hoff = -1;                               // byte offset (inside a stage) of the halo cell whose closure I compute
-  {
-    const int nh = 2 * wy + 2 * wx, h = (t & 31) * (NT / 32) + (t >> 5);
-    if (h < nh * G) {
-      const int g = h / nh, q = h - g * nh;
-      const int o = (q < wy) ? STAGE_ROWS + q * 16 : (q < 2 * wy) ? STAGE_ROWS + COLB + (q - wy) * 16
-                  : (q < 2 * wy + wx) ? (q - 2 * wy) * 16 : TOPROW + (q - 2 * wy - wx) * 16;
-      hoff = g * SG + o;
-    }
-  }
+  // (with 32 x 8 tiles and G = 4 there are more halo cells than threads: a second task for some)
+  auto halo_task = [&](int h) -> int {         // byte offset (inside a stage) of halo task h, or -1
+    const int nh = 2 * wy + 2 * wx;
+    if (h >= nh * G) return -1;
+    const int g = h / nh, q = h - g * nh;
+    const int o = (q < wy) ? STAGE_ROWS + q * 16 : (q < 2 * wy) ? STAGE_ROWS + COLB + (q - wy) * 16
+                : (q < 2 * wy + wx) ? (q - 2 * wy) * 16 : TOPROW + (q - 2 * wy - wx) * 16;
+    return g * SG + o;
+  };
+  const int hoff = halo_task((t & 31) * (NT / 32) + (t >> 5));
+  const int hoff2 = ((2 * TY + 2 * TX) * G > NT) ? halo_task(NT + (t & 31) * (NT / 32) + (t >> 5)) : -1;
   float sxm = 1.f, sxp = 1.f, sym = 1.f, syp = 1.f;     // reflective faces: sign of the face-normal flux (A13)
   if (BCGEN) {
     if (tx == 0 && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) sxm = -1.f;
@@ -154,6 +160,11 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       float a, b;
       closure_ab(*(const float4*)(st + hoff), a, b);
       *(float2*)(ab + (hoff >> 1)) = make_float2(a, b);
+    }
+    if (halo && hoff2 >= 0) {
+      float a, b;
+      closure_ab(*(const float4*)(st + hoff2), a, b);
+      *(float2*)(ab + (hoff2 >> 1)) = make_float2(a, b);
     }
   };
 
@@ -247,6 +258,11 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       closure_ab(*(const float4*)(sn + hoff), a, b);
       *(float2*)(ABb + (hoff >> 1)) = make_float2(a, b);
     }
+    if (!top && hoff2 >= 0) {
+      float a, b;
+      closure_ab(*(const float4*)(sn + hoff2), a, b);
+      *(float2*)(ABb + (hoff2 >> 1)) = make_float2(a, b);
+    }
     // my part of planes j-1, j, j+1 is done (release: the closure writes above)
     __syncwarp();
     if (lane == 0) mbar_arrive(bar_pl);
@@ -338,7 +354,8 @@ int launch_G(const TransportParams& p, const TransportMaps& maps, float4* Uout, 
 }  // namespace
 
 // CTAs resident per SM of the fused pass (one: its ring fills the shared memory) -- for the z-chunk cost model
-int fused_ctas_per_sm() { return 1; }
+int fused_ctas_per_sm() { return CTAS_PER_SM; }
+int fused_tile_y() { return TY; }
 
 // Launches the fused pass over the coarse block; p.tiles_* / p.zchunk / p.nzc describe its own 32 x 16 tiling.
 int launch_fused(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, const ChemParams& cp,
