@@ -147,6 +147,27 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def replica_seed(config, rank, world):
+    """Seed of a rank's replica (DESIGN.md section 8: N > 1 = independent replicas, different seeds per rank);
+    None = the config's own seed (single GPU)."""
+    return None if world == 1 else (150807888 + config) + 1000 * rank
+
+
+def max_over_ranks(value, dist, device):
+    """Device time of the job = the slowest rank's (all-reduce MAX); `dist` is torch.distributed or None."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_step, steps, world, ms):
+    """Aggregate throughput of `world` replicas that each advanced `steps` steps in `ms` (max over ranks)."""
+    return units_per_step * steps * world / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import paper_1508_07888_b200 as E
@@ -171,10 +192,10 @@ def run_ours(args):
     t0 = time.time()
     if args.config == 4:
         # BASELINE config 4: 256^3 coarse + 2 refined levels (CRTA); transport on the coarse level, chemistry on leaves
-        w = make_config(4, n=None if n == 512 else n, seed=None if world == 1 else 150807892 + 1000 * rank)
+        w = make_config(4, n=None if n == 512 else n, seed=replica_seed(4, rank, world))
         n = w.n
     else:
-        w = make_config(5, n=n, variant=args.variant, seed=None if world == 1 else 150807893 + 1000 * rank)
+        w = make_config(5, n=n, variant=args.variant, seed=replica_seed(5, rank, world))
     G = w.G
     ncell = n ** 3
     log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
@@ -207,11 +228,8 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = gpu.kernel_launches() - launches0
     prof = gpu.profile(False)
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = units_per_step * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = whole_job_value(units_per_step, K, world, ms)
 
     # per-kernel roofline (algorithmic bytes of DESIGN.md section 7 / live CUDA-event durations)
     peak, peak_src = measured_peaks()
@@ -294,10 +312,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, "cuda")
     e2e = {"value": units_per_step * Ke * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "steps": Ke, "ms_per_step": 1e3 * e2e_s / Ke}
     gpu.close()
