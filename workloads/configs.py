@@ -252,3 +252,23 @@ def _leaf_centres_l2(ids, p1, p2, n):
     base = _leaf_centres_l1(c1, p1, n) - 0.25 / n          # low corner of the level-1 cell
     off = np.stack([ch & 1, (ch >> 1) & 1, (ch >> 2) & 1], axis=1).astype(np.float64)
     return base + (off + 0.5) * (0.25 / n)
+
+
+def make_hii_region_corner(n=64, n_steps=200):
+    """the static-gas cousin of the paper's HII-region test (section 6.4, after
+    Iliev et al. "Test 2"/"Test 5"): 15 kpc box, uniform hydrogen n = 1e-3 cm^-3 at 100 K and x = 1.2e-3, ONE source of
+    5e48 photons/s with a 1e5 K black-body spectrum in 3 groups placed in the corner cell at the origin, reflective
+    boundaries on the three faces that touch the source and transmissive ones elsewhere, c~ = c/10.
+    The gas does not move here (hydrodynamics is out of scope), so this is the paper's "Test 2"-like static run."""
+    gr = _groups(3)
+    L = 15.0 * CGS.kpc
+    w = Workload("hii-corner-static", n, 3, L, 0.1 * CGS.c, gr["sigma_N"], gr["sigma_E"], gr["E_mean"], gr["frac"],
+                 bc=(BC_REFLECTIVE, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_TRANSMISSIVE))
+    ncell = n ** 3
+    w.n0 = [np.full(ncell, 1e-3, np.float32)]
+    w.x = [np.full(ncell, 1.2e-3, np.float32)]
+    w.T = [np.full(ncell, 100.0, np.float32)]
+    w.src_pos = np.array([[0.5 / n, 0.5 / n, 0.5 / n]], np.float64)
+    w.src_Q = 5e48 * np.asarray(gr["frac"], np.float64)[None, :]
+    w.n_steps = n_steps
+    return w
