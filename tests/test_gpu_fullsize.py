@@ -79,14 +79,14 @@ def _mean8(v):
     return (((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]))) / 8.0
 
 
-def _oracle_cell(w, phys, src, U_in, state, cell, chemistry=True):
+def _oracle_cell(w, phys, src, U_in, state, cell, chemistry=True, flux=None):
     """Oracle result of ONE coupled step for coarse cell `cell`.
     Returns dict(U[G,4], leaves={(level, id): (x, T, sig)}, split={(level, id): (x, T)})."""
     n, G, c, dt, dx = w.n, w.G, w.c_red, w.dt, w.L / w.n
     Ustar = np.zeros((G, 4))
     for g in range(G):
         U0, Um, Up = _stencil_inputs(U_in[g], cell, n)
-        Ustar[g] = O.transport_stencil(c, dt, dx, U0, Um, Up)
+        Ustar[g] = O.transport_stencil(c, dt, dx, U0, Um, Up, flux=flux)
     res = {"leaves": {}, "split": {}}
     if not chemistry:
         S = src.get((0, cell))
@@ -135,7 +135,7 @@ def _restricted_n0(w, n0):
     return r
 
 
-def _check_samples(w, gpu, U_in, state, cells, chemistry=True):
+def _check_samples(w, gpu, U_in, state, cells, chemistry=True, flux=None):
     """Compare the library's state after ONE step from (U_in, state) with the oracle at the sampled coarse cells."""
     phys = O.make_phys(w.G, w.c_red, w.sigma_N, w.sigma_E, w.E_mean, otsa=w.otsa, thermal=w.thermal, e_tol=w.e_tol,
                        max_halvings=w.max_halvings)
@@ -152,7 +152,7 @@ def _check_samples(w, gpu, U_in, state, cells, chemistry=True):
     flips = n_leaves = n_split = 0
     for cell in cells:
         cell = int(cell)
-        r = _oracle_cell(w, phys, src, U_in, state, cell, chemistry)
+        r = _oracle_cell(w, phys, src, U_in, state, cell, chemistry, flux)
         flipped = False
         for (l, cid), (x1, T1, sig) in r["leaves"].items():
             n_leaves += 1
@@ -236,6 +236,24 @@ def test_config5_full_512_sampled_and_budget():
         assert abs((d["photons_total"] - prev) - rhs) <= 1e-6 * d["photons_total"]
         prev = d["photons_total"]
     _whole_grid_properties(w, gpu)
+    gpu.close()
+
+
+def test_config5_full_512_hll_transport_sampled():
+    """The HLL flux (reading A19) at 512^3 x 3 groups, the launch configuration bench.py times as `transport_only_hll`:
+    sampled cells against the oracle's HLL stencil, photons conserved on the periodic box."""
+    w = make_config(5)
+    rng = np.random.default_rng(5121)
+    cells = _sample_cells(w, rng, 3000)
+    gpu = E.EmmaRT(w, chemistry=0, flux=E.FLUX_HLL)
+    rc, d0 = gpu.step(w.dt, 0)
+    rc, d1 = gpu.step(w.dt, 1)
+    assert rc == E.OK and d1["n_nonfinite"] == 0
+    rep = _check_samples(w, gpu, w.U0, {"n0": w.n0, "x": w.x, "T": w.T}, cells, chemistry=False, flux=O.FLUX_HLL)
+    print("cfg5 512^3 HLL transport, sampled:", rep)
+    assert rep["N"] <= TOL and rep["F"] <= TOL, rep
+    inj = float(np.sum(w.src_Q)) * w.dt
+    assert d1["photons_total"] - d0["photons_total"] == pytest.approx(inj, abs=1e-6 * d1["photons_total"])
     gpu.close()
 
 
