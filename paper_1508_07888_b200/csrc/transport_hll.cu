@@ -35,7 +35,8 @@ constexpr int STAGE_ROWS = (TY + 2) * ROWB;
 constexpr int COLB = TY * 16;
 constexpr int SG = STAGE_ROWS + 2 * COLB;      // bytes of one plane (own 32 x 16 box, 2 halo rows, 2 halo columns)
 constexpr int NST = 6;                         // stages of the ring
-constexpr int AUXB = 2 * SG;                   // aux plane: two float4 per cell at twice the byte offset of the cell
+constexpr int AUXB = 2 * SG;                   // aux plane: two sub-planes of one float4 per cell, each laid out like a stage
+                                               // (consecutive lanes -> consecutive 16 B: no bank conflicts)
 constexpr size_t SMEM = (size_t)NST * SG + 2 * AUXB + 8 * (NST + 1);
 
 struct Aux {                                   // closure and wave speeds of one cell
@@ -68,9 +69,8 @@ __device__ __forceinline__ Aux make_aux(const float4& U)
 
 __device__ __forceinline__ void store_aux(unsigned char* plane, int off, const Aux& A)
 {
-  float4* q = (float4*)(plane + 2 * off);
-  q[0] = make_float4(A.a, A.b, A.lm[0], A.lp[0]);
-  q[1] = make_float4(A.lm[1], A.lp[1], A.lm[2], A.lp[2]);
+  *(float4*)(plane + off) = make_float4(A.a, A.b, A.lm[0], A.lp[0]);
+  *(float4*)(plane + SG + off) = make_float4(A.lm[1], A.lp[1], A.lm[2], A.lp[2]);
 }
 
 // flux vector G_d of a cell and the HLL combination for the face between L (towards -d) and R (towards +d)
@@ -221,7 +221,7 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
 
     // my cell and its aux (staged by me one plane ago)
     const float4 cu = *(const float4*)(sc + own);
-    const float4 c0 = *(const float4*)(AXc + 2 * own), c1 = *(const float4*)(AXc + 2 * own + 16);
+    const float4 c0 = *(const float4*)(AXc + own), c1 = *(const float4*)(AXc + SG + own);
     // the plane above: aux now (kept for the z face, staged for the next plane)
     float4 un = *(const float4*)(sn + own);
     if (BCGEN && top && fltop) un.w = -un.w;
@@ -230,7 +230,7 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
       // the face below the chunk: flux from the plane below (afterwards it is carried from plane to plane)
       float4 ub = *(const float4*)(sb + own);
       if (BCGEN && flz) ub.w = -ub.w;
-      const float4 b0 = *(const float4*)(AXb + 2 * own), b1 = *(const float4*)(AXb + 2 * own + 16);
+      const float4 b0 = *(const float4*)(AXb + own), b1 = *(const float4*)(AXb + SG + own);
       Hzm = hll_face<2>(ub, b0.x, b0.y, b1.z, b1.w, cu, c0.x, c0.y, c1.z, c1.w);
     }
     if (!top) {
@@ -240,13 +240,13 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     const float4 Hzp = hll_face<2>(cu, c0.x, c0.y, c1.z, c1.w, un, An.a, An.b, An.lm[2], An.lp[2]);
     float4 u, q;
     float2 r;
-    u = *(const float4*)(sc + oxm); q = *(const float4*)(AXc + 2 * oxm); if (BCGEN) u.y *= sxm;
+    u = *(const float4*)(sc + oxm); q = *(const float4*)(AXc + oxm); if (BCGEN) u.y *= sxm;
     const float4 Hxm = hll_face<0>(u, q.x, q.y, q.z, q.w, cu, c0.x, c0.y, c0.z, c0.w);
-    u = *(const float4*)(sc + oxp); q = *(const float4*)(AXc + 2 * oxp); if (BCGEN) u.y *= sxp;
+    u = *(const float4*)(sc + oxp); q = *(const float4*)(AXc + oxp); if (BCGEN) u.y *= sxp;
     const float4 Hxp = hll_face<0>(cu, c0.x, c0.y, c0.z, c0.w, u, q.x, q.y, q.z, q.w);
-    u = *(const float4*)(sc + oym); q = *(const float4*)(AXc + 2 * oym); r = *(const float2*)(AXc + 2 * oym + 16); if (BCGEN) u.z *= sym;
+    u = *(const float4*)(sc + oym); q = *(const float4*)(AXc + oym); r = *(const float2*)(AXc + SG + oym); if (BCGEN) u.z *= sym;
     const float4 Hym = hll_face<1>(u, q.x, q.y, r.x, r.y, cu, c0.x, c0.y, c1.x, c1.y);
-    u = *(const float4*)(sc + oyp); q = *(const float4*)(AXc + 2 * oyp); r = *(const float2*)(AXc + 2 * oyp + 16); if (BCGEN) u.z *= syp;
+    u = *(const float4*)(sc + oyp); q = *(const float4*)(AXc + oyp); r = *(const float2*)(AXc + SG + oyp); if (BCGEN) u.z *= syp;
     const float4 Hyp = hll_face<1>(cu, c0.x, c0.y, c1.x, c1.y, u, q.x, q.y, r.x, r.y);
     // my reads of planes j-1, j and my aux writes of plane j+1 are done
     __syncwarp();
