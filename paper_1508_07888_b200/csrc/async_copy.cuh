@@ -40,6 +40,7 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 }
 // the same with a short sleep between polls: for waits on other warps (not on data), where a spinning warp would only
 // take issue slots from the warps it is waiting for
+template <int SLEEP_NS = 64>
 __device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
 {
   unsigned done;
@@ -50,7 +51,7 @@ __device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     if (done) break;
-    __nanosleep(64);
+    __nanosleep(SLEEP_NS);
   }
 }
 // one box of a rank-3 tensor -> shared memory, completion (bytes) on an mbarrier
