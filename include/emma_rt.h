@@ -57,7 +57,8 @@ enum { EMMA_RT_OK = 0, EMMA_RT_EINVAL = -1, EMMA_RT_ENOMEM = -2, EMMA_RT_ECUDA =
 
 /* boundary conditions: periodic by nature; transmissive = ghost copies the cell;
  * reflective = the same with the face-normal flux component inverted (A13) */
-enum { EMMA_RT_BC_PERIODIC = 0, EMMA_RT_BC_TRANSMISSIVE = 1, EMMA_RT_BC_REFLECTIVE = 2 };
+enum { EMMA_RT_BC_PERIODIC = 0, EMMA_RT_BC_TRANSMISSIVE = 1, EMMA_RT_BC_REFLECTIVE = 2,
+       EMMA_RT_BC_INFLOW = 3 };   /* ghost = a prescribed state, see emma_rt_set_inflow (reading A20) */
 
 /* fields of emma_rt_read / emma_rt_write.  Element type and count per cell in brackets. */
 enum {
@@ -169,6 +170,12 @@ EMMA_RT_API int emma_rt_set_schedule(emma_rt* h, int32_t fused);
  * DESIGN.md reading A19):  F = [l+ F~_L - l- F~_R + l+ l- (U_R - U_L)] / (l+ - l-),  l+ = max(0, lmax_L, lmax_R),
  * l- = min(0, lmin_L, lmin_R), lmin/lmax the extreme eigenvalues of the M1 flux Jacobian in the face direction.
  * With HLL the coupled step runs the two-pass schedule (the fused pass implements Eq. 32 only).  Returns OK / EINVAL. */
+/* Inflow boundary (reading A20; "the x = 0 boundary is a source of flux of the required
+ * rate"): the ghost cells outside a face whose bc is EMMA_RT_BC_INFLOW hold the state U = (N, Fx, Fy, Fz) [photons cm^-3,
+ * photons cm^-2 s^-1] given here for `group` (zeros until set); a plane-parallel flux F entering through -x is
+ * (F / c_red, F, 0, 0).  face = 0..5 = -x,+x,-y,+y,-z,+z.  With an inflow face the step runs the two-pass schedule and the
+ * non-TMA transport kernel.  The net flux through the face counts (negative) in photons_outflow.  Returns OK / EINVAL. */
+EMMA_RT_API int emma_rt_set_inflow(emma_rt* h, int32_t face, int32_t group, const double U[4]);
 enum { EMMA_RT_FLUX_GLF = 0, EMMA_RT_FLUX_HLL = 1 };
 EMMA_RT_API int emma_rt_set_flux(emma_rt* h, int32_t flux);
 EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */

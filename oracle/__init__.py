@@ -21,6 +21,7 @@ MAX_GROUPS = 4
 OK, EINVAL, ENOMEM, ENONFINITE, ECFL, ESUBCYCLE = 0, -1, -2, -4, -6, -7
 F_U, F_N, F_F, F_X, F_T, F_E, F_N0, F_SUBCYCLES, F_XNEUTRAL = range(9)
 FLUX_GLF, FLUX_HLL = 0, 1
+BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
 
 
 def build(force=False):
@@ -82,6 +83,8 @@ def lib():
     L.orc_transport_stencil_flux.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
     L.orc_m1_wavespeeds.restype = None
     L.orc_m1_wavespeeds.argtypes = [dp, C.c_double, C.c_int, dp, dp]
+    L.orc_set_inflow.restype = C.c_int
+    L.orc_set_inflow.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
     L.orc_set_flux.restype = C.c_int
     L.orc_set_flux.argtypes = [C.c_void_p, C.c_int]
     L.orc_chem_cell.argtypes = [C.POINTER(Phys), C.c_double, C.c_double, dp, dp, dp, dp, C.POINTER(ChemOut)]
@@ -218,12 +221,20 @@ class Oracle:
                               _ptr_array(n0), _ptr_array(x), _ptr_array(T))
         if not self.h:
             raise ValueError("orc_create failed (invalid arguments or out of memory)")
+        for (face, group), U in (getattr(w, "inflow", None) or {}).items():
+            if self.set_inflow(face, group, U) != OK:
+                raise ValueError("orc_set_inflow(face=%d, group=%d) rejected" % (face, group))
         if flux is not None and L.orc_set_flux(self.h, int(flux)) != OK:
             raise ValueError("orc_set_flux: unknown flux %r" % (flux,))
         if w.src_pos is not None and len(w.src_pos):
             rc = self.set_sources(w.src_pos, w.src_Q)
             if rc != OK:
                 raise ValueError("orc_set_sources rc=%d" % rc)
+
+    def set_inflow(self, face, group, U):
+        """Ghost state (N, Fx, Fy, Fz) [cgs] of a BC_INFLOW face (0..5 = -x,+x,-y,+y,-z,+z), reading A20."""
+        U = np.ascontiguousarray(U, np.float64).reshape(4)
+        return lib().orc_set_inflow(self.h, int(face), int(group), _dp(U))
 
     def set_sources(self, pos, Q):
         pos = np.ascontiguousarray(pos, np.float64).reshape(-1, 3)

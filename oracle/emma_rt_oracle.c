@@ -88,8 +88,11 @@ static void glf_flux(const double UL[4], const double UR[4], double c, int d, do
  *     l+ = max(0, lmax(U_L), lmax(U_R)),   l- = min(0, lmin(U_L), lmin(U_R)),
  * with lmin/lmax the extreme eigenvalues of dF~_d/dU for the M1 closure of Eq. 22-23 (A1, A2):
  *     l(f, mu) = c [ mu f -/+ sqrt( (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) ) ] / xi,   xi = sqrt(4 - 3 f^2),
- * f as in the closure (clipped to [0,1], N <= 0 -> f = 0), mu = F_d/|F| (0 if |F| = 0).  l+ = -l- = c gives back
- * Eq. 32.  If l+ - l- = 0 (both cells free-streaming exactly along the face) the flux is (F~_L + F~_R)/2 (= 0 there).
+ * f as in the closure (clipped to [0,1], N <= 0 -> f = 0), mu = F_d/|F| (0 if |F| = 0).  l+ = -l- = c gives back Eq. 32.
+ * With this flux the updated state is kept realizable: if |F'| > c N' after Eq. 30 then F' := c max(N',0) F'/|F'| (N' is not
+ * touched, so photons are conserved).  Without it a beam (f = 1) is unstable: for f > 1 the clipped closure P = N n(x)n has
+ * the speeds -/+c, not the (c, c) these eigenvalues give, and the upwinded flux amplifies an f > 1 perturbation by 1 + nu
+ * per step (seen in the static clump test, tests/test_inflow_shadow.py).  If l+ - l- = 0 (both cells free-streaming exactly along the face) the flux is (F~_L + F~_R)/2 (= 0 there).
  * Pinned in tests against the eigenvalues of the finite-difference Jacobian of orc_closure. */
 void orc_m1_wavespeeds(const double U[4], double c, int d, double* lmin, double* lmax)
 {
@@ -141,6 +144,11 @@ static void transport_core(int flux, double c, double dt, double dx, const doubl
     face_flux(flux, U0, Up[d], c, d, Fp);     /* F_{i+1/2} */
     for (int q = 0; q < 4; q++) out[q] += (dt / dx) * (Fm[q] - Fp[q]);
     if (faceN) { faceN[2 * d] = Fm[0]; faceN[2 * d + 1] = Fp[0]; }
+  }
+  if (flux == ORC_FLUX_HLL) {                /* A19: keep the state realizable, |F| <= c N */
+    double Fn = sqrt(out[1] * out[1] + out[2] * out[2] + out[3] * out[3]);
+    double lim = c * (out[0] > 0.0 ? out[0] : 0.0);
+    if (Fn > lim) for (int q = 1; q < 4; q++) out[q] *= lim / Fn;
   }
 }
 
@@ -295,6 +303,7 @@ int orc_chem_cell(const orc_phys* ph, double dt, double n0, double* x_io, double
 struct orc {
   int n, chemistry;
   int flux;                        /* ORC_FLUX_GLF (Eq. 32) or ORC_FLUX_HLL (A19) */
+  double inflow[6][ORC_MAX_GROUPS][4]; /* A20: ghost state (N, Fx, Fy, Fz) of an ORC_BC_INFLOW face, per group */
   int bc[6];
   orc_phys ph;
   double L, dx;
@@ -318,6 +327,15 @@ int orc_set_flux(orc* o, int flux)
 {
   if (!o || (flux != ORC_FLUX_GLF && flux != ORC_FLUX_HLL)) return ORC_EINVAL;
   o->flux = flux;
+  return ORC_OK;
+}
+
+/* A20: prescribed ghost state of an inflow face (face = -x,+x,-y,+y,-z,+z), cgs */
+int orc_set_inflow(orc* o, int face, int group, const double U[4])
+{
+  if (!o || face < 0 || face > 5 || group < 0 || group >= o->ph.G || !U) return ORC_EINVAL;
+  if (o->bc[face] != ORC_BC_INFLOW) return ORC_EINVAL;
+  for (int q = 0; q < 4; q++) o->inflow[face][group][q] = U[q];
   return ORC_OK;
 }
 
@@ -468,7 +486,7 @@ int64_t orc_source_cell(const orc* o, int64_t i, int* level)
 }
 
 /* ghost value of the neighbour of (i,j,k) in direction d, side s (A13) */
-static void neighbour(const orc* o, const double* Ug, int i, int j, int k, int d, int s, double out[4])
+static void neighbour(const orc* o, const double* Ug, int g, int i, int j, int k, int d, int s, double out[4])
 {
   const int n = o->n;
   int idx[3] = {i, j, k};
@@ -477,6 +495,11 @@ static void neighbour(const orc* o, const double* Ug, int i, int j, int k, int d
   if (idx[d] < 0 || idx[d] >= n) {
     int bc = o->bc[2 * d + (s > 0 ? 1 : 0)];
     if (bc == ORC_BC_PERIODIC) idx[d] = (idx[d] + n) % n;
+    else if (bc == ORC_BC_INFLOW) {          /* A20: the ghost holds the prescribed incoming state */
+      const double* q = o->inflow[2 * d + (s > 0 ? 1 : 0)][g];
+      for (int c = 0; c < 4; c++) out[c] = q[c];
+      return;
+    }
     else {                                   /* transmissive: copy self; reflective: + flux inversion */
       idx[d] = (d == 0 ? i : d == 1 ? j : k);
       flip = (bc == ORC_BC_REFLECTIVE);
@@ -573,8 +596,8 @@ int orc_step(orc* o, double dt, int n_steps, orc_diag* diag)
             size_t id = (size_t)i + (size_t)n * (j + (size_t)n * k);
             double Um[3][4], Up[3][4], faceN[6];
             for (int d = 0; d < 3; d++) {
-              neighbour(o, Ug, i, j, k, d, -1, Um[d]);
-              neighbour(o, Ug, i, j, k, d, +1, Up[d]);
+              neighbour(o, Ug, g, i, j, k, d, -1, Um[d]);
+              neighbour(o, Ug, g, i, j, k, d, +1, Up[d]);
             }
             transport_core(o->flux, c, dt, dx, Ug + 4 * id, Um, Up, Vg + 4 * id, faceN);
             /* net photon flux through non-periodic box faces (A15) */

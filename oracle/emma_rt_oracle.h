@@ -20,7 +20,8 @@ extern "C" {
 
 #define ORC_MAX_GROUPS 4
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ENONFINITE = -4, ORC_ECFL = -6, ORC_ESUBCYCLE = -7 };
-enum { ORC_BC_PERIODIC = 0, ORC_BC_TRANSMISSIVE = 1, ORC_BC_REFLECTIVE = 2 };          /* PAPER.md:436 */
+enum { ORC_BC_PERIODIC = 0, ORC_BC_TRANSMISSIVE = 1, ORC_BC_REFLECTIVE = 2,            /* PAPER.md:436 */
+       ORC_BC_INFLOW = 3 };   /* A20: ghost = a prescribed state (the plane-parallel flux of PAPER.md:562 entering a face) */
 enum { ORC_F_U = 0, ORC_F_N = 1, ORC_F_F = 2, ORC_F_X = 3, ORC_F_T = 4, ORC_F_E = 5, ORC_F_N0 = 6,
        ORC_F_SUBCYCLES = 7, ORC_F_XNEUTRAL = 8 };
 enum { ORC_FLUX_GLF = 0, ORC_FLUX_HLL = 1 };        /* Eq. 32 (PAPER.md:246) / reading A19 (PAPER.md:250) */
@@ -81,6 +82,7 @@ orc* orc_create(int n, const int bc[6], int chemistry, const orc_phys* ph, doubl
                 int n_levels, const int64_t* n_octs, const int64_t* const* parent,
                 const float* const* U0, const float* const* n0, const float* const* x, const float* const* T);
 int  orc_set_sources(orc*, int64_t n_src, const double* pos_box, const double* Q);
+int  orc_set_inflow(orc*, int face, int group, const double U[4]);   /* ghost (N, Fx, Fy, Fz) of an INFLOW face */
 int  orc_set_flux(orc*, int flux);          /* interface flux of the transport sweep; default ORC_FLUX_GLF */
 int  orc_step(orc*, double dt, int n_steps, orc_diag* diag_last);
 int  orc_read(const orc*, int field, int level, int group, double* dst, int64_t n_dst);

@@ -8,4 +8,4 @@ from .binding import (EmmaRT, EmmaRTError, emma_rt_arena_bytes, emma_rt_init, em
                       emma_rt_read, emma_rt_write, emma_rt_free, emma_rt_dt_cfl, lib, lib_path, Config, Diag,
                       FIELD_U, FIELD_N, FIELD_F, FIELD_X, FIELD_T, FIELD_E, FIELD_N0, FIELD_SUBCYCLES, FIELD_XNEUTRAL,
                       OK, EINVAL, ENOMEM, ECUDA, ENONFINITE, ESTATE, ECFL, ESUBCYCLE, EXPORTED_SYMBOLS,
-                      FLUX_GLF, FLUX_HLL)
+                      FLUX_GLF, FLUX_HLL, BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW)

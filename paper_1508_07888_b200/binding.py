@@ -18,8 +18,9 @@ _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYC
 
 EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources", "emma_rt_dt_cfl", "emma_rt_step",
                     "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
-                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_last_error", "emma_rt_free"]
+                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_set_inflow", "emma_rt_last_error", "emma_rt_free"]
 FLUX_GLF, FLUX_HLL = 0, 1
+BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
 KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused"]
 
 
@@ -96,6 +97,8 @@ def lib():
     L.emma_rt_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.emma_rt_set_schedule.restype = C.c_int
     L.emma_rt_set_schedule.argtypes = [C.c_void_p, C.c_int32]
+    L.emma_rt_set_inflow.restype = C.c_int
+    L.emma_rt_set_inflow.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
     L.emma_rt_set_flux.restype = C.c_int
     L.emma_rt_set_flux.argtypes = [C.c_void_p, C.c_int32]
     L.emma_rt_last_error.restype = C.c_char_p
@@ -227,6 +230,8 @@ class EmmaRT:
             self.set_schedule(fused)
         if flux is not None:
             self._check(lib().emma_rt_set_flux(self.h, int(flux)))
+        for (face, group), U in (getattr(w, "inflow", None) or {}).items():
+            self.set_inflow(face, group, U)
         if w.src_pos is not None and len(w.src_pos):
             self._check(emma_rt_set_sources(self.h, w.src_pos, w.src_Q))
 
@@ -249,6 +254,11 @@ class EmmaRT:
 
     def kernel_launches(self):
         return lib().emma_rt_kernel_launches(self.h)
+
+    def set_inflow(self, face, group, U):
+        """Ghost state (N, Fx, Fy, Fz) [cgs] of a BC_INFLOW face (0..5 = -x,+x,-y,+y,-z,+z)."""
+        a = (C.c_double * 4)(*[float(v) for v in U])
+        self._check(lib().emma_rt_set_inflow(self.h, int(face), int(group), a))
 
     def set_schedule(self, fused):
         """fused=1 (default): single-pass transport + chemistry; 0: separate passes."""

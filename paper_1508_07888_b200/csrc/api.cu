@@ -46,7 +46,7 @@ bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
   if (!c || c->struct_size != sizeof(emma_rt_config) || c->abi_version != EMMA_RT_ABI_VERSION) return false;
   if (c->n_coarse < 2 || c->n_coarse > 1290 || c->n_groups < 1 || c->n_groups > MAXG) return false;
   for (int f = 0; f < 6; f++)
-    if (c->bc[f] < 0 || c->bc[f] > 2) return false;
+    if (c->bc[f] < 0 || c->bc[f] > EMMA_RT_BC_INFLOW) return false;
   for (int d = 0; d < 3; d++)                                   // periodic faces come in pairs
     if ((c->bc[2 * d] == EMMA_RT_BC_PERIODIC) != (c->bc[2 * d + 1] == EMMA_RT_BC_PERIODIC)) return false;
   if (!(c->box_len_cm > 0) || !(c->c_red_cm_s > 0) || !(c->e_tol > 0) || c->max_halvings < 0) return false;
@@ -117,6 +117,7 @@ struct emma_rt {
   TransportMaps tmaps_f[2];                    // the same with the fused pass's tile height
   int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
   int flux;                                    // interface flux of the transport update (emma_rt_set_flux)
+  float4 inflow[6][MAXG];                      // ghost state (N, phi) of inflow faces (emma_rt_set_inflow)
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
@@ -206,7 +207,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   make_layout(s, h->lay);
   h->arena = (char*)arena_dev;
   h->st = (cudaStream_t)cfg->stream;
-  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr; h->fused = 1; h->flux = EMMA_RT_FLUX_GLF;
+  h->cur = 0; h->t_sim = 0; h->launches = 0; h->diag_pinned = nullptr; h->fused = 1; h->flux = EMMA_RT_FLUX_GLF; memset(h->inflow, 0, sizeof h->inflow);
   h->prof.st = h->st;
   h->dx = cfg->box_len_cm / s.n;
   *out = h;                                    // returned even on failure so the caller can read last_error
@@ -360,7 +361,9 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
 
   TransportParams tp;
   tp.n = s.n; tp.G = s.G;
-  for (int f = 0; f < 6; f++) tp.bc[f] = h->cfg.bc[f];
+  bool any_inflow = false;
+  for (int f = 0; f < 6; f++) { tp.bc[f] = h->cfg.bc[f]; any_inflow = any_inflow || h->cfg.bc[f] == EMMA_RT_BC_INFLOW; }
+  memcpy(tp.inflow, h->inflow, sizeof tp.inflow);
   tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
   // z chunks.  Every CTA costs (its planes + ~3 planes of prologue) and the SMs hold `per_sm` CTAs each, so a launch
   // takes ceil(blocks / (per_sm SMs)) rounds of (zchunk + 3) plane-times: pick the chunk count that minimises that
@@ -386,7 +389,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   if (!pick_zchunks(tp, tp.tiles_x * tp.tiles_y * s.G, 2)) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
   tp.nst = getenv("EMMA_RT_TUNE_NST") ? atoi(getenv("EMMA_RT_TUNE_NST")) : 6;
   tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
-  const bool use_tma = getenv("EMMA_RT_TUNE_TMA") ? atoi(getenv("EMMA_RT_TUNE_TMA")) != 0 : true;
+  const bool use_tma = !any_inflow && (getenv("EMMA_RT_TUNE_TMA") ? atoi(getenv("EMMA_RT_TUNE_TMA")) != 0 : true);
   tp.want_total = h->cfg.chemistry ? 0 : 1;
   tp.nu = (float)(c * dt / h->dx);
   tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
@@ -407,7 +410,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   const bool hll = h->flux == EMMA_RT_FLUX_HLL;
   TransportParams hp = tp;                     // HLL pass (transport_hll.cu): one group per CTA, one CTA per SM
   if (hll && !pick_zchunks(hp, hp.tiles_x * hp.tiles_y * s.G, hll_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
-  const bool fused = !hll && h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
+  const bool fused = !hll && !any_inflow && h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
   TransportParams fp = tp;
   fp.tiles_y = (s.n + fused_tile_y() - 1) / fused_tile_y();
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
@@ -585,6 +588,17 @@ int emma_rt_set_schedule(emma_rt* h, int32_t fused)
   if (!h) return EMMA_RT_EINVAL;
   if (fused != 0 && fused != 1) return fail(h, EMMA_RT_EINVAL, "fused must be 0 or 1");
   h->fused = fused;
+  return EMMA_RT_OK;
+}
+
+int emma_rt_set_inflow(emma_rt* h, int32_t face, int32_t group, const double U[4])
+{
+  if (!h || !U) return EMMA_RT_EINVAL;
+  if (face < 0 || face > 5 || group < 0 || group >= h->sh.G) return fail(h, EMMA_RT_EINVAL, "face in 0..5, group in range");
+  if (h->cfg.bc[face] != EMMA_RT_BC_INFLOW) return fail(h, EMMA_RT_EINVAL, "face %d is not an inflow face", (int)face);
+  const double c = h->cfg.c_red_cm_s;
+  for (int q = 0; q < 4; q++) if (!std::isfinite(U[q])) return fail(h, EMMA_RT_EINVAL, "non-finite inflow state");
+  h->inflow[face][group] = make_float4((float)U[0], (float)(U[1] / c), (float)(U[2] / c), (float)(U[3] / c));
   return EMMA_RT_OK;
 }
 

@@ -74,6 +74,7 @@ struct TransportParams {
   int want_total;          // 1 when chemistry is off: the transport pass also sums N dV
   float nu;                // c_red dt / dx
   float c0, c1;            // 1 - 3 nu and nu / 2, rounded once from fp64
+  float4 inflow[6][MAXG];  // ghost state (N, phi) of EMMA_RT_BC_INFLOW faces, per group (reading A20)
   double dV;
 };
 

@@ -50,7 +50,7 @@ struct Tile {                                  // per-thread constants of the ma
 };
 
 // DIAG: chemistry is off, so this pass owns the step's photon total and non-finite scan.
-// OPEN: some face is transmissive, so the pass sums the outflow of A15.
+// OPEN: some face is transmissive or an inflow face (A20), so the pass sums the outflow of A15 (and inflow ghosts exist).
 template <bool DIAG, bool OPEN>
 __global__ void __launch_bounds__(NT, 2)
 transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4* __restrict__ Uout,
@@ -106,6 +106,19 @@ transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4
   }
   T.hsgn_y = (hflipc == 1) ? -1.f : 1.f;
   T.hsgn_z = (hflipc == 2) ? -1.f : 1.f;
+  // inflow faces (A20): the ghost is a prescribed state, not a cell of the grid
+  bool hin = false;
+  float4 hval = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (OPEN && T.hduty) {
+    int face = -1;
+    if (t < wy) { if (x0 == 0) face = 0; }
+    else if (t < 2 * wy) { if (x0 + wx == n) face = 1; }
+    else if (t - 2 * wy < wx) { if (y0 == 0) face = 2; }
+    else { if (y0 + wy == n) face = 3; }
+    if (face >= 0 && p.bc[face] == EMMA_RT_BC_INFLOW) { hin = true; hval = p.inflow[face][g]; }
+  }
+  const bool zin_lo = OPEN && z0 == 0 && p.bc[4] == EMMA_RT_BC_INFLOW;
+  const bool zin_hi = OPEN && z1 == n && p.bc[5] == EMMA_RT_BC_INFLOW;
 
   const int pfd = p.pf;
   const float c0 = p.c0, c1 = p.c1;
@@ -129,9 +142,11 @@ transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4
     if (T.act0) { m0 = __ldg(pm + col0); A.u0 = __ldg(pc + col0); B.u0 = __ldg(pn + col0); }
     if (T.act1) { m1 = __ldg(pm + col1); A.u1 = __ldg(pc + col1); B.u1 = __ldg(pn + col1); }
     if (T.hduty) {
-      A.h = __ldg(pc + hcol);
-      if (z0 + 1 < z1) B.h = __ldg(pn + hcol);
+      A.h = hin ? hval : __ldg(pc + hcol);
+      if (z0 + 1 < z1) B.h = hin ? hval : __ldg(pn + hcol);
     }
+    if (zin_lo) m0 = m1 = p.inflow[4][g];
+    if (zin_hi && z0 + 1 >= z1) B.u0 = B.u1 = p.inflow[5][g];
     if (flz) { m0.w = -m0.w; m1.w = -m1.w; }
     float a, b;
     closure_ab(m0, a, b); W0 = below_z(m0, a, b);
@@ -166,7 +181,8 @@ transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4
       const float4* q = last2 ? ptop : pld;
       if (T.act0) NEW.u0 = __ldg(q);
       if (T.act1) NEW.u1 = __ldg(q + d1);
-      if (T.hduty && !last2) NEW.h = __ldg(q + dh);
+      if (last2 && zin_hi) NEW.u0 = NEW.u1 = p.inflow[5][g];
+      if (T.hduty && !last2) NEW.h = hin ? hval : __ldg(q + dh);
     }
     // (b') L2 prefetch of plane z+2+pfd: own cells and the halo cell (the halo columns are 32 separate sectors per
     // warp load, the slowest request of the plane).  Measured at 512^3 x 3: 4.19 -> 4.64 TB/s.
@@ -244,6 +260,21 @@ transport_kernel(const TransportParams p, const float4* __restrict__ Uin, float4
         if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u0.w;
         if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u0.w;
       }
+      // inflow faces: the GLF face flux of Eq. 32 with the prescribed ghost, N-component (in units of c)
+      auto in_lo = [&](const float4& c, float pc_, const float4& gst, float pg) { return 0.5 * ((double)pg + pc_) - 0.5 * ((double)c.x - gst.x); };
+      auto in_hi = [&](const float4& c, float pc_, const float4& gst, float pg) { return 0.5 * ((double)pc_ + pg) - 0.5 * ((double)gst.x - c.x); };
+      for (int k = 0; k < 2; k++) {
+        const bool a = k ? T.act1 : T.act0;
+        if (!a) continue;
+        const float4& c = k ? CUR.u1 : CUR.u0;
+        const int yy = y + k;
+        if (x == 0 && p.bc[0] == EMMA_RT_BC_INFLOW) acc_d.outflow -= in_lo(c, c.y, p.inflow[0][g], p.inflow[0][g].y);
+        if (x == n - 1 && p.bc[1] == EMMA_RT_BC_INFLOW) acc_d.outflow += in_hi(c, c.y, p.inflow[1][g], p.inflow[1][g].y);
+        if (yy == 0 && p.bc[2] == EMMA_RT_BC_INFLOW) acc_d.outflow -= in_lo(c, c.z, p.inflow[2][g], p.inflow[2][g].z);
+        if (yy == n - 1 && p.bc[3] == EMMA_RT_BC_INFLOW) acc_d.outflow += in_hi(c, c.z, p.inflow[3][g], p.inflow[3][g].z);
+        if (z == 0 && p.bc[4] == EMMA_RT_BC_INFLOW) acc_d.outflow -= in_lo(c, c.w, p.inflow[4][g], p.inflow[4][g].w);
+        if (z == n - 1 && p.bc[5] == EMMA_RT_BC_INFLOW) acc_d.outflow += in_hi(c, c.w, p.inflow[5][g], p.inflow[5][g].w);
+      }
       if (T.act1) {
         if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)CUR.u1.y;
         if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)CUR.u1.y;
@@ -282,7 +313,7 @@ int launch_transport(const TransportParams& p, const float4* Uin, float4* Uout, 
 {
   const int nblk = p.tiles_x * p.tiles_y * p.nzc * p.G;
   bool open = false;
-  for (int f = 0; f < 6; f++) open = open || (p.bc[f] == EMMA_RT_BC_TRANSMISSIVE);
+  for (int f = 0; f < 6; f++) open = open || (p.bc[f] == EMMA_RT_BC_TRANSMISSIVE) || (p.bc[f] == EMMA_RT_BC_INFLOW);
   const bool diag = p.want_total != 0;
   if (diag && open) transport_kernel<true, true><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);
   else if (diag) transport_kernel<true, false><<<nblk, NT, 0, st>>>(p, Uin, Uout, parts);

@@ -10,7 +10,7 @@
 // -- algebraically the textbook radicand (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) with mu f = r_d and
 // (2 - xi)/f^2 = 3/(2 + xi); this form has no cancellation at f -> 1 and no 0/0 at f -> 0.  l+ = -l- = 1 gives Eq. 32.
 // The update is U' = U - nu sum_d (H_{d+1/2} - H_{d-1/2}).  If l+ = l- (= 0: both cells stream exactly along the face)
-// the flux vectors vanish too and H = 0.
+// the flux vectors vanish too and H = 0.  The updated state is kept realizable (A19): |phi'| > N' -> phi' := max(N',0) phi'/|phi'|.
 //
 // Shape: as fused.cu with one group per CTA -- 512 threads own a 32 x 16 column, one cell each, and march along z
 // through a TMA-fed ring of planes (j-1, j, j+1 resident, the rest in flight).  Per cell the closure (a, b) and the six
@@ -85,7 +85,9 @@ __device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL,
   if (D == 0) { GL.y += aL; GR.y += aR; } else if (D == 1) { GL.z += aL; GR.z += aR; } else { GL.w += aL; GR.w += aR; }
   const float lp = fmaxf(0.f, fmaxf(lpL, lpR)), lm = fminf(0.f, fminf(lmL, lmR));
   const float den = lp - lm;
-  const float inv = (den > 0.f) ? frcp(den) : 0.f;
+  // l+ = l- = 0 (both cells stream exactly along the face): G vanishes there too and H = 0.  The guard also covers a
+  // denormal den (transverse speeds of ~1e-38 from rounding dust in phi), whose approximate reciprocal is inf
+  const float inv = (den > 1e-20f) ? frcp(den) : 0.f;
   const float wl = lp * inv, wr = -lm * inv, wd = lp * lm * inv;
   float4 H;
   H.x = fmaf(wl, GL.x, fmaf(wr, GR.x, wd * (UR.x - UL.x)));
@@ -139,8 +141,15 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
   // mirrored state (face-normal component negated)
   int hoff = -1;
   float hsx = 1.f, hsy = 1.f;
+  bool hin = false;                            // my halo cell is the ghost of an inflow face (A20): a prescribed state
+  float4 hval = make_float4(0.f, 0.f, 0.f, 0.f);
   {
     const int nh = 2 * wy + 2 * wx, h = lane * (NT / 32) + warp;
+    if (BCGEN && h < nh) {
+      const int face = (h < wy) ? (x0 == 0 ? 0 : -1) : (h < 2 * wy) ? (x0 + wx == n ? 1 : -1)
+                     : (h < 2 * wy + wx) ? (y0 == 0 ? 2 : -1) : (y0 + wy == n ? 3 : -1);
+      if (face >= 0 && p.bc[face] == EMMA_RT_BC_INFLOW) { hin = true; hval = p.inflow[face][g]; }
+    }
     if (h < nh) {
       if (h < wy) { hoff = STAGE_ROWS + h * 16; if (BCGEN && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) hsx = -1.f; }
       else if (h < 2 * wy) { hoff = STAGE_ROWS + COLB + (h - wy) * 16; if (BCGEN && x0 + wx == n && p.bc[1] == EMMA_RT_BC_REFLECTIVE) hsx = -1.f; }
@@ -149,6 +158,8 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     }
   }
 
+  const bool zin_lo = BCGEN && z0 == 0 && p.bc[4] == EMMA_RT_BC_INFLOW;
+  const bool zin_hi = BCGEN && z1 == n && p.bc[5] == EMMA_RT_BC_INFLOW;
   bool flz, fltop, fl;
   const int zm = bc_map(z0 - 1, n, p.bc[4], p.bc[5], flz);
   const int ztop = bc_map(z1, n, p.bc[4], p.bc[5], fltop);
@@ -181,9 +192,10 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
   float4* pst = Uout + ((size_t)g * n + z0) * plane + (act ? ((size_t)y * n + x) : 0);
   Acc acc_d;
 
-  auto halo_aux = [&](const unsigned char* st, unsigned char* aux) {
+  auto halo_aux = [&](unsigned char* st, unsigned char* aux) {
     if (hoff >= 0) {
       float4 h = *(const float4*)(st + hoff);
+      if (BCGEN && hin) { h = hval; *(float4*)(st + hoff) = h; }        // consumers read the ghost from the stage
       if (BCGEN) { h.y *= hsx; h.z *= hsy; }
       store_aux(aux, hoff, make_aux(h));
     }
@@ -193,6 +205,7 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
   {
     mbar_wait(bar0, 0);
     float4 m = *(const float4*)(smem + own);
+    if (BCGEN && zin_lo) m = p.inflow[4][g];
     if (BCGEN && flz) m.w = -m.w;
     store_aux(sAUX, own, make_aux(m));
     mbar_wait(bar0 + 8, 0);
@@ -213,7 +226,7 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     }
     const unsigned char* sb = smem + s_blw * SG;
     const unsigned char* sc = smem + s_cur * SG;
-    const unsigned char* sn = smem + s_nxt * SG;
+    unsigned char* sn = smem + s_nxt * SG;
     unsigned char* AXb = sAUX + ab_blw * AUXB;                         // aux of plane j-1; receives plane j+1
     const unsigned char* AXc = sAUX + ab_cur * AUXB;
     mbar_wait(bar0 + 8 * s_nxt, par_nxt);
@@ -224,11 +237,13 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     const float4 c0 = *(const float4*)(AXc + own), c1 = *(const float4*)(AXc + SG + own);
     // the plane above: aux now (kept for the z face, staged for the next plane)
     float4 un = *(const float4*)(sn + own);
+    if (BCGEN && top && zin_hi) un = p.inflow[5][g];
     if (BCGEN && top && fltop) un.w = -un.w;
     const Aux An = make_aux(un);
     if (j == 0) {
       // the face below the chunk: flux from the plane below (afterwards it is carried from plane to plane)
       float4 ub = *(const float4*)(sb + own);
+      if (BCGEN && zin_lo) ub = p.inflow[4][g];
       if (BCGEN && flz) ub.w = -ub.w;
       const float4 b0 = *(const float4*)(AXb + own), b1 = *(const float4*)(AXb + SG + own);
       Hzm = hll_face<2>(ub, b0.x, b0.y, b1.z, b1.w, cu, c0.x, c0.y, c1.z, c1.w);
@@ -257,6 +272,11 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     o.y = fmaf(-nu, (Hxp.y - Hxm.y) + (Hyp.y - Hym.y) + (Hzp.y - Hzm.y), cu.y);
     o.z = fmaf(-nu, (Hxp.z - Hxm.z) + (Hyp.z - Hym.z) + (Hzp.z - Hzm.z), cu.z);
     o.w = fmaf(-nu, (Hxp.w - Hxm.w) + (Hyp.w - Hym.w) + (Hzp.w - Hzm.w), cu.w);
+    const float Hz_lo = Hzm.x;
+    {                                          // A19: keep the state realizable, |phi| <= max(N, 0)
+      const float p2 = fmaf(o.y, o.y, fmaf(o.z, o.z, o.w * o.w)), Np = fmaxf(o.x, 0.f);
+      if (p2 > Np * Np) { const float sc = Np * rsqrtf(p2); o.y *= sc; o.z *= sc; o.w *= sc; }
+    }
     Hzm = Hzp;
     if (act) {
       *pst = o;
@@ -265,15 +285,15 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
         acc_d.total += (double)o.x;
       }
       if (BCGEN) {
-        // outflow through open faces (A15): with ghost = own cell the HLL flux is the cell's own G_d, N-component
-        // phi_d; through a reflective face it is 0 (mirror states: l- = -l+, the phi_d cancel, N_R = N_L)
+        // outflow through non-periodic faces (A15): the N-component of the face fluxes just evaluated (transmissive:
+        // the cell's own phi_d; reflective: 0 up to rounding; inflow: negative while light enters)
         const int z = z0 + j;
-        if (x == 0 && p.bc[0] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.y;
-        if (x == n - 1 && p.bc[1] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.y;
-        if (y == 0 && p.bc[2] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.z;
-        if (y == n - 1 && p.bc[3] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.z;
-        if (z == 0 && p.bc[4] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow -= (double)cu.w;
-        if (z == n - 1 && p.bc[5] == EMMA_RT_BC_TRANSMISSIVE) acc_d.outflow += (double)cu.w;
+        if (x == 0 && p.bc[0] != EMMA_RT_BC_PERIODIC) acc_d.outflow -= (double)Hxm.x;
+        if (x == n - 1 && p.bc[1] != EMMA_RT_BC_PERIODIC) acc_d.outflow += (double)Hxp.x;
+        if (y == 0 && p.bc[2] != EMMA_RT_BC_PERIODIC) acc_d.outflow -= (double)Hym.x;
+        if (y == n - 1 && p.bc[3] != EMMA_RT_BC_PERIODIC) acc_d.outflow += (double)Hyp.x;
+        if (z == 0 && p.bc[4] != EMMA_RT_BC_PERIODIC) acc_d.outflow -= (double)Hz_lo;
+        if (z == n - 1 && p.bc[5] != EMMA_RT_BC_PERIODIC) acc_d.outflow += (double)Hzp.x;
       }
     }
     pst += plane;

@@ -122,4 +122,10 @@ def transport_periodic_hll(U, c, dt, dx):
         with np.errstate(divide="ignore", invalid="ignore"):
             Fh = np.where(den > 0, (lp * Ft - lm * up(Ft) + lp * lm * (up(U) - U)) / den, 0.5 * (Ft + up(Ft)))
         out -= dt / dx * (Fh - np.roll(Fh, +1, axis=axis))
+    # A19: the updated state is kept realizable, |F| <= c max(N, 0)
+    Fn = np.sqrt((out[..., 1:] ** 2).sum(-1))
+    lim = c * np.maximum(out[..., 0], 0.0)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        scale = np.where(Fn > lim, lim / Fn, 1.0)
+    out[..., 1:] *= scale[..., None]
     return out

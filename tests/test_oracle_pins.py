@@ -619,20 +619,22 @@ def test_H5_hll_bruteforce_transcription_and_conservation(oracle_mod, n, G, seed
     for g in range(G):
         U = o.read(O.F_U, 0, g).reshape(n, n, n, 4)
         scale = np.abs(Ub[g][..., 0]).max()
-        assert np.abs(U[..., 0] - Ub[g][..., 0]).max() <= 1e-10 * scale
-        assert np.abs(U[..., 1:] - Ub[g][..., 1:]).max() <= 1e-10 * c * scale
+        # 1e-8: at f -> 1 (the limiter of A19 puts states there) the speeds are sqrt-sensitive, the two algebraic forms of the
+        # radicand differ by ~sqrt(eps)
+        assert np.abs(U[..., 0] - Ub[g][..., 0]).max() <= 1e-8 * scale
+        assert np.abs(U[..., 1:] - Ub[g][..., 1:]).max() <= 1e-8 * c * scale
         assert U[..., 0].sum() == pytest.approx(U0[g, :, 0].astype(np.float64).sum(), rel=1e-12)
 
 
 def test_H6_hll_is_less_diffusive_than_glf(oracle_mod):
     """HLL is 'less diffusive' than GLF, whose weak shadows come from light leaking sideways.  A beam
     of finite width along x: after 10 steps the photons found outside the beam's own rows are far fewer with HLL."""
-    n, c = 16, C_RED
-    U0 = np.zeros((1, n, n, n, 4))
+    n, c = 16, 2.0 ** 31                        # power-of-two speed: F = c N is exact in fp32, so f = 1, not 1 + 1e-8
+    U0 = np.zeros((1, n, n, n, 4))              # (a non-realizable f > 1 would take the -/+c bounds of A19)
     U0[0, 6:10, 6:10, :, 0] = 1.0
     U0[0, 6:10, 6:10, :, 1] = c
     U0 = U0.reshape(1, n ** 3, 4).astype(np.float32)
-    w = tiny_workload(n, 1, U0=U0, chemistry=0)
+    w = tiny_workload(n, 1, U0=U0, c_red=c, chemistry=0)
     leak = {}
     for name, fl in (("glf", O.FLUX_GLF), ("hll", O.FLUX_HLL)):
         o = O.Oracle(w, flux=fl)

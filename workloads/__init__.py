@@ -10,4 +10,4 @@ Recipes follow SURVEY.md section 8(d); DESIGN.md "Input recipe" restates them.
 from .constants import CGS                                    # noqa: F401
 from .groups import blackbody_groups, sigma_HI                # noqa: F401
 from .fields import gaussian_random_field, lognormal_density  # noqa: F401
-from .configs import make_config, make_hii_region_corner, Workload, refine_by_density  # noqa: F401
+from .configs import make_config, make_hii_region_corner, make_shadow_clump, Workload, refine_by_density  # noqa: F401

@@ -19,7 +19,7 @@ from .groups import blackbody_groups
 
 SEED_BASE = 150807888          # arXiv id 1508.07888; seed = SEED_BASE + config number
 
-BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE = 0, 1, 2
+BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
 
 
 @dataclass
@@ -49,6 +49,8 @@ class Workload:
     # sources
     src_pos: np.ndarray = None  # [n_src,3] float64 in [0,1)
     src_Q: np.ndarray = None    # [n_src,G] float64 photons/s
+    # prescribed ghost state of BC_INFLOW faces: {(face, group): (N, Fx, Fy, Fz) in cgs}  (reading A20)
+    inflow: dict = None
     # stepping
     courant: float = 0.9
     n_steps: int = 1
@@ -270,5 +272,29 @@ def make_hii_region_corner(n=64, n_steps=200):
     w.T = [np.full(ncell, 100.0, np.float32)]
     w.src_pos = np.array([[0.5 / n, 0.5 / n, 0.5 / n]], np.float64)
     w.src_Q = 5e48 * np.asarray(gr["frac"], np.float64)[None, :]
+    w.n_steps = n_steps
+    return w
+
+
+def make_shadow_clump(n=32, n_steps=200):
+    """the static-gas cousin of the paper's clump photo-evaporation test (section
+    6.5, after Iliev et al. 2009): 6.6 kpc box, a dense clump (0.04 cm^-3, 100 K) of radius 0.8 kpc centred on
+    (5.4, 3.3, 3.3) kpc in a thin medium (2e-4 cm^-3, 8000 K), a plane-parallel 1e5 K black-body flux of 1e6 photons
+    cm^-2 s^-1 (1e10 m^-2 s^-1) entering through the x = 0 face (BC_INFLOW), the opposite face transmissive, the other
+    directions periodic.  3 groups, c~ = c/10.  The gas does not move here (hydrodynamics is out of scope)."""
+    gr = _groups(3)
+    L = 6.6 * CGS.kpc
+    c_red = 0.1 * CGS.c
+    w = Workload("shadow-clump-static", n, 3, L, c_red, gr["sigma_N"], gr["sigma_E"], gr["E_mean"], gr["frac"],
+                 bc=(BC_INFLOW, BC_TRANSMISSIVE, BC_PERIODIC, BC_PERIODIC, BC_PERIODIC, BC_PERIODIC))
+    ctr = (np.arange(n) + 0.5) * (6.6 / n)                               # cell centres [kpc]
+    X, Y, Z = np.meshgrid(ctr, ctr, ctr, indexing="ij")                  # arrays indexed [ix, iy, iz]
+    inside = ((X - 5.4) ** 2 + (Y - 3.3) ** 2 + (Z - 3.3) ** 2) <= 0.8 ** 2
+    to_id = lambda a: np.ascontiguousarray(a.transpose(2, 1, 0)).reshape(-1)   # cell id = ix + n (iy + n iz)
+    w.n0 = [to_id(np.where(inside, 0.04, 2e-4)).astype(np.float32)]
+    w.T = [to_id(np.where(inside, 100.0, 8000.0)).astype(np.float32)]
+    w.x = [np.full(n ** 3, 1.2e-3, np.float32)]
+    F = 1.0e6
+    w.inflow = {(0, g): (F * gr["frac"][g] / c_red, F * gr["frac"][g], 0.0, 0.0) for g in range(3)}
     w.n_steps = n_steps
     return w
