@@ -107,6 +107,12 @@ def lib():
     L.orc_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.orc_free.restype = None
     L.orc_free.argtypes = [C.c_void_p]
+    L.orc_set_amr_transport.restype = C.c_int
+    L.orc_set_amr_transport.argtypes = [C.c_void_p, C.c_int]
+    L.orc_write_U.restype = C.c_int
+    L.orc_write_U.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+    L.orc_restrict_U.restype = C.c_int
+    L.orc_restrict_U.argtypes = [C.c_void_p]
     _lib = L
     return L
 
@@ -235,6 +241,17 @@ class Oracle:
         """Ghost state (N, Fx, Fy, Fz) [cgs] of a BC_INFLOW face (0..5 = -x,+x,-y,+y,-z,+z), reading A20."""
         U = np.ascontiguousarray(U, np.float64).reshape(4)
         return lib().orc_set_inflow(self.h, int(face), int(group), _dp(U))
+
+    def set_amr_transport(self, on=True):
+        """Standard (non-CRTA) AMR transport of reading A21."""
+        return lib().orc_set_amr_transport(self.h, int(bool(on)))
+
+    def write_U(self, level, group, U):
+        U = np.ascontiguousarray(U, np.float64).reshape(self.level_cells(level), 4)
+        return lib().orc_write_U(self.h, int(level), int(group), _dp(U))
+
+    def restrict_U(self):
+        return lib().orc_restrict_U(self.h)
 
     def set_sources(self, pos, Q):
         pos = np.ascontiguousarray(pos, np.float64).reshape(-1, 3)

@@ -321,6 +321,11 @@ struct orc {
   double t_sim;
   int64_t cnt_transport_cells[8];  /* cells swept by the transport engine, per level (CRTA: level 0 only) */
   int64_t cnt_chem_cells[8];       /* leaf cells swept by the chemistry engine, per level */
+  /* standard (non-CRTA) AMR transport, reading A21; see the section at the end of this file */
+  int amr;                         /* 0: CRTA (default); 1: level-by-level transport on every level */
+  double* Ul[8];                   /* l >= 1: radiation of level l, [G][ncell_l][4] (level 0 lives in U[cur]) */
+  double* dep[8];                  /* per level: change deposited into leaf cells by the fluxes of the finer level */
+  int32_t* coord[8];               /* [ncell_l][3] integer cell coordinates on level l, in [0, n 2^l) */
 };
 
 int orc_set_flux(orc* o, int flux)
@@ -359,6 +364,7 @@ void orc_free(orc* o)
     free(o->subc[l]); free(o->S[l]);
   }
   free(o->src_cell); free(o->src_level);
+  for (int l = 0; l < 8; l++) { free(o->Ul[l]); free(o->dep[l]); free(o->coord[l]); }
   free(o);
 }
 
@@ -567,8 +573,11 @@ static void cell_update(orc* o, double dt, int l, int64_t cell, const double* Ui
   o->subc[l][cell] = 0;
 }
 
+static int amr_step(orc* o, double dt, int n_steps, orc_diag* diag);
+
 int orc_step(orc* o, double dt, int n_steps, orc_diag* diag)
 {
+  if (o->amr) return amr_step(o, dt, n_steps, diag);
   const int n = o->n, G = o->ph.G;
   const int64_t nc = o->ncell[0];
   const double c = o->ph.c, dx = o->dx;
@@ -672,8 +681,8 @@ int orc_read(const orc* o, int field, int level, int group, double* dst, int64_t
   const int64_t nc = o->ncell[level];
   const int G = o->ph.G;
   if (field == ORC_F_U || field == ORC_F_N || field == ORC_F_F) {
-    if (level != 0 || group < 0 || group >= G) return ORC_EINVAL;
-    const double* Ug = o->U[o->cur] + (size_t)group * nc * 4;
+    if ((level != 0 && !o->amr) || group < 0 || group >= G) return ORC_EINVAL;
+    const double* Ug = (level == 0 ? o->U[o->cur] : o->Ul[level]) + (size_t)group * nc * 4;
     int per = field == ORC_F_U ? 4 : field == ORC_F_N ? 1 : 3;
     if (n_dst < nc * per) return ORC_EINVAL;
     for (int64_t i = 0; i < nc; i++) {
@@ -695,5 +704,338 @@ int orc_read(const orc* o, int field, int level, int group, double* dst, int64_t
       default: return ORC_EINVAL;
     }
   }
+  return ORC_OK;
+}
+
+/* ================================================================================================
+ * Standard (non-CRTA) AMR transport -- SURVEY.md 8f NEXT-2, reading A21 of DESIGN.md
+ * (Eq. 49-51, Fig. 2-3; resolution jumps in the gather).
+ *
+ * Every cell of every level carries (N_g, F_g).  Levels are advanced recursively, finest first,
+ * dt_l = dt_{l-1}/2 (Eq. 50-51 with equal halves):
+ *
+ *     advance(l, dt):   if level l+1 has octs: advance(l+1, dt/2); advance(l+1, dt/2)
+ *                       transport of the LEAF cells of level l over dt     (Eq. 30, 32 / A19)
+ *                       chemistry of the LEAF cells of level l over dt     (Eq. 43-48)
+ *                       split cells of level l := mean of their 8 children (N, F, x, e, A14)
+ *
+ * Faces of a leaf cell of level l (the sequence (i)-(iii) of Fig. 3):
+ *   - neighbour is a leaf of level l: the flux of Eq. 32 between the two states at the start of the step;
+ *   - neighbour of level l is SPLIT: nothing is computed here; the cell has already been "temporarily updated"
+ *     by the fluxes of the two sub-steps of the 4 fine cells behind that face (kept in dep[l] until now);
+ *   - neighbour does not exist on level l (a leaf of level l-1; jumps are <= 1): the missing cell
+ *     is "interpolated linearly from coarse data at the position of the fine virtual cell":
+ *         U_ghost = U_c + sum_a (+-1/4) Delta_a,   Delta_a = minmod(U_c - U_{c-a}, U_{c+a} - U_c)
+ *     per component, with U_c the coarse leaf AT THE START OF ITS OWN STEP (Fig. 3: F(U^{p+1/2}_{l+1}, U^p_l)),
+ *     c+-a its neighbours on level l-1 (a split one holds its children mean, one that is coarser still is
+ *     taken piecewise constant, one outside the box follows the boundary rule of A13/A20 applied to c), the sign
+ *     given by which half of c the virtual cell sits in.  MinMod is the limiter the paper names for its slopes
+ *     (PAPER.md:167); it keeps the ghost inside the range of the coarse values, so N_ghost >= 0.
+ *     The same flux, times dt_l dx_l^2 / dx_{l-1}^3, is deposited into c with the opposite sign.
+ * Box faces follow A13 / A20 on every level.  The CFL number c dt_l / dx_l is the same on every level.
+ * ============================================================================================== */
+
+static double* amr_U(orc* o, int l) { return l == 0 ? o->U[o->cur] : o->Ul[l]; }
+
+static double minmod(double a, double b)
+{
+  if (a * b <= 0.0) return 0.0;
+  return (fabs(a) < fabs(b)) ? a : b;
+}
+
+/* the cell of level <= l that covers the level-l coordinates (ci, cj, ck); *lf = its level */
+static int64_t amr_find(const orc* o, int l, int ci, int cj, int ck, int* lf)
+{
+  const int n = o->n;
+  int64_t cell = (ci >> l) + (int64_t)n * ((cj >> l) + (int64_t)n * (ck >> l));
+  int m = 0;
+  while (m < l) {
+    int64_t oc = o->child[m][cell];
+    if (oc < 0) break;
+    m++;
+    int sh = l - m;
+    cell = 8 * oc + (((ci >> sh) & 1) + 2 * ((cj >> sh) & 1) + 4 * ((ck >> sh) & 1));
+  }
+  *lf = m;
+  return cell;
+}
+
+/* state of group g seen across face (d, s) of the level-l cell with coordinates co[]: kind = 0 a cell of level l
+ * (or a box-face ghost), 1 a split cell of level l (no flux here), 2 a coarser leaf (out = piecewise-constant
+ * value; the caller interpolates).  *nb = the neighbour cell, *lnb its level (box-face ghosts: -1). */
+static int amr_neighbour(orc* o, int l, int g, const int32_t co[3], int64_t self, int d, int s, double out[4],
+                         int64_t* nb, int* lnb)
+{
+  const int nl = o->n << l;
+  int c[3] = {co[0], co[1], co[2]};
+  c[d] += s;
+  *nb = -1; *lnb = -1;
+  if (c[d] < 0 || c[d] >= nl) {
+    int bc = o->bc[2 * d + (s > 0 ? 1 : 0)];
+    if (bc == ORC_BC_PERIODIC) c[d] = (c[d] + nl) % nl;
+    else if (bc == ORC_BC_INFLOW) {
+      for (int q = 0; q < 4; q++) out[q] = o->inflow[2 * d + (s > 0 ? 1 : 0)][g][q];
+      return 0;
+    } else {
+      const double* p = amr_U(o, l) + ((size_t)g * o->ncell[l] + self) * 4;
+      for (int q = 0; q < 4; q++) out[q] = p[q];
+      if (bc == ORC_BC_REFLECTIVE) out[1 + d] = -out[1 + d];
+      return 0;
+    }
+  }
+  int lf;
+  int64_t cell = amr_find(o, l, c[0], c[1], c[2], &lf);
+  const double* p = amr_U(o, lf) + ((size_t)g * o->ncell[lf] + cell) * 4;
+  for (int q = 0; q < 4; q++) out[q] = p[q];
+  *nb = cell; *lnb = lf;
+  if (lf < l) return 2;
+  return (l < o->n_levels && o->child[l][cell] >= 0) ? 1 : 0;
+}
+
+/* the virtual level-l cell at coordinates v[] inside the level-(l-1) leaf c, linearly interpolated */
+static void amr_ghost(orc* o, int l, int g, const int v[3], int64_t c, double out[4])
+{
+  const int lc = l - 1;
+  const double* Uc = amr_U(o, lc) + ((size_t)g * o->ncell[lc] + c) * 4;
+  const int32_t* cc = o->coord[lc] + 3 * c;
+  for (int q = 0; q < 4; q++) out[q] = Uc[q];
+  for (int a = 0; a < 3; a++) {
+    double Um[4], Up[4];
+    int64_t nb; int lnb;
+    amr_neighbour(o, lc, g, cc, c, a, -1, Um, &nb, &lnb);
+    amr_neighbour(o, lc, g, cc, c, a, +1, Up, &nb, &lnb);
+    double sgn = (v[a] & 1) ? 0.25 : -0.25;
+    for (int q = 0; q < 4; q++) out[q] += sgn * minmod(Uc[q] - Um[q], Up[q] - Uc[q]);
+  }
+}
+
+/* transport of the leaf cells of level l over dt (Eq. 30); returns the net outflow through non-periodic box faces */
+static double amr_transport_level(orc* o, int l, double dt)
+{
+  const int G = o->ph.G;
+  const int64_t nc = o->ncell[l];
+  const double c = o->ph.c, dxl = o->dx / (double)(1 << l);
+  const int nl = o->n << l;
+  double* U = amr_U(o, l);
+  double* Un = (double*)malloc(sizeof(double) * (size_t)G * nc * 4);
+  memcpy(Un, U, sizeof(double) * (size_t)G * nc * 4);
+  double of = 0.0;
+  for (int g = 0; g < G; g++)
+    for (int64_t cell = 0; cell < nc; cell++) {
+      if (l < o->n_levels && o->child[l][cell] >= 0) continue;            /* split: restricted later */
+      const int32_t* co = o->coord[l] + 3 * cell;
+      const double* U0 = U + ((size_t)g * nc + cell) * 4;
+      double out[4];
+      for (int q = 0; q < 4; q++) out[q] = U0[q];
+      for (int d = 0; d < 3; d++) {
+        double Fh[2][4];                                                  /* F_{i-1/2}, F_{i+1/2} */
+        for (int side = 0; side < 2; side++) {
+          const int s = side ? +1 : -1;
+          double Unb[4];
+          int64_t nb; int lnb;
+          int kind = amr_neighbour(o, l, g, co, cell, d, s, Unb, &nb, &lnb);
+          if (kind == 1) { for (int q = 0; q < 4; q++) Fh[side][q] = 0.0; continue; }   /* (iii): fine fluxes only */
+          if (kind == 2) {
+            int v[3] = {co[0], co[1], co[2]};
+            v[d] = (v[d] + s + nl) % nl;
+            amr_ghost(o, l, g, v, nb, Unb);
+          }
+          if (side == 0) face_flux(o->flux, Unb, U0, c, d, Fh[0]); else face_flux(o->flux, U0, Unb, c, d, Fh[1]);
+          if (kind == 2) {                                                /* (i)-(ii): the same flux updates the coarse cell */
+            double* dp = o->dep[l - 1] + ((size_t)g * o->ncell[l - 1] + nb) * 4;
+            double w = dt / (8.0 * dxl);                                  /* dt dx_l^2 / (2 dx_l)^3 */
+            for (int q = 0; q < 4; q++) dp[q] += (side ? +w : -w) * Fh[side][q];
+          }
+          if (lnb < 0 && o->bc[2 * d + side] != ORC_BC_PERIODIC)          /* box face (A15) */
+            of += (side ? +1.0 : -1.0) * Fh[side][0] * dxl * dxl * dt;
+        }
+        for (int q = 0; q < 4; q++) out[q] += (dt / dxl) * (Fh[0][q] - Fh[1][q]);
+      }
+      double* dp = o->dep[l] + ((size_t)g * nc + cell) * 4;
+      for (int q = 0; q < 4; q++) { out[q] += dp[q]; dp[q] = 0.0; }
+      if (o->flux == ORC_FLUX_HLL) {                                      /* A19: keep the state realizable */
+        double Fn = sqrt(out[1] * out[1] + out[2] * out[2] + out[3] * out[3]);
+        double lim = c * (out[0] > 0.0 ? out[0] : 0.0);
+        if (Fn > lim) for (int q = 1; q < 4; q++) out[q] *= lim / Fn;
+      }
+      for (int q = 0; q < 4; q++) Un[((size_t)g * nc + cell) * 4 + q] = out[q];
+    }
+  memcpy(U, Un, sizeof(double) * (size_t)G * nc * 4);
+  free(Un);
+  o->cnt_transport_cells[l] += nc;
+  return of;
+}
+
+/* chemistry of the leaf cells of level l over dt (Eq. 43-48), in place */
+static void amr_chem_level(orc* o, int l, double dt, acc_t* a)
+{
+  const int G = o->ph.G;
+  const int64_t nc = o->ncell[l];
+  double* U = amr_U(o, l);
+  double Uin[4 * ORC_MAX_GROUPS], Uout[4 * ORC_MAX_GROUPS];
+  for (int64_t cell = 0; cell < nc; cell++) {
+    if (l < o->n_levels && o->child[l][cell] >= 0) { o->subc[l][cell] = 0; continue; }
+    for (int g = 0; g < G; g++)
+      for (int q = 0; q < 4; q++) Uin[4 * g + q] = U[((size_t)g * nc + cell) * 4 + q];
+    leaf_update(o, dt, l, cell, Uin, Uout, a);
+    for (int g = 0; g < G; g++)
+      for (int q = 0; q < 4; q++) U[((size_t)g * nc + cell) * 4 + q] = Uout[4 * g + q];
+  }
+}
+
+/* split cells of level l := mean of their 8 children (N, F, x, e) */
+static void amr_restrict_level(orc* o, int l)
+{
+  if (l >= o->n_levels) return;
+  const int G = o->ph.G;
+  const int64_t noct = o->ncell[l + 1] / 8;
+  double v[8];
+  for (int64_t oc = 0; oc < noct; oc++) {
+    int64_t p = o->parent[l + 1][oc];
+    for (int g = 0; g < G; g++)
+      for (int q = 0; q < 4; q++) {
+        for (int k = 0; k < 8; k++) v[k] = o->Ul[l + 1][((size_t)g * o->ncell[l + 1] + 8 * oc + k) * 4 + q];
+        amr_U(o, l)[((size_t)g * o->ncell[l] + p) * 4 + q] = mean8(v);
+      }
+    o->x[l][p] = mean8(o->x[l + 1] + 8 * oc);
+    o->e[l][p] = mean8(o->e[l + 1] + 8 * oc);
+  }
+}
+
+static void amr_advance(orc* o, int l, double dt, acc_t* a, double* outflow)
+{
+  if (l < o->n_levels && o->ncell[l + 1] > 0) {
+    amr_advance(o, l + 1, 0.5 * dt, a, outflow);
+    amr_advance(o, l + 1, 0.5 * dt, a, outflow);
+  }
+  *outflow += amr_transport_level(o, l, dt);
+  amr_chem_level(o, l, dt, a);
+  amr_restrict_level(o, l);
+}
+
+static int amr_step(orc* o, double dt, int n_steps, orc_diag* diag)
+{
+  const int G = o->ph.G;
+  if (!(dt > 0.0) || n_steps < 0) return ORC_EINVAL;
+  if (3.0 * o->ph.c * dt > o->dx * (1.0 + 1e-12)) return ORC_ECFL;      /* A4; the same CFL number on every level */
+  int rc_all = ORC_OK;
+  orc_diag dg;
+  memset(&dg, 0, sizeof dg);
+  dg.dtau_min = INFINITY;
+  for (int step = 0; step < n_steps; step++) {
+    acc_t a;
+    acc_init(&a);
+    double of = 0.0;
+    amr_advance(o, 0, dt, &a, &of);
+    if (a.rc != ORC_OK && rc_all == ORC_OK) rc_all = a.rc;
+    o->t_sim += dt;
+    for (int l = 0; l < 8; l++) o->cnt_chem_cells[l] += a.leaves[l];
+    dg.photons_injected = a.injected; dg.photons_absorbed = a.absorbed; dg.photons_recomb_emitted = a.recomb;
+    dg.photons_outflow = of; dg.dtau_min = a.dtau_min;
+    dg.subcycles_total = a.nsub; dg.subcycles_max = a.nsub_max; dg.halvings_total = a.nhalv;
+  }
+  /* photons on the leaves, and the non-finite scan */
+  double tot = 0.0;
+  int64_t bad = 0;
+  for (int l = 0; l <= o->n_levels; l++) {
+    double dxl = o->dx / (double)(1 << l), dV = dxl * dxl * dxl;
+    const double* U = amr_U(o, l);
+    for (int64_t cell = 0; cell < o->ncell[l]; cell++) {
+      int leaf = !(l < o->n_levels && o->child[l][cell] >= 0);
+      for (int g = 0; g < G; g++) {
+        const double* p = U + ((size_t)g * o->ncell[l] + cell) * 4;
+        if (leaf) tot += p[0] * dV;
+        for (int q = 0; q < 4; q++) bad += !isfinite(p[q]);
+      }
+      bad += !isfinite(o->x[l][cell]) + !isfinite(o->e[l][cell]);
+    }
+  }
+  dg.photons_total = tot; dg.n_nonfinite = bad; dg.t_sim = o->t_sim;
+  if (diag) *diag = dg;
+  if (bad && rc_all == ORC_OK) rc_all = ORC_ENONFINITE;
+  return rc_all;
+}
+
+/* Switch to the standard AMR transport (A21).  Computes the cell coordinates of every level, checks that
+ * resolution jumps across faces are <= 1 (ORC_EINVAL otherwise) and gives every refined cell the
+ * radiation of its parent ("physical quantities are straightforwardly injected from coarse values"). */
+int orc_set_amr_transport(orc* o, int on)
+{
+  if (!o) return ORC_EINVAL;
+  if (!on) { o->amr = 0; return ORC_OK; }
+  const int G = o->ph.G, n = o->n;
+  for (int l = 0; l <= o->n_levels; l++) {
+    const int64_t nc = o->ncell[l];
+    size_t na = nc > 0 ? (size_t)nc : 1;
+    free(o->coord[l]); free(o->dep[l]);
+    o->coord[l] = (int32_t*)malloc(na * 3 * sizeof(int32_t));
+    o->dep[l] = (double*)calloc(na * 4 * G, sizeof(double));
+    if (l >= 1) { free(o->Ul[l]); o->Ul[l] = (double*)calloc(na * 4 * G, sizeof(double)); }
+    if (!o->coord[l] || !o->dep[l] || (l >= 1 && !o->Ul[l])) return ORC_ENOMEM;
+    if (l == 0) {
+      for (int64_t id = 0; id < nc; id++) {
+        o->coord[0][3 * id] = (int32_t)(id % n);
+        o->coord[0][3 * id + 1] = (int32_t)((id / n) % n);
+        o->coord[0][3 * id + 2] = (int32_t)(id / ((int64_t)n * n));
+      }
+    } else {
+      for (int64_t oc = 0; oc < nc / 8; oc++) {
+        int64_t p = o->parent[l][oc];
+        const int32_t* pc = o->coord[l - 1] + 3 * p;
+        for (int k = 0; k < 8; k++) {
+          int32_t* cc = o->coord[l] + 3 * (8 * oc + k);
+          cc[0] = 2 * pc[0] + (k & 1); cc[1] = 2 * pc[1] + ((k >> 1) & 1); cc[2] = 2 * pc[2] + ((k >> 2) & 1);
+          for (int g = 0; g < G; g++)
+            for (int q = 0; q < 4; q++)
+              o->Ul[l][((size_t)g * nc + 8 * oc + k) * 4 + q] = amr_U(o, l - 1)[((size_t)g * o->ncell[l - 1] + p) * 4 + q];
+        }
+      }
+    }
+  }
+  for (int l = 1; l <= o->n_levels; l++) {
+    const int nl = n << l;
+    for (int64_t cell = 0; cell < o->ncell[l]; cell++)
+      for (int d = 0; d < 3; d++)
+        for (int s = -1; s <= 1; s += 2) {
+          int c[3] = {o->coord[l][3 * cell], o->coord[l][3 * cell + 1], o->coord[l][3 * cell + 2]};
+          c[d] += s;
+          if (c[d] < 0 || c[d] >= nl) {
+            if (o->bc[2 * d + (s > 0)] != ORC_BC_PERIODIC) continue;
+            c[d] = (c[d] + nl) % nl;
+          }
+          int lf;
+          amr_find(o, l, c[0], c[1], c[2], &lf);
+          if (lf < l - 1) return ORC_EINVAL;
+        }
+  }
+  o->amr = 1;
+  return ORC_OK;
+}
+
+/* overwrite the radiation of one level and group (tests: random refined states); src is [ncell_l][4] */
+int orc_write_U(orc* o, int level, int group, const double* src)
+{
+  if (!o || level < 0 || level > o->n_levels || group < 0 || group >= o->ph.G || !src) return ORC_EINVAL;
+  if (level > 0 && !o->amr) return ORC_EINVAL;
+  double* U = amr_U(o, level) + (size_t)group * o->ncell[level] * 4;
+  for (int64_t i = 0; i < o->ncell[level] * 4; i++) U[i] = src[i];
+  return ORC_OK;
+}
+
+/* bottom-up restriction of the radiation after orc_write_U (split cells := children mean) */
+int orc_restrict_U(orc* o)
+{
+  if (!o || !o->amr) return ORC_EINVAL;
+  const int G = o->ph.G;
+  double v[8];
+  for (int l = o->n_levels - 1; l >= 0; l--)
+    for (int64_t oc = 0; oc < o->ncell[l + 1] / 8; oc++) {
+      int64_t p = o->parent[l + 1][oc];
+      for (int g = 0; g < G; g++)
+        for (int q = 0; q < 4; q++) {
+          for (int k = 0; k < 8; k++) v[k] = o->Ul[l + 1][((size_t)g * o->ncell[l + 1] + 8 * oc + k) * 4 + q];
+          amr_U(o, l)[((size_t)g * o->ncell[l] + p) * 4 + q] = mean8(v);
+        }
+    }
   return ORC_OK;
 }

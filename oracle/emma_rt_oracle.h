@@ -84,6 +84,12 @@ orc* orc_create(int n, const int bc[6], int chemistry, const orc_phys* ph, doubl
 int  orc_set_sources(orc*, int64_t n_src, const double* pos_box, const double* Q);
 int  orc_set_inflow(orc*, int face, int group, const double U[4]);   /* ghost (N, Fx, Fy, Fz) of an INFLOW face */
 int  orc_set_flux(orc*, int flux);          /* interface flux of the transport sweep; default ORC_FLUX_GLF */
+/* standard (non-CRTA) AMR transport, reading A21: transport + chemistry on the leaves of every
+ * level, dt_l = dt/2^l, finest first, fine fluxes deposited into coarser neighbours, linear (MinMod) ghosts at jumps.
+ * EINVAL if a resolution jump across a face exceeds 1.  Refined cells start with their parent's radiation. */
+int  orc_set_amr_transport(orc*, int on);
+int  orc_write_U(orc*, int level, int group, const double* src);   /* [ncell_l][4]; level > 0 needs amr transport on */
+int  orc_restrict_U(orc*);                                         /* split cells := children mean, after orc_write_U */
 int  orc_step(orc*, double dt, int n_steps, orc_diag* diag_last);
 int  orc_read(const orc*, int field, int level, int group, double* dst, int64_t n_dst);
 int64_t orc_level_cells(const orc*, int level);
