@@ -11,6 +11,8 @@
  *      point sources entering Eq. 43 (A12);
  *   4. restriction of N, F, x, e to split cells (children mean, A14);
  *   5. fp64 diagnostics (photon budget A15, min chemical time, sub-cycle counts).
+ * With config.amr_transport = 1 steps 1-4 become the standard AMR scheme (transport and chemistry on the leaves of
+ * every level with dt_l = dt / 2^l; see the field's comment).
  *
  * Conventions
  *   - All pointers are HOST pointers unless the argument name ends in `_dev` or the call has an
@@ -45,7 +47,7 @@ extern "C" {
 #define EMMA_RT_API
 #endif
 
-#define EMMA_RT_ABI_VERSION 1
+#define EMMA_RT_ABI_VERSION 2
 #define EMMA_RT_MAX_GROUPS 4
 #define EMMA_RT_MAX_LEVELS 4          /* refined levels above the base */
 #define EMMA_RT_MAX_SUBSTEPS 65535    /* accepted sub-steps per cell per step before EMMA_RT_ESUBCYCLE (A9) */
@@ -95,6 +97,15 @@ typedef struct {
   double   E_mean[EMMA_RT_MAX_GROUPS];    /* Eq. 38 [erg]                                                     */
   double   e_tol;               /* 0.1                                                         */
   void*    stream;              /* cudaStream_t of the caller (e.g. torch's current stream); 0 = default      */
+  int32_t  amr_transport;       /* 0: CRTA, transport on the coarse level only (the default).
+                                   1: the standard AMR scheme (reading A21): every
+                                   level carries (N, F); advance(l, dt) = advance(l+1, dt/2) twice, then Eq. 30 and
+                                   Eq. 43-48 on the leaves of level l, then split cells := children mean.  Fluxes
+                                   through a coarse-fine face are computed by the fine cells from a MinMod-limited
+                                   linear ghost and deposited into the coarse leaf.  Needs face jumps <= 1 (else
+                                   EMMA_RT_EINVAL at init), <= 3 refined levels, the Eq. 32 flux; U0 is injected into
+                                   the refined cells at init; FIELD_U/N/F can then be read and U written on any level */
+  int32_t  reserved0;
 } emma_rt_config;
 
 typedef struct {                /* static AMR description (host pointers, borrowed during init only)          */
@@ -158,7 +169,8 @@ EMMA_RT_API int64_t emma_rt_kernel_launches(const emma_rt* h);                 /
  * nullable) the summed CUDA-event durations and launch counts of the emma_rt_step kernels recorded since the last
  * call, clears them, and switches recording on (enable != 0) or off for the steps that follow.  Off by default. */
 enum { EMMA_RT_K_TRANSPORT = 0, EMMA_RT_K_CHEM_MAIN = 1, EMMA_RT_K_CHEM_TAIL = 2, EMMA_RT_K_CHEM_REFINED = 3,
-       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_FUSED = 6, EMMA_RT_K_COUNT = 7 };
+       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_FUSED = 6, EMMA_RT_K_AMR_TRANSPORT = 7, EMMA_RT_K_AMR_CHEM = 8,
+       EMMA_RT_K_COUNT = 9 };
 EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out);
 /* Schedule of the coupled step on the unrefined coarse cells (same result up to fp32 rounding order of nothing: both
  * schedules run the same arithmetic).  fused = 1 (default): ONE pass does the transport update (Eq. 30, 32) and the

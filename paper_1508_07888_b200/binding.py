@@ -11,7 +11,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libemma_rt.so")
 
-MAX_GROUPS, MAX_LEVELS, ABI_VERSION = 4, 4, 1
+MAX_GROUPS, MAX_LEVELS, ABI_VERSION = 4, 4, 2
 OK, EINVAL, ENOMEM, ECUDA, ENONFINITE, ESTATE, ECFL, ESUBCYCLE = 0, -1, -2, -3, -4, -5, -6, -7
 FIELD_U, FIELD_N, FIELD_F, FIELD_X, FIELD_T, FIELD_E, FIELD_N0, FIELD_SUBCYCLES, FIELD_XNEUTRAL = range(9)
 _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYCLES: (1, np.uint32)}
@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources"
                     "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_set_inflow", "emma_rt_last_error", "emma_rt_free"]
 FLUX_GLF, FLUX_HLL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
-KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused"]
+KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused", "amr_transport", "amr_chem"]
 
 
 class EmmaRTError(RuntimeError):
@@ -36,7 +36,8 @@ class Config(C.Structure):
                 ("thermal", C.c_int32), ("record_subcycles", C.c_int32), ("max_halvings", C.c_int32),
                 ("device", C.c_int32), ("max_source_cells", C.c_int64), ("box_len_cm", C.c_double),
                 ("c_red_cm_s", C.c_double), ("sigma_N", C.c_double * MAX_GROUPS), ("sigma_E", C.c_double * MAX_GROUPS),
-                ("E_mean", C.c_double * MAX_GROUPS), ("e_tol", C.c_double), ("stream", C.c_void_p)]
+                ("E_mean", C.c_double * MAX_GROUPS), ("e_tol", C.c_double), ("stream", C.c_void_p),
+                ("amr_transport", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class Amr(C.Structure):
@@ -110,7 +111,8 @@ def lib():
 
 
 def make_config(n_coarse, n_groups, box_len_cm, c_red_cm_s, sigma_N, sigma_E, E_mean, bc=(0,) * 6, otsa=1, chemistry=1,
-                thermal=1, record_subcycles=0, max_halvings=60, device=0, max_source_cells=0, e_tol=0.1, stream=0):
+                thermal=1, record_subcycles=0, max_halvings=60, device=0, max_source_cells=0, e_tol=0.1, stream=0,
+                amr_transport=0):
     c = Config()
     c.struct_size, c.abi_version = C.sizeof(Config), ABI_VERSION
     c.n_coarse, c.n_groups = int(n_coarse), int(n_groups)
@@ -122,6 +124,7 @@ def make_config(n_coarse, n_groups, box_len_cm, c_red_cm_s, sigma_N, sigma_E, E_
     for g in range(max(0, min(int(n_groups), MAX_GROUPS, len(sigma_N)))):
         c.sigma_N[g], c.sigma_E[g], c.E_mean[g] = float(sigma_N[g]), float(sigma_E[g]), float(E_mean[g])
     c.stream = stream
+    c.amr_transport, c.reserved0 = int(amr_transport), 0
     return c
 
 
@@ -203,7 +206,7 @@ class EmmaRT:
     """Owns the torch arena and the handle.  `w` is any object with the attributes of workloads.Workload."""
 
     def __init__(self, w, device=0, record_subcycles=0, chemistry=None, thermal=None, otsa=None, bc=None,
-                 max_source_cells=0, stream=None, fused=None, flux=None):
+                 max_source_cells=0, stream=None, fused=None, flux=None, amr_transport=0):
         import torch
         if not torch.cuda.is_available():
             raise EmmaRTError(ECUDA, "no CUDA device: this library has no CPU fallback")
@@ -217,7 +220,8 @@ class EmmaRT:
                                chemistry=w.chemistry if chemistry is None else chemistry,
                                thermal=w.thermal if thermal is None else thermal,
                                record_subcycles=record_subcycles, max_halvings=w.max_halvings, device=device,
-                               max_source_cells=max_source_cells, e_tol=w.e_tol, stream=st)
+                               max_source_cells=max_source_cells, e_tol=w.e_tol, stream=st,
+                               amr_transport=amr_transport)
         nbytes = emma_rt_arena_bytes(self.cfg, w.parent)
         if nbytes == 0:
             raise EmmaRTError(EINVAL, "invalid configuration")

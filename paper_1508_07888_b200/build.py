@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libemma_rt.so")
-SOURCES = ["api.cu", "transport.cu", "transport_tma.cu", "transport_hll.cu", "chemistry.cu", "fused.cu", "util.cu"]
+SOURCES = ["api.cu", "amr.cu", "transport.cu", "transport_tma.cu", "transport_hll.cu", "chemistry.cu", "fused.cu", "util.cu"]
 HEADERS = [os.path.join(CSRC, "emma_rt_internal.cuh"), os.path.join(CSRC, "transport_math.cuh"), os.path.join(CSRC, "chem_math.cuh"),
            os.path.join(CSRC, "async_copy.cuh"), os.path.join(INC, "emma_rt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

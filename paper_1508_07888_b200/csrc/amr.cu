@@ -1,0 +1,445 @@
+// amr.cu -- standard (non-CRTA) AMR transport on refined levels (reading A21;
+// PAPER.md:327-355 Eq. 49-51 / Fig. 2-3, PAPER.md:436 resolution jumps).
+//
+// The host (api.cu) runs the recursion advance(l, dt) = [advance(l+1, dt/2) x 2] -> transport(l) -> chemistry(l) ->
+// restriction(l+1 -> l).  This file holds the kernels of one level:
+//   * amr_transport_kernel: Eq. 30 + 32 for the LEAF cells of a refined level, one thread per cell and all G groups.
+//     Neighbours are found through the oct structure the paper describes (each oct points to the 6 cells of
+//     the level below that surround its parent cell); siblings sit in the same 128-byte oct record.  A face towards a
+//     split cell computes nothing (the fine cells behind it deposit), a face towards a coarser leaf uses the MinMod-limited
+//     linear ghost and deposits the same flux / 8 into that leaf with red.global.add.f32.
+//   * level 0 keeps the dense TMA kernel (transport_tma.cu) for the whole block; amr_fix0_kernel then recomputes the
+//     (few) leaves that touch a split cell without the faces towards it and adds what the fine cells deposited: the
+//     regular block stays on the bandwidth-bound kernel, the irregular part is a sparse second pass.
+//   * amr_chem_kernel: Eq. 43-48 in place on the leaves of a refined level (chem_math.cuh, same arithmetic as CRTA's).
+//   * restriction, initial injection, sources with chemistry off, outflow of level 0.
+#include "chem_math.cuh"
+#include "transport_math.cuh"
+
+namespace emma {
+namespace {
+
+// kind: 0 a leaf of the same level, 1 a split cell of the same level, 2 a leaf of the level below (coarser),
+//       3 box ghost = the cell itself (flip >= 0: that flux component inverted, A13), 4 inflow ghost (A20)
+struct NbRef { int kind, lvl, flip, face; long long cell; };
+
+__device__ __forceinline__ NbRef box_ghost(int bc, int a, int side, int lvl, long long self)
+{
+  NbRef r;
+  r.lvl = lvl; r.cell = self; r.face = 2 * a + side; r.flip = -1;
+  if (bc == EMMA_RT_BC_INFLOW) r.kind = 4;
+  else { r.kind = 3; if (bc == EMMA_RT_BC_REFLECTIVE) r.flip = a; }
+  return r;
+}
+
+// neighbour of a level-0 cell by coordinates
+__device__ NbRef nb_ref0(const AmrDev& A, long long cell, int a, int side)
+{
+  const int n = A.n;
+  const int i = (int)(cell % n), j = (int)((cell / n) % n), k = (int)(cell / ((long long)n * n));
+  int ca = (a == 0) ? i : (a == 1) ? j : k;
+  const long long stride = (a == 0) ? 1 : (a == 1) ? n : (long long)n * n;
+  const int cn = ca + (side ? 1 : -1);
+  long long nb;
+  if (cn < 0 || cn >= n) {
+    const int bc = A.bc[2 * a + side];
+    if (bc != EMMA_RT_BC_PERIODIC) return box_ghost(bc, a, side, 0, cell);
+    nb = cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride;
+  } else nb = cell + (side ? stride : -stride);
+  NbRef r;
+  r.lvl = 0; r.cell = nb; r.flip = -1; r.face = 0;
+  r.kind = (A.child[0] && A.child[0][nb] >= 0) ? 1 : 0;
+  return r;
+}
+
+// neighbour of a cell of level l >= 1 through the oct structure
+__device__ NbRef nb_ref(const AmrDev& A, int l, long long cell, int a, int side)
+{
+  if (l == 0) return nb_ref0(A, cell, a, side);
+  const long long oct = cell >> 3;
+  const int k = (int)(cell & 7);
+  const int bit = (k >> a) & 1;
+  NbRef r;
+  r.flip = -1; r.face = 0;
+  long long nb;
+  if (side != bit) nb = (oct << 3) | (k ^ (1 << a));               // sibling in the same oct
+  else {
+    const int p = A.nbr[l][oct * 6 + 2 * a + side];                 // cell of level l-1 next to the parent cell
+    if (p < 0) return box_ghost(-1 - p, a, side, l, cell);
+    const int ch = A.child[l - 1][p];
+    if (ch < 0) { r.kind = 2; r.lvl = l - 1; r.cell = p; return r; }
+    nb = ((long long)ch << 3) | (k ^ (1 << a));
+  }
+  r.lvl = l; r.cell = nb;
+  r.kind = (l < A.nl && A.child[l][nb] >= 0) ? 1 : 0;
+  return r;
+}
+
+__device__ __forceinline__ float4 nb_load(const AmrDev& A, const NbRef& r, int g, const float4& self)
+{
+  if (r.kind == 4) return A.inflow[r.face][g];
+  if (r.kind == 3) {
+    float4 u = self;
+    if (r.flip == 0) u.y = -u.y; else if (r.flip == 1) u.z = -u.z; else if (r.flip == 2) u.w = -u.w;
+    return u;
+  }
+  return A.U[r.lvl][(size_t)g * A.ncell[r.lvl] + r.cell];
+}
+
+__device__ __forceinline__ float minmod(float a, float b)
+{
+  if (a * b <= 0.f) return 0.f;
+  return (fabsf(a) < fabsf(b)) ? a : b;
+}
+
+// the missing fine neighbour is interpolated linearly from coarse data at the position of the virtual
+// fine cell (child index kv of the coarse leaf c on level lc); slopes MinMod-limited (A21)
+__device__ float4 ghost_state(const AmrDev& A, int lc, long long c, int kv, int g)
+{
+  const float4 Uc = A.U[lc][(size_t)g * A.ncell[lc] + c];
+  float4 out = Uc;
+#pragma unroll
+  for (int b = 0; b < 3; b++) {
+    const NbRef rm = nb_ref(A, lc, c, b, 0), rp = nb_ref(A, lc, c, b, 1);
+    const float4 Um = nb_load(A, rm, g, Uc), Up = nb_load(A, rp, g, Uc);
+    const float sg = ((kv >> b) & 1) ? 0.25f : -0.25f;
+    out.x = fmaf(sg, minmod(Uc.x - Um.x, Up.x - Uc.x), out.x);
+    out.y = fmaf(sg, minmod(Uc.y - Um.y, Up.y - Uc.y), out.y);
+    out.z = fmaf(sg, minmod(Uc.z - Um.z, Up.z - Uc.z), out.z);
+    out.w = fmaf(sg, minmod(Uc.w - Um.w, Up.w - Uc.w), out.w);
+  }
+  return out;
+}
+
+// G_a(U) = (phi_a, a e_a + b phi_a phi): the flux vector of direction a in units of c_red (closure_ab: P = a I + b phi(x)phi)
+__device__ __forceinline__ float4 flux_vec(const float4& U, float ca, float cb, int a)
+{
+  const float pa = (a == 0) ? U.y : (a == 1) ? U.z : U.w;
+  const float t = cb * pa;
+  float4 Gv = make_float4(pa, t * U.y, t * U.z, t * U.w);
+  if (a == 0) Gv.y += ca; else if (a == 1) Gv.z += ca; else Gv.w += ca;
+  return Gv;
+}
+
+// change of the cell (state Ui, closure ai/bi) caused by the Eq. 32 flux through its face (a, side) towards state Un:
+//   + face: -nu F^ = -(nu/2) [(G_i + U_i) + (G_n - U_n)];   - face: +(nu/2) [(G_n + U_n) + (G_i - U_i)]
+__device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui, float ai, float bi, const float4& Un, float nuh)
+{
+  float an, bn;
+  closure_ab(Un, an, bn);
+  const float4 Gi = flux_vec(Ui, ai, bi, a), Gn = flux_vec(Un, an, bn, a);
+  float4 r;
+  if (side) {
+    r.x = -nuh * ((Gi.x + Ui.x) + (Gn.x - Un.x)); r.y = -nuh * ((Gi.y + Ui.y) + (Gn.y - Un.y));
+    r.z = -nuh * ((Gi.z + Ui.z) + (Gn.z - Un.z)); r.w = -nuh * ((Gi.w + Ui.w) + (Gn.w - Un.w));
+  } else {
+    r.x = nuh * ((Gn.x + Un.x) + (Gi.x - Ui.x)); r.y = nuh * ((Gn.y + Un.y) + (Gi.y - Ui.y));
+    r.z = nuh * ((Gn.z + Un.z) + (Gi.z - Ui.z)); r.w = nuh * ((Gn.w + Un.w) + (Gi.w - Ui.w));
+  }
+  return r;
+}
+
+__device__ __forceinline__ void red_add4(float4* p, const float4& v)
+{
+  float* q = reinterpret_cast<float*>(p);
+  atomicAdd(q + 0, v.x); atomicAdd(q + 1, v.y); atomicAdd(q + 2, v.z); atomicAdd(q + 3, v.w);
+}
+
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, double dV, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const long long ncell = A.ncell[l];
+  const float4* __restrict__ Ul = A.U[l];
+  const int* child = (l < A.nl) ? A.child[l] : nullptr;
+  for (long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x; cell < ncell; cell += (long long)gridDim.x * blockDim.x) {
+    if (child && child[cell] >= 0) continue;                        // split: restricted from its children later
+    float4 Ui[G], ac[G];
+    float ai[G], bi[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      Ui[g] = Ul[(size_t)g * ncell + cell];
+      closure_ab(Ui[g], ai[g], bi[g]);
+      ac[g] = Ui[g];
+    }
+    const int k = (int)(cell & 7);
+    for (int a = 0; a < 3; a++)
+      for (int side = 0; side < 2; side++) {
+        const NbRef r = nb_ref(A, l, cell, a, side);
+        if (r.kind == 1) continue;                                  // Fig. 3 (iii): fed by the fine steps
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 Un = (r.kind == 2) ? ghost_state(A, r.lvl, r.cell, k ^ (1 << a), g) : nb_load(A, r, g, Ui[g]);
+          const float4 d = face_change(a, side, Ui[g], ai[g], bi[g], Un, nuh);
+          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+          if (r.kind == 2)                                          // Fig. 3 (i)-(ii): the same flux, seen from the coarse leaf
+            red_add4(A.dep[r.lvl] + (size_t)g * A.ncell[r.lvl] + r.cell, make_float4(-0.125f * d.x, -0.125f * d.y, -0.125f * d.z, -0.125f * d.w));
+          if (r.kind >= 3) acc.outflow -= (double)d.x * dV;         // A15: net N-flux through a box face
+        }
+      }
+    if (l < A.nl) {
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        float4* dp = A.dep[l] + (size_t)g * ncell + cell;
+        const float4 d = *dp;
+        if (d.x != 0.f || d.y != 0.f || d.z != 0.f || d.w != 0.f) {
+          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+          *dp = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < G; g++) Unew[(size_t)g * ncell + cell] = ac[g];
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// Eq. 43-48 on the leaves of a refined level, in place, over cp.dt (= dt / 2^level)
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_chem_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, const int* __restrict__ child,
+                int count_total, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const long long ncell = L.ncell;
+  for (long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x; cell < ncell; cell += (long long)gridDim.x * blockDim.x) {
+    if (child && child[cell] >= 0) { if (cp.record) L.subc[cell] = 0; continue; }
+    CellState<G> c;
+    load_cell<G>(L, cell, U, ncell, cell, c);
+    CellTally tl;
+    float rem = cp.dt, dmin = FINF;
+    bool ok = true;
+    while (ok && rem > 0.f) ok = substep<G>(cp, c, rem, tl, dmin);
+    if (!ok) acc.err |= 1u;
+    store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
+    const double before = acc.total;
+    fold(acc, tl, c.N, G, L.dV);
+    if (!count_total) acc.total = before;                            // photons are counted once per coarse step
+    acc.dtau_min = fminf(acc.dtau_min, dmin);
+    if (!finite_cell<G>(c)) acc.nonfinite++;
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// chemistry off (A9): N += S dt in the source cells of the level; count_total: also sum N dV over the leaves
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_sources_kernel(const LevelDev L, float4* __restrict__ U, const int* __restrict__ child, float dt, int count_total,
+                   Partial* __restrict__ parts)
+{
+  Acc acc;
+  const long long ncell = L.ncell;
+  for (long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x; cell < ncell; cell += (long long)gridDim.x * blockDim.x) {
+    if (child && child[cell] >= 0) continue;
+    float S[G];
+    load_sources<G>(L, cell, S);
+    float s = 0.f;
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      float4* p = U + (size_t)g * ncell + cell;
+      if (S[g] != 0.f) {
+        const float add = S[g] * dt;
+        p->x += add;
+        acc.injected += (double)add * L.dV;
+      }
+      s += p->x;
+    }
+    if (count_total) acc.total += (double)s * L.dV;
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+__device__ __forceinline__ float oct_sum8(float v)
+{
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  return v;
+}
+
+// split cell := mean of its 8 children (N, phi; with_gas: x and e too), 8 lanes per oct
+template <int G>
+__global__ void __launch_bounds__(256)
+amr_restrict_kernel(const LevelDev L, const LevelDev Lbelow, const float4* __restrict__ Uf, float4* __restrict__ Uc,
+                    int with_gas)
+{
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = cell < L.ncell;                                  // uniform per 8-lane group
+  float4 m[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float4 u = valid ? Uf[(size_t)g * L.ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
+    m[g].x = 0.125f * oct_sum8(u.x); m[g].y = 0.125f * oct_sum8(u.y);
+    m[g].z = 0.125f * oct_sum8(u.z); m[g].w = 0.125f * oct_sum8(u.w);
+  }
+  float x = 0.f, y = 0.f, e = 0.f;
+  if (valid && with_gas) { decode_x(L.xs[cell], x, y); e = L.eps[cell] * L.n0[cell]; }
+  const float xm = 0.125f * oct_sum8(x), ym = 0.125f * oct_sum8(y), em = 0.125f * oct_sum8(e);
+  if (valid && (cell & 7) == 0) {
+    const long long pc = L.parent[cell >> 3];
+#pragma unroll
+    for (int g = 0; g < G; g++) Uc[(size_t)g * Lbelow.ncell + pc] = m[g];
+    if (with_gas) { Lbelow.xs[pc] = encode_x(xm, ym); Lbelow.eps[pc] = em / Lbelow.n0[pc]; }
+  }
+}
+
+// refined cells start with the radiation of their parent
+template <int G>
+__global__ void amr_inject_init_kernel(const LevelDev L, const float4* __restrict__ Uc, long long ncell_c, float4* __restrict__ Uf)
+{
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell >= L.ncell) return;
+  const long long pc = L.parent[cell >> 3];
+#pragma unroll
+  for (int g = 0; g < G; g++) Uf[(size_t)g * L.ncell + cell] = Uc[(size_t)g * ncell_c + pc];
+}
+
+// level 0 after the dense pass: the leaves with a split face neighbour are recomputed from the old states, face by
+// face, without the faces that look at a split cell (Fig. 3 (iii)), plus what the fine cells behind those faces
+// deposited during their two sub-steps.  Recomputed, not corrected: taking a large coarse flux back out of the dense
+// result would leave its rounding error on a possibly much smaller remainder.
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restrict__ Unew, const int* __restrict__ fix_cell,
+                const unsigned char* __restrict__ fix_mask, int n_fix, float nuh)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_fix) return;
+  const long long cell = fix_cell[i];
+  const unsigned mask = fix_mask[i];
+  const long long nc = A.ncell[0];
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float4 Ui = Uold[(size_t)g * nc + cell];
+    float ai, bi;
+    closure_ab(Ui, ai, bi);
+    float4 ac = Ui;
+    for (int f = 0; f < 6; f++) {
+      if ((mask >> f) & 1u) continue;
+      const NbRef r = nb_ref0(A, cell, f >> 1, f & 1);
+      const float4 Un = (r.kind >= 3) ? nb_load(A, r, g, Ui) : Uold[(size_t)g * nc + r.cell];
+      const float4 d = face_change(f >> 1, f & 1, Ui, ai, bi, Un, nuh);
+      ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+    }
+    float4* dp = A.dep[0] + (size_t)g * nc + cell;
+    const float4 d = *dp;
+    ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+    *dp = make_float4(0.f, 0.f, 0.f, 0.f);
+    Unew[(size_t)g * nc + cell] = ac;
+  }
+}
+
+// net N-flux through the non-periodic box faces of the level-0 LEAVES (the dense pass also counts split cells, whose
+// faces belong to their children here), from the old states
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_outflow0_kernel(const AmrDev A, const float4* __restrict__ Uold, float nuh, double dV, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const int n = A.n;
+  const long long per = (long long)n * n, nc = A.ncell[0];
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < 6 * per; t += (long long)gridDim.x * blockDim.x) {
+    const int f = (int)(t / per), a = f >> 1, side = f & 1;
+    if (A.bc[f] == EMMA_RT_BC_PERIODIC) continue;
+    const int u = (int)(t % n), v = (int)((t / n) % n), w = side ? n - 1 : 0;
+    const long long cell = (a == 0) ? w + (long long)n * (u + (long long)n * v)
+                         : (a == 1) ? u + (long long)n * (w + (long long)n * v) : u + (long long)n * (v + (long long)n * w);
+    if (A.child[0] && A.child[0][cell] >= 0) continue;
+    const NbRef r = nb_ref0(A, cell, a, side);
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      const float4 Ui = Uold[(size_t)g * nc + cell];
+      float ai, bi;
+      closure_ab(Ui, ai, bi);
+      const float4 d = face_change(a, side, Ui, ai, bi, nb_load(A, r, g, Ui), nuh);
+      acc.outflow -= (double)d.x * dV;
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+int grid_for(long long work, int block, int cap)
+{
+  long long b = (work + block - 1) / block;
+  if (b < 1) b = 1;
+  if (b > cap) b = cap;
+  return (int)b;
+}
+constexpr int AMR_GRID_CAP = 148 * 8;            // whole waves of 8 CTAs of 128 threads per SM; each block writes one Partial
+
+}  // namespace
+
+#define AMR_DISPATCH(G, CALL)                                   \
+  switch (G) {                                                  \
+    case 1: { constexpr int GG = 1; CALL; } break;              \
+    case 2: { constexpr int GG = 2; CALL; } break;              \
+    case 3: { constexpr int GG = 3; CALL; } break;              \
+    default: { constexpr int GG = 4; CALL; } break;             \
+  }
+
+int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
+                         cudaStream_t st)
+{
+  const int nb = grid_for(A.ncell[level], 128, AMR_GRID_CAP);
+  AMR_DISPATCH(A.G, (amr_transport_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts)));
+  *n_parts = nb;
+  return 1;
+}
+
+int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, Partial* parts,
+                    int* n_parts, cudaStream_t st)
+{
+  const int nb = grid_for(L.ncell, 128, AMR_GRID_CAP);
+  const int* child = level < A.nl ? A.child[level] : nullptr;
+  AMR_DISPATCH(A.G, (amr_chem_kernel<GG><<<nb, 128, 0, st>>>(cp, L, A.U[level], child, count_total, parts)));
+  *n_parts = nb;
+  return 1;
+}
+
+int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, Partial* parts,
+                       int* n_parts, cudaStream_t st)
+{
+  const int nb = grid_for(L.ncell, 128, AMR_GRID_CAP);
+  const int* child = level < A.nl ? A.child[level] : nullptr;
+  AMR_DISPATCH(A.G, (amr_sources_kernel<GG><<<nb, 128, 0, st>>>(L, A.U[level], child, dt, count_total, parts)));
+  *n_parts = nb;
+  return 1;
+}
+
+int launch_amr_restrict(const LevelDev& Lfine, const LevelDev& Lcoarse, const AmrDev& A, int level_fine, int with_gas,
+                        cudaStream_t st)
+{
+  if (Lfine.ncell == 0) return 0;
+  const int nb = (int)((Lfine.ncell + 255) / 256);
+  AMR_DISPATCH(A.G, (amr_restrict_kernel<GG><<<nb, 256, 0, st>>>(Lfine, Lcoarse, A.U[level_fine], A.U[level_fine - 1], with_gas)));
+  return 1;
+}
+
+int launch_amr_inject_init(const LevelDev& Lfine, const AmrDev& A, int level_fine, cudaStream_t st)
+{
+  if (Lfine.ncell == 0) return 0;
+  const int nb = (int)((Lfine.ncell + 255) / 256);
+  AMR_DISPATCH(A.G, (amr_inject_init_kernel<GG><<<nb, 256, 0, st>>>(Lfine, A.U[level_fine - 1], A.ncell[level_fine - 1], A.U[level_fine])));
+  return 1;
+}
+
+int launch_amr_fix0(const AmrDev& A, const float4* Uold, float4* Unew, const int* fix_cell, const unsigned char* fix_mask,
+                    int n_fix, float nuh, cudaStream_t st)
+{
+  if (n_fix == 0) return 0;
+  const int nb = (n_fix + 127) / 128;
+  AMR_DISPATCH(A.G, (amr_fix0_kernel<GG><<<nb, 128, 0, st>>>(A, Uold, Unew, fix_cell, fix_mask, n_fix, nuh)));
+  return 1;
+}
+
+int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, Partial* parts, int* n_parts,
+                        cudaStream_t st)
+{
+  const int nb = grid_for(6LL * A.n * A.n, 128, 148 * 2);
+  AMR_DISPATCH(A.G, (amr_outflow0_kernel<GG><<<nb, 128, 0, st>>>(A, Uold, nuh, dV, parts)));
+  *n_parts = nb;
+  return 1;
+}
+
+}  // namespace emma

@@ -31,6 +31,9 @@ struct Layout {
   size_t parent[MAXL + 1], anc0[MAXL + 1], child[MAXL + 1], Ut[MAXL + 1];
   size_t srcmask[MAXL + 1], src_cell[MAXL + 1], src_S[MAXL + 1];
   size_t queue, qcount, parts, diag;
+  // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
+  // child index and the list of level-0 leaves that touch a split cell
+  size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], achild0, afix_cell, afix_mask;
   size_t total;
 };
 
@@ -38,7 +41,7 @@ struct Shape {
   int n, G, nl;
   long long ncell[MAXL + 1], nocts[MAXL + 1];
   long long max_src;
-  bool record, need_queue;
+  bool record, need_queue, amr;
 };
 
 bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
@@ -65,6 +68,9 @@ bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
   s.max_src = c->max_source_cells > 0 ? c->max_source_cells : 65536;
   s.record = c->record_subcycles != 0;
   s.need_queue = c->chemistry != 0 && c->thermal != 0;
+  if (c->amr_transport != 0 && c->amr_transport != 1) return false;
+  s.amr = c->amr_transport == 1 && s.nl > 0;
+  if (s.amr && s.nl > 3) return false;          // partial-sum slots: 2^(nl+1) - 1 level sweeps per step
   return true;
 }
 
@@ -93,6 +99,18 @@ void make_layout(const Shape& s, Layout& L)
   L.qcount = take(256);
   L.parts = take((size_t)PART_SLOTS * sizeof(Partial));
   L.diag = take(sizeof(DiagDev));
+  if (s.amr) {
+    for (int l = 0; l <= s.nl; l++) {
+      if (l >= 1) {
+        for (int b = 0; b < 2; b++) L.aU[b][l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
+        L.anbr[l] = take((size_t)s.nocts[l] * 6 * 4);
+      }
+      if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
+    }
+    L.achild0 = take((size_t)s.ncell[0] * 4);
+    L.afix_cell = take((size_t)s.nocts[1] * 6 * 4);
+    L.afix_mask = take((size_t)s.nocts[1] * 6);
+  }
   L.total = off;
 }
 
@@ -118,9 +136,18 @@ struct emma_rt {
   int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
   int flux;                                    // interface flux of the transport update (emma_rt_set_flux)
   float4 inflow[6][MAXG];                      // ghost state (N, phi) of inflow faces (emma_rt_set_inflow)
+  // standard AMR transport (A21)
+  int acur[MAXL + 1];                          // aU[acur[l]][l] holds the current radiation of refined level l
+  int n_fix;                                   // level-0 leaves with a split face neighbour
+  bool amr_dirty;                              // U was written: restrict bottom-up before the next step
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
+  float4* Ulev(int l, int other = 0) const       // current (other = 0) or scratch radiation buffer of a level
+  {
+    if (l == 0) return U(other ? 1 - cur : cur);
+    return (float4*)(arena + lay.aU[other ? 1 - acur[l] : acur[l]][l]);
+  }
   Partial* parts() const { return (Partial*)(arena + lay.parts); }
   unsigned int* qcount() const { return (unsigned int*)(arena + lay.qcount); }
   DiagDev* diag() const { return (DiagDev*)(arena + lay.diag); }
@@ -145,6 +172,25 @@ int fail(emma_rt* h, int code, const char* fmt, ...)
     if (e__ != cudaSuccess) return fail(h, EMMA_RT_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
   } while (0)
 
+// device view of the hierarchy in AMR-transport mode, with the buffers that are current right now
+AmrDev amr_view(const emma_rt* h)
+{
+  AmrDev A;
+  memset(&A, 0, sizeof A);
+  const Shape& s = h->sh;
+  A.nl = s.nl; A.n = s.n; A.G = s.G;
+  for (int f = 0; f < 6; f++) A.bc[f] = h->cfg.bc[f];
+  memcpy(A.inflow, h->inflow, sizeof A.inflow);
+  for (int l = 0; l <= s.nl; l++) {
+    A.ncell[l] = s.ncell[l];
+    A.U[l] = h->Ulev(l);
+    A.dep[l] = l < s.nl ? (float4*)(h->arena + h->lay.adep[l]) : nullptr;
+    A.child[l] = l == 0 ? (const int*)(h->arena + h->lay.achild0) : l < s.nl ? h->lv[l].child : nullptr;
+    A.nbr[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbr[l]) : nullptr;
+  }
+  return A;
+}
+
 size_t field_elem_bytes(int field)
 {
   switch (field) {
@@ -159,7 +205,8 @@ int upload_field(emma_rt* h, int field, int level, int group, const void* src, b
 {
   const long long nc = h->sh.ncell[level];
   const size_t eb = field_elem_bytes(field);
-  float4* Ug = (field == EMMA_RT_FIELD_U) ? h->U(h->cur) + (size_t)group * nc : nullptr;
+  float4* Ug = (field == EMMA_RT_FIELD_U) ? h->Ulev(level) + (size_t)group * nc : nullptr;
+  if (field == EMMA_RT_FIELD_U && h->sh.amr) h->amr_dirty = true;
   if (src_is_device) {
     h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, 0, nc, src, h->st);
     CUDA_TRY(h, cudaGetLastError());
@@ -271,6 +318,73 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     for (auto& kv : h->child_of[0]) refined_h[kv.first >> 5] |= 1u << (kv.first & 31);
     CUDA_TRY(h, cudaMemcpyAsync(h->lv[0].refined, refined_h.data(), refined_h.size() * 4, cudaMemcpyHostToDevice, h->st));
   }
+  // ---- standard AMR transport (A21): the paper's oct neighbour pointers, level-0 child index, fix list
+  std::vector<std::vector<int>> nbr_h(s.nl + 1);
+  std::vector<int> child0_h, fix_cell_h;
+  std::vector<unsigned char> fix_mask_h;
+  h->n_fix = 0; h->amr_dirty = false;
+  for (int l = 0; l <= MAXL; l++) h->acur[l] = 0;
+  if (s.amr) {
+    const int n = s.n;
+    auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
+    // neighbour of a level-0 cell, or the box-face code
+    auto nb0 = [&](long long cell, int a, int side) -> long long {
+      const long long stride = a == 0 ? 1 : a == 1 ? n : (long long)n * n;
+      const int ca = a == 0 ? (int)(cell % n) : a == 1 ? (int)((cell / n) % n) : (int)(cell / ((long long)n * n));
+      const int cn = ca + (side ? 1 : -1);
+      if (cn < 0 || cn >= n) {
+        if (h->cfg.bc[2 * a + side] != EMMA_RT_BC_PERIODIC) return bc_code(a, side);
+        return cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride;
+      }
+      return cell + (side ? stride : -stride);
+    };
+    for (int l = 1; l <= s.nl; l++) {
+      nbr_h[l].resize((size_t)s.nocts[l] * 6);
+      for (long long o = 0; o < s.nocts[l]; o++) {
+        const long long p = parent_h[l][o];                      // the oct's parent cell, on level l-1
+        for (int a = 0; a < 3; a++)
+          for (int side = 0; side < 2; side++) {
+            long long q;
+            if (l == 1) q = nb0(p, a, side);
+            else {
+              const long long po = p >> 3;                       // the parent cell's own oct (level l-1)
+              const int k = (int)(p & 7), bit = (k >> a) & 1;
+              if (side != bit) q = (po << 3) | (k ^ (1 << a));
+              else {
+                const int pp = nbr_h[l - 1][po * 6 + 2 * a + side];     // cell of level l-2
+                if (pp < 0) q = pp;
+                else {
+                  auto it = h->child_of[l - 2].find(pp);
+                  if (it == h->child_of[l - 2].end())
+                    return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 across a face of oct %lld of level %d (PAPER.md:75)", o, l);
+                  q = ((long long)it->second << 3) | (k ^ (1 << a));
+                }
+              }
+            }
+            nbr_h[l][o * 6 + 2 * a + side] = (int)q;
+          }
+      }
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbr[l], nbr_h[l].data(), nbr_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+    }
+    child0_h.assign((size_t)s.ncell[0], -1);
+    for (auto& kv : h->child_of[0]) child0_h[kv.first] = kv.second;
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.achild0, child0_h.data(), child0_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+    // level-0 leaves next to a split cell, with the mask of the faces that look at one (sorted by cell id)
+    std::map<long long, unsigned> fix;
+    for (auto& kv : h->child_of[0])
+      for (int a = 0; a < 3; a++)
+        for (int side = 0; side < 2; side++) {
+          const long long q = nb0(kv.first, a, side);
+          if (q < 0 || child0_h[q] >= 0) continue;
+          fix[q] |= 1u << (2 * a + (1 - side));                   // q sees the split cell through its opposite face
+        }
+    for (auto& kv : fix) { fix_cell_h.push_back((int)kv.first); fix_mask_h.push_back((unsigned char)kv.second); }
+    h->n_fix = (int)fix_cell_h.size();
+    if (h->n_fix) {
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_cell, fix_cell_h.data(), fix_cell_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_mask, fix_mask_h.data(), fix_mask_h.size(), cudaMemcpyHostToDevice, h->st));
+    }
+  }
   CUDA_TRY(h, cudaStreamSynchronize(h->st));   // host staging vectors go out of scope below
 
   // ---- fields: N0, X, T (-> eps, A10) per level; U0 per group; then the children means of split cells (A14)
@@ -284,6 +398,10 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     for (int g = 0; g < s.G; g++)
       if (fields->U0[g] && (rc = upload_field(h, EMMA_RT_FIELD_U, 0, g, fields->U0[g], false)) != EMMA_RT_OK) return rc;
   for (int l = s.nl; l >= 1; l--) h->launches += launch_restrict_init(h->lv, l, h->st);
+  if (s.amr) {                                 // refined cells start with their parent's radiation
+    const AmrDev A = amr_view(h);
+    for (int l = 1; l <= s.nl; l++) h->launches += launch_amr_inject_init(h->lv[l], A, l, h->st);
+  }
   CUDA_TRY(h, cudaGetLastError());
   CUDA_TRY(h, cudaStreamSynchronize(h->st));
   return EMMA_RT_OK;
@@ -308,7 +426,7 @@ int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos, const doub
     double ox = fx - ix, oy = fy - iy, oz = fz - iz;
     int lvl = 0;
     long long cell = ix + (long long)s.n * (iy + (long long)s.n * iz);
-    if (h->cfg.chemistry) {                      // chemistry off: sources are folded to the coarse cell (A9)
+    if (h->cfg.chemistry || s.amr) {             // CRTA with chemistry off: sources are folded to the coarse cell (A9)
       while (lvl < s.nl) {
         auto it = h->child_of[lvl].find(cell);
         if (it == h->child_of[lvl].end()) break;
@@ -415,7 +533,88 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   fp.tiles_y = (s.n + fused_tile_y() - 1) / fused_tile_y();
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
 
-  for (int step = 0; step < n_steps; step++) {
+  if (s.amr) {
+    // standard AMR scheme (A21): advance(l, dt) = advance(l+1, dt/2) x 2 -> transport(l) -> chemistry(l) -> restrict(l+1 -> l)
+    if (hll) return fail(h, EMMA_RT_ESTATE, "amr_transport runs the Eq. 32 flux only");
+    const float nuh = (float)(0.5 * (c * dt / h->dx));           // the same CFL number on every level
+    tp.want_total = 0;
+    bool open_faces = false;
+    for (int f = 0; f < 6; f++) open_faces = open_faces || h->cfg.bc[f] != EMMA_RT_BC_PERIODIC;
+    if (h->amr_dirty) {                                          // U was written: split cells := children mean
+      for (int l = s.nl; l >= 1; l--) h->launches += launch_amr_restrict(h->lv[l], h->lv[l - 1], amr_view(h), l, 0, h->st);
+      h->amr_dirty = false;
+    }
+    for (int step = 0; step < n_steps; step++) {
+      int off = 0;
+      Partial* P = h->parts();
+      // (level, dt, last sub-step of the level in this coarse step) in execution order, finest first
+      struct Call { int l; double dt; bool last; };
+      std::vector<Call> order;
+      struct Rec { static void go(std::vector<Call>& o, int l, int nl, const long long* nc, double dtl, bool last) {
+        if (l < nl && nc[l + 1] > 0) { go(o, l + 1, nl, nc, 0.5 * dtl, false); go(o, l + 1, nl, nc, 0.5 * dtl, last); }
+        o.push_back({l, dtl, last});
+      } };
+      Rec::go(order, 0, s.nl, s.ncell, dt, true);
+      for (const Call& cl : order) {
+        const int l = cl.l;
+        int np = 0;
+        if (off + 3 * MAX_PART_BLOCKS > PART_SLOTS) return fail(h, EMMA_RT_EINVAL, "too many level sweeps for the partial-sum slots");
+        if (l == 0) {
+          // dense pass over the whole block (its partials are not used: split cells must not count), then the
+          // sparse correction of the leaves that touch a split cell
+          h->prof.begin(EMMA_RT_K_TRANSPORT);
+          if (use_tma) {
+            const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+            if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            h->launches += k;
+          } else h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
+          h->prof.end();
+          AmrDev A = amr_view(h);
+          h->prof.begin(EMMA_RT_K_OTHER);
+          if (open_faces) { h->launches += launch_amr_outflow0(A, h->U(h->cur), nuh, h->lv[0].dV, P + off, &np, h->st); off += np; }
+          h->launches += launch_amr_fix0(A, h->U(h->cur), h->U(1 - h->cur), (const int*)(h->arena + h->lay.afix_cell),
+                                         (const unsigned char*)(h->arena + h->lay.afix_mask), h->n_fix, nuh, h->st);
+          h->prof.end();
+          h->cur = 1 - h->cur;
+          if (h->cfg.chemistry) {
+            h->launches += launch_chem_level0(cp, h->lv[0], h->U(h->cur), s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
+                                              P + off, &np, h->sm_count, h->st, &h->prof);
+            off += np;
+          } else {
+            h->prof.begin(EMMA_RT_K_OTHER);
+            h->launches += launch_amr_sources(h->lv[0], amr_view(h), 0, (float)dt, 1, P + off, &np, h->st);
+            h->prof.end();
+            off += np;
+          }
+        } else {
+          AmrDev A = amr_view(h);
+          h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
+          h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, P + off, &np, h->st);
+          h->prof.end();
+          off += np;
+          h->acur[l] = 1 - h->acur[l];
+          A = amr_view(h);
+          ChemParams cl_cp = cp;
+          cl_cp.dt = (float)cl.dt;
+          h->prof.begin(EMMA_RT_K_AMR_CHEM);
+          if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, P + off, &np, h->st);
+          else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, P + off, &np, h->st);
+          h->prof.end();
+          off += np;
+        }
+        if (l < s.nl && s.ncell[l + 1] > 0) {
+          h->prof.begin(EMMA_RT_K_OTHER);
+          h->launches += launch_amr_restrict(h->lv[l + 1], h->lv[l], amr_view(h), l + 1, h->cfg.chemistry ? 1 : 0, h->st);
+          h->prof.end();
+        }
+      }
+      h->t_sim += dt;
+      h->prof.begin(EMMA_RT_K_FINALIZE);
+      h->launches += launch_finalize(P, off, h->diag(), h->qcount(), h->t_sim, h->st);
+      h->prof.end();
+    }
+  }
+  for (int step = 0; step < (s.amr ? 0 : n_steps); step++) {
     int off = 0, np = 0;
     Partial* P = h->parts();
     if (fused) {
@@ -516,12 +715,12 @@ int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* 
   if (level < 0 || level > s.nl) return fail(h, EMMA_RT_EINVAL, "level out of range");
   if (field < EMMA_RT_FIELD_U || field > EMMA_RT_FIELD_XNEUTRAL) return fail(h, EMMA_RT_EINVAL, "unknown field");
   const bool rad = field == EMMA_RT_FIELD_U || field == EMMA_RT_FIELD_N || field == EMMA_RT_FIELD_F;
-  if (rad && (level != 0 || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "radiation fields live on level 0, group in range");
+  if (rad && ((level != 0 && !s.amr) || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "radiation fields live on level 0 (every level with amr_transport), group in range");
   if (field == EMMA_RT_FIELD_SUBCYCLES && !s.record) return fail(h, EMMA_RT_ESTATE, "record_subcycles was not set");
   const long long nc = s.ncell[level];
   const size_t eb = field_elem_bytes(field);
   if (bytes != (size_t)nc * eb) return fail(h, EMMA_RT_EINVAL, "size mismatch: %zu != %zu", bytes, (size_t)nc * eb);
-  const float4* Ug = rad ? h->U(h->cur) + (size_t)group * nc : nullptr;
+  const float4* Ug = rad ? h->Ulev(level) + (size_t)group * nc : nullptr;
   const float cr = (float)h->cfg.c_red_cm_s;
   if (dst_is_device) {
     h->launches += launch_export(field, h->lv[level], Ug, cr, 0, nc, dst, h->st);
@@ -548,7 +747,7 @@ int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const
   if (level < 0 || level > s.nl) return fail(h, EMMA_RT_EINVAL, "level out of range");
   if (field != EMMA_RT_FIELD_U && field != EMMA_RT_FIELD_X && field != EMMA_RT_FIELD_T && field != EMMA_RT_FIELD_N0)
     return fail(h, EMMA_RT_EINVAL, "field is not writable");
-  if (field == EMMA_RT_FIELD_U && (level != 0 || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "U lives on level 0, group in range");
+  if (field == EMMA_RT_FIELD_U && ((level != 0 && !s.amr) || group < 0 || group >= s.G)) return fail(h, EMMA_RT_EINVAL, "U lives on level 0 (every level with amr_transport), group in range");
   const size_t eb = field_elem_bytes(field);
   if (bytes != (size_t)s.ncell[level] * eb) return fail(h, EMMA_RT_EINVAL, "size mismatch");
   return upload_field(h, field, level, group, src, src_is_device != 0);
@@ -606,6 +805,7 @@ int emma_rt_set_flux(emma_rt* h, int32_t flux)
 {
   if (!h) return EMMA_RT_EINVAL;
   if (flux != EMMA_RT_FLUX_GLF && flux != EMMA_RT_FLUX_HLL) return fail(h, EMMA_RT_EINVAL, "unknown flux %d", (int)flux);
+  if (flux == EMMA_RT_FLUX_HLL && h->sh.amr) return fail(h, EMMA_RT_ESTATE, "amr_transport runs the Eq. 32 flux only");
   h->flux = flux;
   return EMMA_RT_OK;
 }

@@ -204,3 +204,36 @@ __device__ inline void block_reduce_store(const Acc& a, Partial* out)
 }
 
 }  // namespace emma
+
+// ---- standard (non-CRTA) AMR transport, reading A21 (amr.cu) -------------------------------------------
+namespace emma {
+
+// device view of the level hierarchy in AMR-transport mode.  Every level carries its own radiation; `nbr` is the
+// paper's oct structure ("6 pointers toward the 6 Cartesian neighbors cells of c^{l-1}").
+struct AmrDev {
+  int nl, n, G;
+  int bc[6];
+  long long ncell[MAXL + 1];
+  float4* U[MAXL + 1];          // current radiation of the level, [G][ncell]
+  float4* dep[MAXL + 1];        // change deposited into leaves by the fluxes of the level above, [G][ncell] (levels < nl)
+  const int* child[MAXL + 1];   // [ncell] oct on the level above or -1 (levels < nl)
+  const int* nbr[MAXL + 1];     // [nocts][6] cell of the level below next to the oct's parent cell in -x,+x,-y,+y,-z,+z,
+                                // or -1 - bc for a non-periodic box face (levels >= 1)
+  float4 inflow[6][MAXG];
+};
+
+int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
+                         cudaStream_t st);
+int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, Partial* parts,
+                    int* n_parts, cudaStream_t st);
+int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, Partial* parts,
+                       int* n_parts, cudaStream_t st);
+int launch_amr_restrict(const LevelDev& Lfine, const LevelDev& Lcoarse, const AmrDev& A, int level_fine, int with_gas,
+                        cudaStream_t st);
+int launch_amr_inject_init(const LevelDev& Lfine, const AmrDev& A, int level_fine, cudaStream_t st);
+int launch_amr_fix0(const AmrDev& A, const float4* Uold, float4* Unew, const int* fix_cell, const unsigned char* fix_mask,
+                    int n_fix, float nuh, cudaStream_t st);
+int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, Partial* parts, int* n_parts,
+                        cudaStream_t st);
+
+}  // namespace emma

@@ -1,0 +1,160 @@
+"""T2: the standard (non-CRTA) AMR transport (config.amr_transport = 1; reading A21) against
+the fp64 oracle, element by element on every level.
+
+The oracle's scheme is pinned on the CPU (tests/test_oracle_amr.py M1-M7).  Here: transport alone from random states on
+jump-balanced 1- and 2-level meshes (periodic and open/reflective boxes, G = 1..3), the coupled step with sources and
+chemistry over several coarse steps, the photon budget, the refusals (face jump > 1, HLL), field I/O on refined levels.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+import paper_1508_07888_b200 as E
+from workloads.amr import make_amr_standard
+
+from .helpers import tiny_workload
+from .parity import budget_residual, clean_masks, coarse_ancestors
+
+pytestmark = pytest.mark.gpu
+
+TOL_NF, TOL_XT, TOL_BUDGET = 1e-5, 1e-4, 1e-6
+
+
+def _random_levels(rng, w, fmax=0.8, lo=-6, hi=-3):
+    out = []
+    for l in range(w.n_levels + 1):
+        m = len(w.n0[l])
+        per = []
+        for _ in range(w.G):
+            U = np.empty((m, 4))
+            U[:, 0] = 10.0 ** rng.uniform(lo, hi, m)
+            v = rng.standard_normal((m, 3))
+            v /= np.linalg.norm(v, axis=1)[:, None]
+            U[:, 1:] = v * (rng.uniform(0, fmax, m) * w.c_red * U[:, 0])[:, None]
+            per.append(U.astype(np.float32))
+        out.append(per)
+    return out
+
+
+def _pair(w, U=None, **kw):
+    orc = O.Oracle(w, **kw)
+    assert orc.set_amr_transport(True) == O.OK
+    gpu = E.EmmaRT(w, record_subcycles=1, amr_transport=1, **kw)
+    if U is not None:
+        for l in range(w.n_levels + 1):
+            for g in range(w.G):
+                assert orc.write_U(l, g, U[l][g].astype(np.float64)) == O.OK
+                assert gpu.write(E.FIELD_U, l, g, U[l][g]) == E.OK
+        assert orc.restrict_U() == O.OK            # the library restricts on its own before the next step
+    return orc, gpu
+
+
+def _errors(orc, gpu, w, masks=None):
+    """A17 norms per level, floor relative to the level's largest N."""
+    eN = eF = 0.0
+    for l in range(w.n_levels + 1):
+        for g in range(w.G):
+            Uo = orc.read(O.F_U, l, g)
+            Ug = gpu.read(E.FIELD_U, l, g).astype(np.float64)
+            sc = np.maximum(np.abs(Uo[:, 0]), max(1e-12 * np.abs(Uo[:, 0]).max(), 1e-300))
+            rN = np.abs(Ug[:, 0] - Uo[:, 0]) / sc
+            rF = np.abs(Ug[:, 1:] - Uo[:, 1:]).max(axis=1) / (w.c_red * sc)
+            if masks is not None:
+                rN, rF = rN[masks[l]], rF[masks[l]]
+            if rN.size:
+                eN, eF = max(eN, rN.max()), max(eF, rF.max())
+    return eN, eF
+
+
+@pytest.mark.parametrize("n,G,levels,bc", [(16, 1, 2, (0,) * 6), (16, 3, 2, (0,) * 6), (12, 2, 1, (0,) * 6),
+                                           (16, 2, 2, (1, 1, 2, 1, 0, 0)), (10, 1, 2, (2, 2, 1, 1, 1, 2))])
+def test_amr_transport_one_coarse_step(n, G, levels, bc):
+    rng = np.random.default_rng(100 * n + 10 * G + levels)
+    w = make_amr_standard(n=n, G=3 if G == 3 else 1, levels=levels, seed=77 + n, thresh1=3.0, thresh2=4.0)
+    if G == 2:
+        t = tiny_workload(n, G=2, parent=w.parent, chemistry=0, bc=bc, L=w.L)
+        w = t
+    w.bc, w.chemistry, w.src_pos = tuple(bc), 0, None
+    assert 0 < len(w.parent[0]) < n ** 3 and (levels == 1 or len(w.parent[1]) > 0)
+    U = _random_levels(rng, w)
+    orc, gpu = _pair(w, U, chemistry=0)
+    for step in range(2):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        eN, eF = _errors(orc, gpu, w)
+        assert eN <= TOL_NF and eF <= TOL_NF, (step, eN, eF)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+        assert abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-6 * do["photons_total"]
+    gpu.close()
+
+
+def test_amr_photons_conserved_on_the_gpu():
+    rng = np.random.default_rng(3)
+    w = make_amr_standard(n=16, G=1, levels=2, seed=5, thresh1=3.0, thresh2=4.0)
+    w.chemistry, w.src_pos = 0, None
+    orc, gpu = _pair(w, _random_levels(rng, w), chemistry=0)
+    _, d0 = gpu.step(w.dt, 1)
+    _, d1 = gpu.step(w.dt, 3)
+    assert abs(d1["photons_total"] - d0["photons_total"]) <= TOL_BUDGET * d0["photons_total"]
+    gpu.close()
+
+
+@pytest.mark.parametrize("G", [1, 3])
+def test_amr_coupled_steps(G):
+    """sources in the finest leaves, chemistry on every level with its own dt; x, T after 12 coarse steps."""
+    n, n_steps = 16, 12
+    w = make_amr_standard(n=n, G=G, levels=2, seed=21 + G, thresh1=3.0, thresh2=4.0)
+    w.src_Q = w.src_Q * 300.0                                  # bright enough to ionise the source leaves in 12 steps
+    orc, gpu = _pair(w)
+    flips, prev = [], 0.0
+    anc = coarse_ancestors(w)
+    for step in range(1, n_steps + 1):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        assert budget_residual(dg, prev) <= TOL_BUDGET, (step, dg)
+        prev = dg["photons_total"]
+        assert dg["photons_injected"] == pytest.approx(do["photons_injected"], rel=1e-6)
+        assert dg["photons_absorbed"] == pytest.approx(do["photons_absorbed"], rel=1e-4)
+        for l in range(w.n_levels + 1):
+            so = orc.read(O.F_SUBCYCLES, l).astype(np.int64)
+            sg = gpu.read(E.FIELD_SUBCYCLES, l).astype(np.int64)
+            for c in np.flatnonzero(so != sg):
+                flips.append((step, l, int(c), int(anc[l][c])))
+    masks = clean_masks(w, flips, n_steps)
+    frac = sum((~m).sum() for m in masks) / sum(m.size for m in masks)
+    assert frac <= 0.05, (len(flips), frac)
+    for name, fo, fg in (("x", O.F_X, E.FIELD_X), ("T", O.F_T, E.FIELD_T)):
+        for l in range(w.n_levels + 1):
+            a = orc.read(fo, l)[masks[l]]
+            b = gpu.read(fg, l).astype(np.float64)[masks[l]]
+            assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, (name, l)
+    # radiation: optically thick cells amplify the fp32 rounding of 1-x (tests/parity.py absorption_condition); compare
+    # where light has arrived, with the A17 floor
+    eN, eF = _errors(orc, gpu, w, masks)
+    assert eN <= 2e-4 and eF <= 2e-4, (eN, eF)
+    assert orc.read(O.F_X, 2).max() > 0.5                      # the sources did ionise their leaves
+    gpu.close()
+
+
+def test_amr_refusals_and_io():
+    n = 8
+    parents = [np.array([21 + 64], np.int64), np.array([0], np.int64)]       # a level-2 oct inside a lone level-1 oct
+    w = tiny_workload(n, G=1, parent=parents)
+    with pytest.raises(E.EmmaRTError) as ei:
+        E.EmmaRT(w, amr_transport=1)
+    assert ei.value.code == E.EINVAL
+    w = make_amr_standard(n=8, G=1, levels=1, thresh1=3.0)
+    gpu = E.EmmaRT(w, amr_transport=1)
+    assert E.lib().emma_rt_set_flux(gpu.h, E.FLUX_HLL) == E.ESTATE
+    m = gpu.level_cells(1)
+    U = np.arange(4 * m, dtype=np.float32).reshape(m, 4)
+    assert gpu.write(E.FIELD_U, 1, 0, U) == E.OK
+    back = gpu.read(E.FIELD_U, 1, 0)
+    np.testing.assert_allclose(back, U, rtol=2e-7)
+    gpu.close()
+    crta = E.EmmaRT(w)                                         # CRTA handle: refined radiation is not addressable
+    with pytest.raises(E.EmmaRTError):
+        crta.read(E.FIELD_U, 1, 0)
+    crta.close()
