@@ -190,9 +190,14 @@ def run_ours(args):
 
     n, K, W = args.n, args.steps, args.warmup
     t0 = time.time()
-    if args.config == 4:
+    if args.config == 4 and not args.amr_standard:
         # BASELINE config 4: 256^3 coarse + 2 refined levels (CRTA); transport on the coarse level, chemistry on leaves
         w = make_config(4, n=None if n == 512 else n, seed=replica_seed(4, rank, world))
+        n = w.n
+    elif args.amr_standard:
+        # the standard (non-CRTA) AMR scheme on a jump-balanced config-4-like mesh
+        from workloads.amr import make_amr_standard
+        w = make_amr_standard(n=256 if n == 512 else n, G=3, levels=2, seed=replica_seed(4, rank, world))
         n = w.n
     else:
         w = make_config(5, n=n, variant=args.variant, seed=replica_seed(5, rank, world))
@@ -200,9 +205,14 @@ def run_ours(args):
     ncell = n ** 3
     log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
 
-    gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
+    amr = 1 if args.amr_standard else 0
+    gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr)
     dt = w.dt
     units_per_step = leaf_count(w) * G            # config 5: n^3 G; config 4: leaf cells x G
+    lv_cells = [n ** 3] + [8 * len(p) for p in w.parent]
+    lv_leaves = [c - s for c, s in zip(lv_cells, [len(p) for p in w.parent] + [0])]
+    if amr:                                       # a level-l leaf is advanced 2^l times per coarse step (dt_l = dt/2^l)
+        units_per_step = sum(lv_leaves[l] << l for l in range(len(lv_leaves))) * G
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -236,11 +246,18 @@ def run_ours(args):
     alg = {"transport": 32.0 * ncell * G,                    # 16 B read + 16 B write per cell-group
            "chem_main": (32.0 * G + 20.0) * ncell,           # U in/out + n0, x, e in + x, e out per cell
            "fused": (32.0 * G + 20.0) * ncell}               # single pass: U in, U out, n0, x, e in, x, e out
+    # refined-level sweeps of the standard AMR scheme: bytes of all the sweeps of one coarse step (levels >= 1)
+    alg_step = {"amr_transport": 32.0 * G * sum(lv_leaves[l] << l for l in range(1, len(lv_leaves))),
+                "amr_chem": (32.0 * G + 20.0) * sum(lv_leaves[l] << l for l in range(1, len(lv_leaves)))}
     kern = {}
     for k, (kms, cnt) in prof.items():
         if cnt:
             kern[k] = {"ms_per_launch": kms / cnt, "launches": int(cnt), "share": kms / ms}
-            if k in alg:
+            if k in alg_step and amr:
+                kern[k]["GBps"] = alg_step[k] * K / (kms * 1e-3) / 1e9
+                kern[k]["frac"] = kern[k]["GBps"] / peak
+                alg[k] = alg_step[k] * K / cnt
+            elif k in alg:
                 kern[k]["GBps"] = alg[k] / (kms / cnt * 1e-3) / 1e9
                 kern[k]["frac"] = kern[k]["GBps"] / peak
     dominant = max((k for k in kern if k in alg), key=lambda k: kern[k]["share"])
@@ -251,7 +268,7 @@ def run_ours(args):
 
     # ---------------- transport-only throughput (chemistry = 0), same grid, K steps
     tr = hll = None
-    if not args.skip_transport_only:
+    if not args.skip_transport_only and not amr:
         gpu.close()
         gpu = None
         torch.cuda.empty_cache()
@@ -282,7 +299,7 @@ def run_ours(args):
         hll["frac"] = hll["GBps"] / peak
         g3.close()
         torch.cuda.empty_cache()
-        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1)
+        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr)
 
     # ---------------- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
     Ke = max(1, min(K, args.e2e_steps))
@@ -319,7 +336,21 @@ def run_ours(args):
 
     # ---------------- oracle on the host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
-    if rank == 0 and world == 1 and not args.skip_cpu_baseline:
+    if rank == 0 and world == 1 and not args.skip_cpu_baseline and amr:
+        import oracle as O
+        from workloads.amr import make_amr_standard
+        ws = make_amr_standard(n=32, G=3, levels=2)
+        orc = O.Oracle(ws)
+        assert orc.set_amr_transport(True) == O.OK
+        lc = [ws.n ** 3] + [8 * len(p) for p in ws.parent]
+        ll = [c - s_ for c, s_ in zip(lc, [len(p) for p in ws.parent] + [0])]
+        t0 = time.perf_counter()
+        orc.step(ws.dt, 6)
+        secs = time.perf_counter() - t0
+        cpu = {"value": sum(ll[l] << l for l in range(3)) * 3 * 6 / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
+               "sample": "standard-AMR recipe at 32^3 coarse + 2 levels x 3 groups, 6 coarse steps, fp64 C oracle (the AMR "
+                         "recursion of the oracle is serial)"}
+    elif rank == 0 and world == 1 and not args.skip_cpu_baseline:
         val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N if args.config == 5 else 96, ORACLE_SAMPLE_STEPS, 0, args.variant, args.config)
         cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                "sample": "config %s recipe at %d^3 x 3 groups, %d coupled steps from the initial state, fp64 C oracle, "
@@ -332,7 +363,11 @@ def run_ours(args):
                 "data": "synthetic",
                 "config": {"workload": ("BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
                                         "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)))
-                           if args.config == 5 else
+                           if args.config == 5 and not amr else
+                           ("standard AMR scheme (SURVEY 8f NEXT-2, reading A21): %d^3 coarse + 2 refined levels on a jump-balanced "
+                            "config-4-like mesh, %d groups, cells per level %s, leaves per level %s, %d sources; value counts "
+                            "leaf-cell-group updates, a level-l leaf 2^l times per coarse step" % (n, G, lv_cells, lv_leaves, len(w.src_pos)))
+                           if amr else
                            ("BASELINE config 4: %d^3 coarse + 2 refined levels (CRTA), %d groups, lognormal sigma_ln=1.5, "
                             "%d leaves, %d sources; value counts leaf-cell-group updates" % (n, G, leaf_count(w), len(w.src_pos))),
                            "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
@@ -358,6 +393,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[4, 5], help="BASELINE config: 5 (default, the metric's) or 4 (CRTA)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--unfused", action="store_true", help="separate transport and chemistry passes")
+    ap.add_argument("--amr-standard", action="store_true",
+                    help="the standard (non-CRTA) AMR scheme on a jump-balanced 256^3 + 2 levels mesh (SURVEY 8f NEXT-2)")
     ap.add_argument("--skip-transport-only", action="store_true")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     args = ap.parse_args()

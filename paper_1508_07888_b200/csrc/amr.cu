@@ -6,8 +6,9 @@
 //   * amr_transport_kernel: Eq. 30 + 32 for the LEAF cells of a refined level, one thread per cell and all G groups.
 //     Neighbours are found through the oct structure the paper describes (each oct points to the 6 cells of
 //     the level below that surround its parent cell); siblings sit in the same 128-byte oct record.  A face towards a
-//     split cell computes nothing (the fine cells behind it deposit), a face towards a coarser leaf uses the MinMod-limited
-//     linear ghost and deposits the same flux / 8 into that leaf with red.global.add.f32.
+//     split cell computes nothing (the fine cells behind it deposit).
+//   * amr_ghost_faces_kernel: the faces towards a coarser leaf, one thread per face from a host-built list: MinMod-limited
+//     linear ghost, flux, the fine cell's change and the same flux / 8 deposited into that leaf (red.global.add.f32).
 //   * level 0 keeps the dense TMA kernel (transport_tma.cu) for the whole block; amr_fix0_kernel then recomputes the
 //     (few) leaves that touch a split cell without the faces towards it and adds what the fine cells deposited: the
 //     regular block stays on the bandwidth-bound kernel, the irregular part is a sparse second pass.
@@ -36,7 +37,8 @@ __device__ __forceinline__ NbRef box_ghost(int bc, int a, int side, int lvl, lon
 __device__ NbRef nb_ref0(const AmrDev& A, long long cell, int a, int side)
 {
   const int n = A.n;
-  const int i = (int)(cell % n), j = (int)((cell / n) % n), k = (int)(cell / ((long long)n * n));
+  const unsigned uc = (unsigned)cell, t = uc / (unsigned)n;          // n^3 < 2^32 (n <= 1290)
+  const int i = (int)(uc % (unsigned)n), j = (int)(t % (unsigned)n), k = (int)(t / (unsigned)n);
   int ca = (a == 0) ? i : (a == 1) ? j : k;
   const long long stride = (a == 0) ? 1 : (a == 1) ? n : (long long)n * n;
   const int cn = ca + (side ? 1 : -1);
@@ -92,25 +94,6 @@ __device__ __forceinline__ float minmod(float a, float b)
   return (fabsf(a) < fabsf(b)) ? a : b;
 }
 
-// the missing fine neighbour is interpolated linearly from coarse data at the position of the virtual
-// fine cell (child index kv of the coarse leaf c on level lc); slopes MinMod-limited (A21)
-__device__ float4 ghost_state(const AmrDev& A, int lc, long long c, int kv, int g)
-{
-  const float4 Uc = A.U[lc][(size_t)g * A.ncell[lc] + c];
-  float4 out = Uc;
-#pragma unroll
-  for (int b = 0; b < 3; b++) {
-    const NbRef rm = nb_ref(A, lc, c, b, 0), rp = nb_ref(A, lc, c, b, 1);
-    const float4 Um = nb_load(A, rm, g, Uc), Up = nb_load(A, rp, g, Uc);
-    const float sg = ((kv >> b) & 1) ? 0.25f : -0.25f;
-    out.x = fmaf(sg, minmod(Uc.x - Um.x, Up.x - Uc.x), out.x);
-    out.y = fmaf(sg, minmod(Uc.y - Um.y, Up.y - Uc.y), out.y);
-    out.z = fmaf(sg, minmod(Uc.z - Um.z, Up.z - Uc.z), out.z);
-    out.w = fmaf(sg, minmod(Uc.w - Um.w, Up.w - Uc.w), out.w);
-  }
-  return out;
-}
-
 // G_a(U) = (phi_a, a e_a + b phi_a phi): the flux vector of direction a in units of c_red (closure_ab: P = a I + b phi(x)phi)
 __device__ __forceinline__ float4 flux_vec(const float4& U, float ca, float cb, int a)
 {
@@ -163,18 +146,15 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
       closure_ab(Ui[g], ai[g], bi[g]);
       ac[g] = Ui[g];
     }
-    const int k = (int)(cell & 7);
     for (int a = 0; a < 3; a++)
       for (int side = 0; side < 2; side++) {
         const NbRef r = nb_ref(A, l, cell, a, side);
-        if (r.kind == 1) continue;                                  // Fig. 3 (iii): fed by the fine steps
+        if (r.kind == 1 || r.kind == 2) continue;                   // split: fed by the fine steps (Fig. 3 (iii));
+                                                                    // coarser: amr_ghost_faces_kernel adds that face
 #pragma unroll
         for (int g = 0; g < G; g++) {
-          const float4 Un = (r.kind == 2) ? ghost_state(A, r.lvl, r.cell, k ^ (1 << a), g) : nb_load(A, r, g, Ui[g]);
-          const float4 d = face_change(a, side, Ui[g], ai[g], bi[g], Un, nuh);
+          const float4 d = face_change(a, side, Ui[g], ai[g], bi[g], nb_load(A, r, g, Ui[g]), nuh);
           ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
-          if (r.kind == 2)                                          // Fig. 3 (i)-(ii): the same flux, seen from the coarse leaf
-            red_add4(A.dep[r.lvl] + (size_t)g * A.ncell[r.lvl] + r.cell, make_float4(-0.125f * d.x, -0.125f * d.y, -0.125f * d.z, -0.125f * d.w));
           if (r.kind >= 3) acc.outflow -= (double)d.x * dV;         // A15: net N-flux through a box face
         }
       }
@@ -193,6 +173,47 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     for (int g = 0; g < G; g++) Unew[(size_t)g * ncell + cell] = ac[g];
   }
   block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// The faces of refined leaves that look at a coarser leaf (resolution jump), one thread per face from a list the host
+// built once for the static mesh: the six coarse references are resolved once, then per group the MinMod ghost
+// (PAPER.md:436), the Eq. 32 flux, the fine cell's change (added to what amr_transport_kernel wrote) and the same
+// flux / 8 deposited into the coarse leaf (Fig. 3 (i)-(ii)).  Uniform work per thread: the irregular part of the
+// level is taken out of the per-cell kernel, where it made every warp on a patch boundary run the ghost code.
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, const int* __restrict__ slot_cell,
+                       const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face, int n_slots)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_slots) return;
+  const long long cell = slot_cell[i], c = slot_coarse[i];
+  const int f = slot_face[i], a = f >> 1, side = f & 1, lc = l - 1;
+  const int kv = (int)(cell & 7) ^ (1 << a);                        // child index of the virtual cell inside c
+  const long long ncell = A.ncell[l], ncc = A.ncell[lc];
+  NbRef rr[6];
+#pragma unroll
+  for (int b = 0; b < 3; b++) { rr[2 * b] = nb_ref(A, lc, c, b, 0); rr[2 * b + 1] = nb_ref(A, lc, c, b, 1); }
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float4 Uc = A.U[lc][(size_t)g * ncc + c];
+    float4 Un = Uc;
+#pragma unroll
+    for (int b = 0; b < 3; b++) {
+      const float4 Um = nb_load(A, rr[2 * b], g, Uc), Up = nb_load(A, rr[2 * b + 1], g, Uc);
+      const float sg = ((kv >> b) & 1) ? 0.25f : -0.25f;
+      Un.x = fmaf(sg, minmod(Uc.x - Um.x, Up.x - Uc.x), Un.x);
+      Un.y = fmaf(sg, minmod(Uc.y - Um.y, Up.y - Uc.y), Un.y);
+      Un.z = fmaf(sg, minmod(Uc.z - Um.z, Up.z - Uc.z), Un.z);
+      Un.w = fmaf(sg, minmod(Uc.w - Um.w, Up.w - Uc.w), Un.w);
+    }
+    const float4 Ui = A.U[l][(size_t)g * ncell + cell];
+    float ai, bi;
+    closure_ab(Ui, ai, bi);
+    const float4 d = face_change(a, side, Ui, ai, bi, Un, nuh);
+    red_add4(Unew + (size_t)g * ncell + cell, d);                   // a cell can have up to 3 such faces
+    red_add4(A.dep[lc] + (size_t)g * ncc + c, make_float4(-0.125f * d.x, -0.125f * d.y, -0.125f * d.z, -0.125f * d.w));
+  }
 }
 
 // Eq. 43-48 on the leaves of a refined level, in place, over cp.dt (= dt / 2^level)
@@ -384,6 +405,15 @@ int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, do
   const int nb = grid_for(A.ncell[level], 128, AMR_GRID_CAP);
   AMR_DISPATCH(A.G, (amr_transport_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts)));
   *n_parts = nb;
+  return 1;
+}
+
+int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
+                           const unsigned char* slot_face, int n_slots, cudaStream_t st)
+{
+  if (n_slots == 0) return 0;
+  const int nb = (n_slots + 127) / 128;
+  AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, n_slots)));
   return 1;
 }
 

@@ -34,6 +34,7 @@ struct Layout {
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
   size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], achild0, afix_cell, afix_mask;
+  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
 
@@ -104,6 +105,10 @@ void make_layout(const Shape& s, Layout& L)
       if (l >= 1) {
         for (int b = 0; b < 2; b++) L.aU[b][l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
         L.anbr[l] = take((size_t)s.nocts[l] * 6 * 4);
+        // capacity: every face cell of every oct (24 per oct); the list built at init is normally a small fraction
+        L.aslot_cell[l] = take((size_t)s.nocts[l] * 24 * 4);
+        L.aslot_coarse[l] = take((size_t)s.nocts[l] * 24 * 4);
+        L.aslot_face[l] = take((size_t)s.nocts[l] * 24);
       }
       if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
     }
@@ -139,6 +144,7 @@ struct emma_rt {
   // standard AMR transport (A21)
   int acur[MAXL + 1];                          // aU[acur[l]][l] holds the current radiation of refined level l
   int n_fix;                                   // level-0 leaves with a split face neighbour
+  int n_slots[MAXL + 1];                       // faces of the leaves of a refined level towards a coarser leaf
   bool amr_dirty;                              // U was written: restrict bottom-up before the next step
   char err[256];
 
@@ -323,7 +329,9 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   std::vector<int> child0_h, fix_cell_h;
   std::vector<unsigned char> fix_mask_h;
   h->n_fix = 0; h->amr_dirty = false;
-  for (int l = 0; l <= MAXL; l++) h->acur[l] = 0;
+  for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
+  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1);
+  std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
   if (s.amr) {
     const int n = s.n;
     auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
@@ -369,6 +377,30 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     child0_h.assign((size_t)s.ncell[0], -1);
     for (auto& kv : h->child_of[0]) child0_h[kv.first] = kv.second;
     CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.achild0, child0_h.data(), child0_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+    // faces of refined cells towards a coarser leaf: (fine cell, coarse leaf, face), 4 per oct face
+    for (int l = 1; l <= s.nl; l++) {
+      for (long long o = 0; o < s.nocts[l]; o++)
+        for (int f = 0; f < 6; f++) {
+          const int pcell = nbr_h[l][o * 6 + f];
+          if (pcell < 0) continue;
+          const bool split = (l == 1) ? child0_h[pcell] >= 0 : child_h[l - 1][pcell] >= 0;
+          if (split) continue;
+          const int a = f >> 1, side = f & 1;
+          for (int k = 0; k < 8; k++) {
+            if (((k >> a) & 1) != side) continue;
+            if (l < s.nl && child_h[l][(o << 3) | k] >= 0) continue;      // jumps <= 1 make this impossible; be safe
+            slot_cell_h[l].push_back((int)((o << 3) | k));
+            slot_coarse_h[l].push_back(pcell);
+            slot_face_h[l].push_back((unsigned char)f);
+          }
+        }
+      h->n_slots[l] = (int)slot_cell_h[l].size();
+      if (h->n_slots[l]) {
+        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_cell[l], slot_cell_h[l].data(), slot_cell_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_coarse[l], slot_coarse_h[l].data(), slot_coarse_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_face[l], slot_face_h[l].data(), slot_face_h[l].size(), cudaMemcpyHostToDevice, h->st));
+      }
+    }
     // level-0 leaves next to a split cell, with the mask of the faces that look at one (sorted by cell id)
     std::map<long long, unsigned> fix;
     for (auto& kv : h->child_of[0])
@@ -590,6 +622,9 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           AmrDev A = amr_view(h);
           h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
           h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, P + off, &np, h->st);
+          h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
+                                                (const int*)(h->arena + h->lay.aslot_coarse[l]),
+                                                (const unsigned char*)(h->arena + h->lay.aslot_face[l]), h->n_slots[l], h->st);
           h->prof.end();
           off += np;
           h->acur[l] = 1 - h->acur[l];
