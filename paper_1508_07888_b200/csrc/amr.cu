@@ -106,10 +106,9 @@ __device__ __forceinline__ float4 flux_vec(const float4& U, float ca, float cb, 
 
 // change of the cell (state Ui, closure ai/bi) caused by the Eq. 32 flux through its face (a, side) towards state Un:
 //   + face: -nu F^ = -(nu/2) [(G_i + U_i) + (G_n - U_n)];   - face: +(nu/2) [(G_n + U_n) + (G_i - U_i)]
-__device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui, float ai, float bi, const float4& Un, float nuh)
+__device__ __forceinline__ float4 face_change_pre(int a, int side, const float4& Ui, float ai, float bi, const float4& Un,
+                                                 float an, float bn, float nuh)
 {
-  float an, bn;
-  closure_ab(Un, an, bn);
   const float4 Gi = flux_vec(Ui, ai, bi, a), Gn = flux_vec(Un, an, bn, a);
   float4 r;
   if (side) {
@@ -121,6 +120,12 @@ __device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui,
   }
   return r;
 }
+__device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui, float ai, float bi, const float4& Un, float nuh)
+{
+  float an, bn;
+  closure_ab(Un, an, bn);
+  return face_change_pre(a, side, Ui, ai, bi, Un, an, bn, nuh);
+}
 
 __device__ __forceinline__ void red_add4(float4* p, const float4& v)
 {
@@ -128,36 +133,73 @@ __device__ __forceinline__ void red_add4(float4* p, const float4& v)
   atomicAdd(q + 0, v.x); atomicAdd(q + 1, v.y); atomicAdd(q + 2, v.z); atomicAdd(q + 3, v.w);
 }
 
+// 8 consecutive lanes hold one oct: the three sibling faces of a cell take the neighbour's state AND its closure from
+// the partner lane (shfl.xor by 1, 2, 4): no load and no second closure for half of the faces.  The three outer faces
+// go through `nbo` (same-level neighbour oct, derived on the host from the paper's neighbour-cell pointers for the
+// static mesh): one dependent load less than nbr -> child.
 template <int G>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 8)
 amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, double dV, Partial* __restrict__ parts)
 {
   Acc acc;
-  const long long ncell = A.ncell[l];
+  const long long ncell = A.ncell[l];                                // a multiple of 8
   const float4* __restrict__ Ul = A.U[l];
-  const int* child = (l < A.nl) ? A.child[l] : nullptr;
-  for (long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x; cell < ncell; cell += (long long)gridDim.x * blockDim.x) {
-    if (child && child[cell] >= 0) continue;                        // split: restricted from its children later
+  const int* __restrict__ child = (l < A.nl) ? A.child[l] : nullptr;
+  const int* __restrict__ nbo = A.nbo[l];
+  const long long span = (long long)gridDim.x * blockDim.x;
+  for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += span) {
+    const long long cell = base + threadIdx.x;
+    const bool valid = cell < ncell;                                 // uniform per 8-lane group
+    const bool leaf = valid && !(child && child[cell] >= 0);
     float4 Ui[G], ac[G];
     float ai[G], bi[G];
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      Ui[g] = Ul[(size_t)g * ncell + cell];
+      Ui[g] = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
       closure_ab(Ui[g], ai[g], bi[g]);
       ac[g] = Ui[g];
     }
-    for (int a = 0; a < 3; a++)
-      for (int side = 0; side < 2; side++) {
-        const NbRef r = nb_ref(A, l, cell, a, side);
-        if (r.kind == 1 || r.kind == 2) continue;                   // split: fed by the fine steps (Fig. 3 (iii));
-                                                                    // coarser: amr_ghost_faces_kernel adds that face
+    const int k = (int)(cell & 7);
+    const long long oct = cell >> 3;
 #pragma unroll
-        for (int g = 0; g < G; g++) {
-          const float4 d = face_change(a, side, Ui[g], ai[g], bi[g], nb_load(A, r, g, Ui[g]), nuh);
+    for (int a = 0; a < 3; a++) {
+      const int bit = (k >> a) & 1;
+      // sibling face: side = 1 - bit
+      const bool sib_leaf = __shfl_xor_sync(0xffffffffu, leaf ? 1 : 0, 1 << a) != 0;
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        float4 Us;
+        Us.x = __shfl_xor_sync(0xffffffffu, Ui[g].x, 1 << a); Us.y = __shfl_xor_sync(0xffffffffu, Ui[g].y, 1 << a);
+        Us.z = __shfl_xor_sync(0xffffffffu, Ui[g].z, 1 << a); Us.w = __shfl_xor_sync(0xffffffffu, Ui[g].w, 1 << a);
+        const float as = __shfl_xor_sync(0xffffffffu, ai[g], 1 << a), bs = __shfl_xor_sync(0xffffffffu, bi[g], 1 << a);
+        if (leaf && sib_leaf) {                                      // a split sibling: fed by the fine steps (Fig. 3 (iii))
+          const float4 d = face_change_pre(a, 1 - bit, Ui[g], ai[g], bi[g], Us, as, bs, nuh);
           ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
-          if (r.kind >= 3) acc.outflow -= (double)d.x * dV;         // A15: net N-flux through a box face
         }
       }
+      // outer face: side = bit
+      if (!leaf) continue;
+      const int no = nbo[oct * 6 + 2 * a + bit];
+      if (no == -1) continue;                                        // coarser leaf: amr_ghost_faces_kernel adds that face
+      if (no >= 0) {
+        const long long nb = ((long long)no << 3) | (k ^ (1 << a));
+        if (child && child[nb] >= 0) continue;                       // split neighbour
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 d = face_change(a, bit, Ui[g], ai[g], bi[g], Ul[(size_t)g * ncell + nb], nuh);
+          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+        }
+      } else {                                                       // box face: -2 - bc
+        const NbRef r = box_ghost(-2 - no, a, bit, l, cell);
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 d = face_change(a, bit, Ui[g], ai[g], bi[g], nb_load(A, r, g, Ui[g]), nuh);
+          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+          acc.outflow -= (double)d.x * dV;                           // A15: net N-flux through a box face
+        }
+      }
+    }
+    if (!leaf) continue;
     if (l < A.nl) {
 #pragma unroll
       for (int g = 0; g < G; g++) {

@@ -33,7 +33,7 @@ struct Layout {
   size_t queue, qcount, parts, diag;
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
-  size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], achild0, afix_cell, afix_mask;
+  size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
   size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
@@ -105,6 +105,7 @@ void make_layout(const Shape& s, Layout& L)
       if (l >= 1) {
         for (int b = 0; b < 2; b++) L.aU[b][l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
         L.anbr[l] = take((size_t)s.nocts[l] * 6 * 4);
+        L.anbo[l] = take((size_t)s.nocts[l] * 6 * 4);
         // capacity: every face cell of every oct (24 per oct); the list built at init is normally a small fraction
         L.aslot_cell[l] = take((size_t)s.nocts[l] * 24 * 4);
         L.aslot_coarse[l] = take((size_t)s.nocts[l] * 24 * 4);
@@ -193,6 +194,7 @@ AmrDev amr_view(const emma_rt* h)
     A.dep[l] = l < s.nl ? (float4*)(h->arena + h->lay.adep[l]) : nullptr;
     A.child[l] = l == 0 ? (const int*)(h->arena + h->lay.achild0) : l < s.nl ? h->lv[l].child : nullptr;
     A.nbr[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbr[l]) : nullptr;
+    A.nbo[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbo[l]) : nullptr;
   }
   return A;
 }
@@ -330,7 +332,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   std::vector<unsigned char> fix_mask_h;
   h->n_fix = 0; h->amr_dirty = false;
   for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
-  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1);
+  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1);
   std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
   if (s.amr) {
     const int n = s.n;
@@ -377,6 +379,16 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     child0_h.assign((size_t)s.ncell[0], -1);
     for (auto& kv : h->child_of[0]) child0_h[kv.first] = kv.second;
     CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.achild0, child0_h.data(), child0_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+    // same-level neighbour octs, derived from the neighbour-cell pointers
+    for (int l = 1; l <= s.nl; l++) {
+      nbo_h[l].resize((size_t)s.nocts[l] * 6);
+      for (size_t i = 0; i < nbo_h[l].size(); i++) {
+        const int pcell = nbr_h[l][i];
+        if (pcell < 0) { nbo_h[l][i] = pcell - 1; continue; }              // -1 - bc  ->  -2 - bc
+        nbo_h[l][i] = (l == 1) ? child0_h[pcell] : child_h[l - 1][pcell];  // oct of level l, or -1: coarser leaf
+      }
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+    }
     // faces of refined cells towards a coarser leaf: (fine cell, coarse leaf, face), 4 per oct face
     for (int l = 1; l <= s.nl; l++) {
       for (long long o = 0; o < s.nocts[l]; o++)

@@ -219,6 +219,8 @@ struct AmrDev {
   const int* child[MAXL + 1];   // [ncell] oct on the level above or -1 (levels < nl)
   const int* nbr[MAXL + 1];     // [nocts][6] cell of the level below next to the oct's parent cell in -x,+x,-y,+y,-z,+z,
                                 // or -1 - bc for a non-periodic box face (levels >= 1)
+  const int* nbo[MAXL + 1];     // [nocts][6] derived for the static mesh: the oct of the SAME level behind each face of the
+                                // oct, -1 if that side is a coarser leaf, -2 - bc for a non-periodic box face (levels >= 1)
   float4 inflow[6][MAXG];
 };
 

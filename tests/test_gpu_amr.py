@@ -70,7 +70,7 @@ def _errors(orc, gpu, w, masks=None):
                                            (16, 2, 2, (1, 1, 2, 1, 0, 0)), (10, 1, 2, (2, 2, 1, 1, 1, 2))])
 def test_amr_transport_one_coarse_step(n, G, levels, bc):
     rng = np.random.default_rng(100 * n + 10 * G + levels)
-    w = make_amr_standard(n=n, G=3 if G == 3 else 1, levels=levels, seed=77 + n, thresh1=3.0, thresh2=4.0)
+    w = make_amr_standard(n=n, G=3 if G == 3 else 1, levels=levels, seed=77 + n, thresh1=2.0, thresh2=2.5)
     if G == 2:
         t = tiny_workload(n, G=2, parent=w.parent, chemistry=0, bc=bc, L=w.L)
         w = t
@@ -91,7 +91,7 @@ def test_amr_transport_one_coarse_step(n, G, levels, bc):
 
 def test_amr_photons_conserved_on_the_gpu():
     rng = np.random.default_rng(3)
-    w = make_amr_standard(n=16, G=1, levels=2, seed=5, thresh1=3.0, thresh2=4.0)
+    w = make_amr_standard(n=16, G=1, levels=2, seed=5, thresh1=2.0, thresh2=2.5)
     w.chemistry, w.src_pos = 0, None
     orc, gpu = _pair(w, _random_levels(rng, w), chemistry=0)
     _, d0 = gpu.step(w.dt, 1)
@@ -104,7 +104,7 @@ def test_amr_photons_conserved_on_the_gpu():
 def test_amr_coupled_steps(G):
     """sources in the finest leaves, chemistry on every level with its own dt; x, T after 12 coarse steps."""
     n, n_steps = 16, 12
-    w = make_amr_standard(n=n, G=G, levels=2, seed=21 + G, thresh1=3.0, thresh2=4.0)
+    w = make_amr_standard(n=n, G=G, levels=2, seed=21 + G, thresh1=2.0, thresh2=2.5)
     w.src_Q = w.src_Q * 300.0                                  # bright enough to ionise the source leaves in 12 steps
     orc, gpu = _pair(w)
     flips, prev = [], 0.0
@@ -145,7 +145,7 @@ def test_amr_refusals_and_io():
     with pytest.raises(E.EmmaRTError) as ei:
         E.EmmaRT(w, amr_transport=1)
     assert ei.value.code == E.EINVAL
-    w = make_amr_standard(n=8, G=1, levels=1, thresh1=3.0)
+    w = make_amr_standard(n=8, G=1, levels=1, thresh1=2.0)
     gpu = E.EmmaRT(w, amr_transport=1)
     assert E.lib().emma_rt_set_flux(gpu.h, E.FLUX_HLL) == E.ESTATE
     m = gpu.level_cells(1)

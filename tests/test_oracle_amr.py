@@ -96,7 +96,7 @@ def test_M1_full_refinement_is_the_uniform_fine_grid(levels, flux):
 
 
 def _partial_mesh(n, rng, levels=2):
-    w = make_amr_standard(n=n, G=1, levels=levels, seed=int(rng.integers(1 << 30)), thresh1=3.0, thresh2=4.0)
+    w = make_amr_standard(n=n, G=1, levels=levels, seed=int(rng.integers(1 << 30)), thresh1=2.0, thresh2=2.5)
     assert 0 < len(w.parent[0]) < n ** 3
     return w
 
@@ -223,7 +223,7 @@ def test_M4_brute_force(case):
 
 
 def test_M5_fig6_call_counts_of_the_standard_scheme():
-    w = make_amr_standard(n=8, G=1, levels=2, thresh1=3.0, thresh2=4.0)
+    w = make_amr_standard(n=8, G=1, levels=2, thresh1=2.0, thresh2=2.5)
     assert len(w.parent) == 2 and len(w.parent[1]) > 0
     o = oracle.Oracle(w)
     assert o.set_amr_transport(True) == oracle.OK

@@ -2,9 +2,11 @@
 
 Input recipe only: which cells are split, the densities of the children, the sources.  The paper's marking rule
 (PAPER.md:75-81): (i) mark cells by a physical criterion, (ii) "if a cell is marked for refinement, so must be its 26
-neighbors", jumps between neighbours never exceed one level.  Here: a coarse cell is marked when n0 > thresh * nbar,
-the marks are dilated once over the 26 neighbours (periodic wrap), and a level-1 cell is split only if it exceeds the
-threshold AND all its 26 level-1 neighbours exist, which keeps every face jump <= 1 by construction.
+neighbors", jumps between neighbours never exceed one level.  Here the criterion is the coarse density averaged over
+the 27 cells around a cell (S; refinement follows mass on a few-cell scale, so refined regions are patches, not single
+cells): a coarse cell is marked when S > thresh1 * nbar and the marks are dilated once over the 26 neighbours (periodic
+wrap); a level-1 cell is split when its parent has S > thresh2 * nbar (thresh2 >= thresh1: nested patches) and all its
+26 level-1 neighbours exist, which keeps every face jump <= 1 by construction.
 """
 import numpy as np
 
@@ -20,6 +22,15 @@ def _dilate26(m):
             for dx in (-1, 0, 1):
                 out |= np.roll(m, (dz, dy, dx), axis=(0, 1, 2))
     return out
+
+
+def _mean27(a):
+    out = np.zeros_like(a, dtype=np.float64)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                out += np.roll(a, (dz, dy, dx), axis=(0, 1, 2))
+    return out / 27.0
 
 
 def _all26(m):
@@ -39,9 +50,10 @@ def _children_density(n0_parent, rng):
     return ch.reshape(-1)
 
 
-def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=4.0, thresh2=8.0, levels=2):
+def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=2.5, thresh2=4.0, levels=2):
     """n0c: float64 [n^3] coarse densities.  Returns (parents, n0_levels): parents = [p1, p2][:levels]."""
-    mark0 = _dilate26((n0c.reshape(n, n, n) > thresh1 * nbar))
+    S = _mean27(n0c.reshape(n, n, n))
+    mark0 = _dilate26(S > thresh1 * nbar)
     p1 = np.flatnonzero(mark0.reshape(-1)).astype(np.int64)
     n01 = _children_density(n0c[p1], rng)
     if levels == 1 or len(p1) == 0:
@@ -53,15 +65,14 @@ def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=4.0, thresh2=8.0, levels=
         kx, ky, kz = k & 1, (k >> 1) & 1, (k >> 2) & 1
         id1[2 * K + kz, 2 * J + ky, 2 * I + kx] = 8 * np.arange(len(p1)) + k
     exist = id1 >= 0
-    dens1 = np.zeros(id1.shape)
-    dens1[exist] = n01[id1[exist]]
-    mark1 = exist & (dens1 > thresh2 * nbar) & _all26(exist)
+    S1 = np.repeat(np.repeat(np.repeat(S, 2, axis=0), 2, axis=1), 2, axis=2)       # the parent's S on the level-1 grid
+    mark1 = exist & (S1 > thresh2 * nbar) & _all26(exist)
     p2 = np.sort(id1[mark1]).astype(np.int64)
     n02 = _children_density(n01[p2], rng)
     return [p1, p2], [n0c, n01, n02]
 
 
-def make_amr_standard(n=16, G=3, levels=2, n_steps=4, n_src=None, sigma_ln=1.5, seed=None, thresh1=8.0, thresh2=8.0):
+def make_amr_standard(n=16, G=3, levels=2, n_steps=4, n_src=None, sigma_ln=1.5, seed=None, thresh1=2.5, thresh2=4.0):
     """Config-4-like box on a jump-balanced mesh, for the standard AMR transport: lognormal density,
     sources in the densest leaves of the finest level, x = 1.2e-3, T = 100 K, N = F = 0, periodic."""
     rng = np.random.default_rng(SEED_BASE + 42 if seed is None else seed)
