@@ -227,8 +227,9 @@ __global__ void __launch_bounds__(128)
 amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, const int* __restrict__ slot_cell,
                        const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face, int n_slots)
 {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_slots) return;
+  const int i0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = i0 < n_slots;                                   // n_slots is a multiple of 4: uniform per 4 lanes
+  const int i = live ? i0 : n_slots - 1;                            // idle lanes redo the last entry, write nothing
   const long long cell = slot_cell[i], c = slot_coarse[i];
   const int f = slot_face[i], a = f >> 1, side = f & 1, lc = l - 1;
   const int kv = (int)(cell & 7) ^ (1 << a);                        // child index of the virtual cell inside c
@@ -253,8 +254,15 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
     float ai, bi;
     closure_ab(Ui, ai, bi);
     const float4 d = face_change(a, side, Ui, ai, bi, Un, nuh);
-    red_add4(Unew + (size_t)g * ncell + cell, d);                   // a cell can have up to 3 such faces
-    red_add4(A.dep[lc] + (size_t)g * ncc + c, make_float4(-0.125f * d.x, -0.125f * d.y, -0.125f * d.z, -0.125f * d.w));
+    if (live) red_add4(Unew + (size_t)g * ncell + cell, d);         // a cell can have up to 3 such faces
+    // the 4 faces of one oct side are 4 consecutive list entries (aligned lanes) and share the coarse leaf: one deposit
+    float4 s4 = d;
+    s4.x += __shfl_xor_sync(0xffffffffu, s4.x, 1); s4.y += __shfl_xor_sync(0xffffffffu, s4.y, 1);
+    s4.z += __shfl_xor_sync(0xffffffffu, s4.z, 1); s4.w += __shfl_xor_sync(0xffffffffu, s4.w, 1);
+    s4.x += __shfl_xor_sync(0xffffffffu, s4.x, 2); s4.y += __shfl_xor_sync(0xffffffffu, s4.y, 2);
+    s4.z += __shfl_xor_sync(0xffffffffu, s4.z, 2); s4.w += __shfl_xor_sync(0xffffffffu, s4.w, 2);
+    if ((threadIdx.x & 3) == 0 && live)
+      red_add4(A.dep[lc] + (size_t)g * ncc + c, make_float4(-0.125f * s4.x, -0.125f * s4.y, -0.125f * s4.z, -0.125f * s4.w));
   }
 }
 

@@ -398,9 +398,10 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
           const bool split = (l == 1) ? child0_h[pcell] >= 0 : child_h[l - 1][pcell] >= 0;
           if (split) continue;
           const int a = f >> 1, side = f & 1;
-          for (int k = 0; k < 8; k++) {
+          for (int k = 0; k < 8; k++) {                                    // always 4 entries per oct side (kept aligned)
             if (((k >> a) & 1) != side) continue;
-            if (l < s.nl && child_h[l][(o << 3) | k] >= 0) continue;      // jumps <= 1 make this impossible; be safe
+            if (l < s.nl && child_h[l][(o << 3) | k] >= 0)
+              return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 at oct %lld of level %d (PAPER.md:75)", o, l);
             slot_cell_h[l].push_back((int)((o << 3) | k));
             slot_coarse_h[l].push_back(pcell);
             slot_face_h[l].push_back((unsigned char)f);
