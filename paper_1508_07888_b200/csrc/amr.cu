@@ -225,7 +225,8 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
 template <int G>
 __global__ void __launch_bounds__(128)
 amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, const int* __restrict__ slot_cell,
-                       const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face, int n_slots)
+                       const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face,
+                       const int* __restrict__ slot_refs, int n_slots)
 {
   const int i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = i0 < n_slots;                                   // n_slots is a multiple of 4: uniform per 4 lanes
@@ -234,16 +235,32 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
   const int f = slot_face[i], a = f >> 1, side = f & 1, lc = l - 1;
   const int kv = (int)(cell & 7) ^ (1 << a);                        // child index of the virtual cell inside c
   const long long ncell = A.ncell[l], ncc = A.ncell[lc];
-  NbRef rr[6];
+  // the six level-(l-1) neighbours of c, resolved on the host for the static mesh (one record per oct side):
+  //   >= 0 a cell of level l-1; <= -16 the coarser leaf -16 - code of level l-2 (piecewise constant); -1 box ghost = c
+  //   itself; -2, -3, -4 the same with flux component 0, 1, 2 inverted (A13); -5 the inflow state of that face (A20)
+  int rc[6];
 #pragma unroll
-  for (int b = 0; b < 3; b++) { rr[2 * b] = nb_ref(A, lc, c, b, 0); rr[2 * b + 1] = nb_ref(A, lc, c, b, 1); }
+  for (int j = 0; j < 6; j++) rc[j] = slot_refs[(size_t)(i >> 2) * 6 + j];
+  const long long ncc2 = lc > 0 ? A.ncell[lc - 1] : 0;
 #pragma unroll
   for (int g = 0; g < G; g++) {
     const float4 Uc = A.U[lc][(size_t)g * ncc + c];
+    float4 Unb[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+      const int code = rc[j];
+      if (code >= 0) Unb[j] = A.U[lc][(size_t)g * ncc + code];
+      else if (code <= -16) Unb[j] = A.U[lc - 1][(size_t)g * ncc2 + (-16 - code)];
+      else if (code == -5) Unb[j] = A.inflow[j][g];
+      else {
+        Unb[j] = Uc;
+        if (code == -2) Unb[j].y = -Uc.y; else if (code == -3) Unb[j].z = -Uc.z; else if (code == -4) Unb[j].w = -Uc.w;
+      }
+    }
     float4 Un = Uc;
 #pragma unroll
     for (int b = 0; b < 3; b++) {
-      const float4 Um = nb_load(A, rr[2 * b], g, Uc), Up = nb_load(A, rr[2 * b + 1], g, Uc);
+      const float4 Um = Unb[2 * b], Up = Unb[2 * b + 1];
       const float sg = ((kv >> b) & 1) ? 0.25f : -0.25f;
       Un.x = fmaf(sg, minmod(Uc.x - Um.x, Up.x - Uc.x), Un.x);
       Un.y = fmaf(sg, minmod(Uc.y - Um.y, Up.y - Uc.y), Un.y);
@@ -375,30 +392,57 @@ __global__ void __launch_bounds__(128)
 amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restrict__ Unew, const int* __restrict__ fix_cell,
                 const unsigned char* __restrict__ fix_mask, int n_fix, float nuh)
 {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_fix) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;                // one thread per (cell, group): independent loads
+  if (t >= n_fix * G) return;
+  const int i = t / G, g = t - i * G;
   const long long cell = fix_cell[i];
   const unsigned mask = fix_mask[i];
   const long long nc = A.ncell[0];
+  // all seven states and the deposit are requested before anything is used (the cells are scattered: one DRAM round
+  // trip instead of seven); a masked or box face reads the cell itself
+  const int n = A.n;
+  const unsigned uc = (unsigned)cell, tq = uc / (unsigned)n;
+  const int ci[3] = {(int)(uc % (unsigned)n), (int)(tq % (unsigned)n), (int)(tq / (unsigned)n)};
+  const long long stride[3] = {1, n, (long long)n * n};
+  long long idx[6];
+  int ghost[6];                                                     // 0 cell, 1 transmissive, 2 reflective, 3 inflow
+  bool on[6];
 #pragma unroll
-  for (int g = 0; g < G; g++) {
-    const float4 Ui = Uold[(size_t)g * nc + cell];
-    float ai, bi;
-    closure_ab(Ui, ai, bi);
-    float4 ac = Ui;
-    for (int f = 0; f < 6; f++) {
-      if ((mask >> f) & 1u) continue;
-      const NbRef r = nb_ref0(A, cell, f >> 1, f & 1);
-      const float4 Un = (r.kind >= 3) ? nb_load(A, r, g, Ui) : Uold[(size_t)g * nc + r.cell];
-      const float4 d = face_change(f >> 1, f & 1, Ui, ai, bi, Un, nuh);
+  for (int f = 0; f < 6; f++) {
+    const int a = f >> 1, side = f & 1, cn = ci[a] + (side ? 1 : -1);
+    on[f] = !((mask >> f) & 1u);
+    ghost[f] = 0;
+    idx[f] = cell + (side ? stride[a] : -stride[a]);
+    if (cn < 0 || cn >= n) {
+      const int bc = A.bc[f];
+      if (bc == EMMA_RT_BC_PERIODIC) idx[f] = cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride[a];
+      else { idx[f] = cell; ghost[f] = bc; }
+    }
+    if (!on[f]) idx[f] = cell;
+  }
+  const float4 Ui = Uold[(size_t)g * nc + cell];
+  float4* dp = A.dep[0] + (size_t)g * nc + cell;
+  const float4 dpv = *dp;
+  float4 Un[6];
+#pragma unroll
+  for (int f = 0; f < 6; f++) Un[f] = Uold[(size_t)g * nc + idx[f]];
+#pragma unroll
+  for (int f = 0; f < 6; f++) {
+    if (ghost[f] == EMMA_RT_BC_INFLOW) Un[f] = A.inflow[f][g];
+    else if (ghost[f] == EMMA_RT_BC_REFLECTIVE) { if ((f >> 1) == 0) Un[f].y = -Un[f].y; else if ((f >> 1) == 1) Un[f].z = -Un[f].z; else Un[f].w = -Un[f].w; }
+  }
+  float ai, bi;
+  closure_ab(Ui, ai, bi);
+  float4 ac = Ui;
+#pragma unroll
+  for (int f = 0; f < 6; f++)
+    if (on[f]) {
+      const float4 d = face_change(f >> 1, f & 1, Ui, ai, bi, Un[f], nuh);
       ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
     }
-    float4* dp = A.dep[0] + (size_t)g * nc + cell;
-    const float4 d = *dp;
-    ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
-    *dp = make_float4(0.f, 0.f, 0.f, 0.f);
-    Unew[(size_t)g * nc + cell] = ac;
-  }
+  ac.x += dpv.x; ac.y += dpv.y; ac.z += dpv.z; ac.w += dpv.w;
+  *dp = make_float4(0.f, 0.f, 0.f, 0.f);
+  Unew[(size_t)g * nc + cell] = ac;
 }
 
 // net N-flux through the non-periodic box faces of the level-0 LEAVES (the dense pass also counts split cells, whose
@@ -459,11 +503,11 @@ int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, do
 }
 
 int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
-                           const unsigned char* slot_face, int n_slots, cudaStream_t st)
+                           const unsigned char* slot_face, const int* slot_refs, int n_slots, cudaStream_t st)
 {
   if (n_slots == 0) return 0;
   const int nb = (n_slots + 127) / 128;
-  AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, n_slots)));
+  AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots)));
   return 1;
 }
 
@@ -508,7 +552,7 @@ int launch_amr_fix0(const AmrDev& A, const float4* Uold, float4* Unew, const int
                     int n_fix, float nuh, cudaStream_t st)
 {
   if (n_fix == 0) return 0;
-  const int nb = (n_fix + 127) / 128;
+  const int nb = (int)(((long long)n_fix * A.G + 127) / 128);
   AMR_DISPATCH(A.G, (amr_fix0_kernel<GG><<<nb, 128, 0, st>>>(A, Uold, Unew, fix_cell, fix_mask, n_fix, nuh)));
   return 1;
 }

@@ -34,7 +34,7 @@ struct Layout {
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
   size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
-  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1];   // faces of refined leaves towards a coarser leaf
+  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
 
@@ -110,6 +110,7 @@ void make_layout(const Shape& s, Layout& L)
         L.aslot_cell[l] = take((size_t)s.nocts[l] * 24 * 4);
         L.aslot_coarse[l] = take((size_t)s.nocts[l] * 24 * 4);
         L.aslot_face[l] = take((size_t)s.nocts[l] * 24);
+        L.aslot_refs[l] = take((size_t)s.nocts[l] * 6 * 6 * 4);     // 6 neighbour references per oct side
       }
       if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
     }
@@ -332,7 +333,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   std::vector<unsigned char> fix_mask_h;
   h->n_fix = 0; h->amr_dirty = false;
   for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
-  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1);
+  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1), slot_refs_h(s.nl + 1);
   std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
   if (s.amr) {
     const int n = s.n;
@@ -398,6 +399,27 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
           const bool split = (l == 1) ? child0_h[pcell] >= 0 : child_h[l - 1][pcell] >= 0;
           if (split) continue;
           const int a = f >> 1, side = f & 1;
+          // the six neighbours of the coarse leaf `pcell` on its own level l-1, for the ghost slopes (reading A21)
+          for (int b = 0; b < 3; b++)
+            for (int sd = 0; sd < 2; sd++) {
+              long long q;                                                 // >= 0: cell of level l-1; else a code
+              auto box = [&](int code) { const int bc = -1 - code; return bc == EMMA_RT_BC_INFLOW ? -5 : bc == EMMA_RT_BC_REFLECTIVE ? -2 - b : -1; };
+              if (l == 1) { q = nb0(pcell, b, sd); if (q < 0) q = box((int)q); }
+              else {
+                const long long po = pcell >> 3;
+                const int kk = pcell & 7, bit = (kk >> b) & 1;
+                if (sd != bit) q = (po << 3) | (kk ^ (1 << b));
+                else {
+                  const int pp = nbr_h[l - 1][po * 6 + 2 * b + sd];       // cell of level l-2
+                  if (pp < 0) q = box(pp);
+                  else {
+                    const int ch = (l == 2) ? child0_h[pp] : child_h[l - 2][pp];
+                    q = ch >= 0 ? (((long long)ch << 3) | (kk ^ (1 << b))) : (-16LL - pp);
+                  }
+                }
+              }
+              slot_refs_h[l].push_back((int)q);
+            }
           for (int k = 0; k < 8; k++) {                                    // always 4 entries per oct side (kept aligned)
             if (((k >> a) & 1) != side) continue;
             if (l < s.nl && child_h[l][(o << 3) | k] >= 0)
@@ -412,6 +434,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
         CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_cell[l], slot_cell_h[l].data(), slot_cell_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
         CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_coarse[l], slot_coarse_h[l].data(), slot_coarse_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
         CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_face[l], slot_face_h[l].data(), slot_face_h[l].size(), cudaMemcpyHostToDevice, h->st));
+        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_refs[l], slot_refs_h[l].data(), slot_refs_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
       }
     }
     // level-0 leaves next to a split cell, with the mask of the faces that look at one (sorted by cell id)
@@ -637,7 +660,8 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, P + off, &np, h->st);
           h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
                                                 (const int*)(h->arena + h->lay.aslot_coarse[l]),
-                                                (const unsigned char*)(h->arena + h->lay.aslot_face[l]), h->n_slots[l], h->st);
+                                                (const unsigned char*)(h->arena + h->lay.aslot_face[l]),
+                                                (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], h->st);
           h->prof.end();
           off += np;
           h->acur[l] = 1 - h->acur[l];

@@ -227,7 +227,7 @@ struct AmrDev {
 int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
                          cudaStream_t st);
 int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
-                           const unsigned char* slot_face, int n_slots, cudaStream_t st);
+                           const unsigned char* slot_face, const int* slot_refs, int n_slots, cudaStream_t st);
 int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, Partial* parts,
                     int* n_parts, cudaStream_t st);
 int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, Partial* parts,
