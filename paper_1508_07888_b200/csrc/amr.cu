@@ -133,10 +133,22 @@ __device__ __forceinline__ void red_add4(float4* p, const float4& v)
   atomicAdd(q + 0, v.x); atomicAdd(q + 1, v.y); atomicAdd(q + 2, v.z); atomicAdd(q + 3, v.w);
 }
 
-// 8 consecutive lanes hold one oct: the three sibling faces of a cell take the neighbour's state AND its closure from
-// the partner lane (shfl.xor by 1, 2, 4): no load and no second closure for half of the faces.  The three outer faces
-// go through `nbo` (same-level neighbour oct, derived on the host from the paper's neighbour-cell pointers for the
-// static mesh): one dependent load less than nbr -> child.
+// U + sgn G_a(U): what a neighbour on the -(sgn = +1) or +(sgn = -1) side of direction a adds to a cell (the algebra of
+// transport.cu: with phi = F/c the update is U' = U (1 - m nu/2) + (nu/2) sum_faces (U_n -/+ G_n) + (nu/2) sum_a p_a G_a(U),
+// m = faces that exist, p_a = (- face exists) - (+ face exists); m = 6, p = 0 for a cell with six regular faces)
+__device__ __forceinline__ float4 nb_term(const float4& U, float ca, float cb, int a, float sgn)
+{
+  const float pa = (a == 0) ? U.y : (a == 1) ? U.z : U.w;
+  const float u = fmaf(sgn * cb, pa, 1.f);
+  float4 r = make_float4(fmaf(sgn, pa, U.x), U.y * u, U.z * u, U.w * u);
+  if (a == 0) r.y = fmaf(sgn, ca, r.y); else if (a == 1) r.z = fmaf(sgn, ca, r.z); else r.w = fmaf(sgn, ca, r.w);
+  return r;
+}
+
+// 8 consecutive lanes hold one oct: across the three sibling faces each lane computes the term its partner needs
+// (U +/- G_a of its own state, with its own closure) and the two swap it with shfl.xor by 1, 2, 4: no load and no second
+// closure for half of the faces.  The three outer faces go through `nbo` (same-level neighbour oct, derived on the host
+// from the paper's neighbour-cell pointers for the static mesh): one dependent load less than nbr -> child.
 template <int G>
 __global__ void __launch_bounds__(128, 8)
 amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, double dV, Partial* __restrict__ parts)
@@ -151,33 +163,33 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     const long long cell = base + threadIdx.x;
     const bool valid = cell < ncell;                                 // uniform per 8-lane group
     const bool leaf = valid && !(child && child[cell] >= 0);
-    float4 Ui[G], ac[G];
+    float4 Ui[G], sum[G];
     float ai[G], bi[G];
 #pragma unroll
     for (int g = 0; g < G; g++) {
       Ui[g] = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
       closure_ab(Ui[g], ai[g], bi[g]);
-      ac[g] = Ui[g];
+      sum[g] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     const int k = (int)(cell & 7);
     const long long oct = cell >> 3;
+    int m = 0;                                                       // faces that exist
+    int pmask = 0;                                                   // 2 bits per direction: (- face exists) | (+ face exists) << 1
 #pragma unroll
     for (int a = 0; a < 3; a++) {
       const int bit = (k >> a) & 1;
-      // sibling face: side = 1 - bit
+      // sibling face (side 1 - bit): this lane is the partner's neighbour on side `bit`: it sends U - G (bit = 1) or U + G
       const bool sib_leaf = __shfl_xor_sync(0xffffffffu, leaf ? 1 : 0, 1 << a) != 0;
+      const float sg = bit ? -1.f : 1.f;
 #pragma unroll
       for (int g = 0; g < G; g++) {
-        float4 Us;
-        Us.x = __shfl_xor_sync(0xffffffffu, Ui[g].x, 1 << a); Us.y = __shfl_xor_sync(0xffffffffu, Ui[g].y, 1 << a);
-        Us.z = __shfl_xor_sync(0xffffffffu, Ui[g].z, 1 << a); Us.w = __shfl_xor_sync(0xffffffffu, Ui[g].w, 1 << a);
-        const float as = __shfl_xor_sync(0xffffffffu, ai[g], 1 << a), bs = __shfl_xor_sync(0xffffffffu, bi[g], 1 << a);
-        if (leaf && sib_leaf) {                                      // a split sibling: fed by the fine steps (Fig. 3 (iii))
-          const float4 d = face_change_pre(a, 1 - bit, Ui[g], ai[g], bi[g], Us, as, bs, nuh);
-          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
-        }
+        const float4 T = nb_term(Ui[g], ai[g], bi[g], a, sg);
+        const float tx = __shfl_xor_sync(0xffffffffu, T.x, 1 << a), ty = __shfl_xor_sync(0xffffffffu, T.y, 1 << a);
+        const float tz = __shfl_xor_sync(0xffffffffu, T.z, 1 << a), tw = __shfl_xor_sync(0xffffffffu, T.w, 1 << a);
+        if (sib_leaf) { sum[g].x += tx; sum[g].y += ty; sum[g].z += tz; sum[g].w += tw; }   // split sibling: Fig. 3 (iii)
       }
-      // outer face: side = bit
+      if (sib_leaf) { m++; pmask |= 1 << (2 * a + (1 - bit)); }
+      // outer face (side = bit)
       if (!leaf) continue;
       const int no = nbo[oct * 6 + 2 * a + bit];
       if (no == -1) continue;                                        // coarser leaf: amr_ghost_faces_kernel adds that face
@@ -186,20 +198,51 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
         if (child && child[nb] >= 0) continue;                       // split neighbour
 #pragma unroll
         for (int g = 0; g < G; g++) {
-          const float4 d = face_change(a, bit, Ui[g], ai[g], bi[g], Ul[(size_t)g * ncell + nb], nuh);
-          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+          const float4 Un = Ul[(size_t)g * ncell + nb];
+          float an, bn;
+          closure_ab(Un, an, bn);
+          const float4 T = nb_term(Un, an, bn, a, bit ? -1.f : 1.f);
+          sum[g].x += T.x; sum[g].y += T.y; sum[g].z += T.z; sum[g].w += T.w;
         }
       } else {                                                       // box face: -2 - bc
         const NbRef r = box_ghost(-2 - no, a, bit, l, cell);
 #pragma unroll
         for (int g = 0; g < G; g++) {
-          const float4 d = face_change(a, bit, Ui[g], ai[g], bi[g], nb_load(A, r, g, Ui[g]), nuh);
-          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
-          acc.outflow -= (double)d.x * dV;                           // A15: net N-flux through a box face
+          const float4 Un = nb_load(A, r, g, Ui[g]);
+          float an, bn;
+          closure_ab(Un, an, bn);
+          const float4 T = nb_term(Un, an, bn, a, bit ? -1.f : 1.f);
+          sum[g].x += T.x; sum[g].y += T.y; sum[g].z += T.z; sum[g].w += T.w;
+          // A15: N-flux through the box face, nu F^ = (nu/2) [(G_i + G_n) -/+ (U_n - U_i)]_N with G_N = phi_a
+          const float pi = (a == 0) ? Ui[g].y : (a == 1) ? Ui[g].z : Ui[g].w, pn = (a == 0) ? Un.y : (a == 1) ? Un.z : Un.w;
+          const float fl = bit ? nuh * ((pi + pn) - (Un.x - Ui[g].x)) : -nuh * ((pi + pn) - (Ui[g].x - Un.x));
+          acc.outflow += (double)fl * dV;
+        }
+      }
+      m++; pmask |= 1 << (2 * a + bit);
+    }
+    if (!leaf) continue;
+    const float own = fmaf(-nuh, (float)m, 1.f);
+    float4 ac[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      ac[g].x = fmaf(nuh, sum[g].x, own * Ui[g].x); ac[g].y = fmaf(nuh, sum[g].y, own * Ui[g].y);
+      ac[g].z = fmaf(nuh, sum[g].z, own * Ui[g].z); ac[g].w = fmaf(nuh, sum[g].w, own * Ui[g].w);
+    }
+    if (pmask != 63) {                                               // a missing face: the own flux does not cancel
+#pragma unroll
+      for (int a = 0; a < 3; a++) {
+        const int p = ((pmask >> (2 * a)) & 1) - ((pmask >> (2 * a + 1)) & 1);
+        if (p == 0) continue;
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 Gv = flux_vec(Ui[g], ai[g], bi[g], a);
+          const float w = nuh * (float)p;
+          ac[g].x = fmaf(w, Gv.x, ac[g].x); ac[g].y = fmaf(w, Gv.y, ac[g].y);
+          ac[g].z = fmaf(w, Gv.z, ac[g].z); ac[g].w = fmaf(w, Gv.w, ac[g].w);
         }
       }
     }
-    if (!leaf) continue;
     if (l < A.nl) {
 #pragma unroll
       for (int g = 0; g < G; g++) {
