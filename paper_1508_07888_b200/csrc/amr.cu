@@ -17,6 +17,10 @@
 #include "chem_math.cuh"
 #include "transport_math.cuh"
 
+#ifndef AMR_T_CTAS
+#define AMR_T_CTAS 6
+#endif
+
 namespace emma {
 namespace {
 
@@ -149,7 +153,7 @@ __device__ __forceinline__ float4 nb_term(const float4& U, float ca, float cb, i
 // closure for half of the faces.  The three outer faces go through `nbo` (same-level neighbour oct, derived on the host
 // from the paper's neighbour-cell pointers for the static mesh): one dependent load less than nbr -> child.
 template <int G>
-__global__ void __launch_bounds__(128, 8)
+__global__ void __launch_bounds__(128, AMR_T_CTAS)
 amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, double dV, Partial* __restrict__ parts)
 {
   Acc acc;
@@ -162,18 +166,44 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     const long long cell = base + threadIdx.x;
     const bool valid = cell < ncell;                                 // uniform per 8-lane group
     const bool leaf = valid && !(child && child[cell] >= 0);
+    // only leaves next to a split cell of their own level can have received deposits (bitmap built on the host); the
+    // deposit is requested together with the cell's own state so that its latency overlaps with the face work
+    const bool hd = leaf && l < A.nl && ((A.hasdep[l][cell >> 5] >> (cell & 31)) & 1u);
     float4 Ui[G], sum[G];
     float ai[G], bi[G];
 #pragma unroll
     for (int g = 0; g < G; g++) {
       Ui[g] = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
+      sum[g] = hd ? A.dep[l][(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int g = 0; g < G; g++) {
       closure_ab(Ui[g], ai[g], bi[g]);
-      sum[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+      // sum accumulates (U_n -/+ G_n) and is multiplied by nu/2 at the end: the deposit enters divided by nu/2
+      const float inv = 1.f / nuh;
+      sum[g].x *= inv; sum[g].y *= inv; sum[g].z *= inv; sum[g].w *= inv;
     }
     const int k = (int)(cell & 7);
     const long long oct = cell >> 3;
     int m = 0;                                                       // faces that exist
     int pmask = 0;                                                   // 2 bits per direction: (- face exists) | (+ face exists) << 1
+    // outer faces, indices first (all three pointer loads, then all three split tests, in flight together); a face that
+    // does not exist on this level reads the cell itself and is masked out, so the state loads below are branch-free
+    int no[3];
+    long long nb[3];
+    bool reg[3];
+#pragma unroll
+    for (int a = 0; a < 3; a++) no[a] = leaf ? nbo[oct * 6 + 2 * a + ((k >> a) & 1)] : -1;
+#pragma unroll
+    for (int a = 0; a < 3; a++) nb[a] = (no[a] >= 0) ? (((long long)no[a] << 3) | (k ^ (1 << a))) : (valid ? cell : 0);
+    int chn[3];
+#pragma unroll
+    for (int a = 0; a < 3; a++) chn[a] = (child && no[a] >= 0) ? child[nb[a]] : -1;
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      reg[a] = no[a] >= 0 && chn[a] < 0;                             // a leaf of this level behind the face
+      if (!reg[a]) nb[a] = valid ? cell : 0;
+    }
 #pragma unroll
     for (int a = 0; a < 3; a++) {
       const int bit = (k >> a) & 1;
@@ -188,37 +218,34 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
         if (sib_leaf) { sum[g].x += tx; sum[g].y += ty; sum[g].z += tz; sum[g].w += tw; }   // split sibling: Fig. 3 (iii)
       }
       if (sib_leaf) { m++; pmask |= 1 << (2 * a + (1 - bit)); }
-      // outer face (side = bit)
-      if (!leaf) continue;
-      const int no = nbo[oct * 6 + 2 * a + bit];
-      if (no == -1) continue;                                        // coarser leaf: amr_ghost_faces_kernel adds that face
-      if (no >= 0) {
-        const long long nb = ((long long)no << 3) | (k ^ (1 << a));
-        if (child && child[nb] >= 0) continue;                       // split neighbour
+      // outer face (side = bit): regular neighbour, branch-free
+      const float wgt = reg[a] ? 1.f : 0.f;
 #pragma unroll
-        for (int g = 0; g < G; g++) {
-          const float4 Un = Ul[(size_t)g * ncell + nb];
-          float an, bn;
-          closure_ab(Un, an, bn);
-          const float4 T = nb_term(Un, an, bn, a, bit ? -1.f : 1.f);
-          sum[g].x += T.x; sum[g].y += T.y; sum[g].z += T.z; sum[g].w += T.w;
-        }
-      } else {                                                       // box face: -2 - bc
-        const NbRef r = box_ghost(-2 - no, a, bit, l, cell);
+      for (int g = 0; g < G; g++) {
+        const float4 Un = Ul[(size_t)g * ncell + nb[a]];
+        float an, bn;
+        closure_ab(Un, an, bn);
+        const float4 T = nb_term(Un, an, bn, a, sg);
+        sum[g].x = fmaf(wgt, T.x, sum[g].x); sum[g].y = fmaf(wgt, T.y, sum[g].y);
+        sum[g].z = fmaf(wgt, T.z, sum[g].z); sum[g].w = fmaf(wgt, T.w, sum[g].w);
+      }
+      if (reg[a]) { m++; pmask |= 1 << (2 * a + bit); }
+      if (leaf && no[a] <= -2) {                                     // box face: -2 - bc (rare: the slow path)
+        const NbRef r = box_ghost(-2 - no[a], a, bit, l, cell);
 #pragma unroll
         for (int g = 0; g < G; g++) {
           const float4 Un = nb_load(A, r, g, Ui[g]);
           float an, bn;
           closure_ab(Un, an, bn);
-          const float4 T = nb_term(Un, an, bn, a, bit ? -1.f : 1.f);
+          const float4 T = nb_term(Un, an, bn, a, sg);
           sum[g].x += T.x; sum[g].y += T.y; sum[g].z += T.z; sum[g].w += T.w;
           // A15: N-flux through the box face, nu F^ = (nu/2) [(G_i + G_n) -/+ (U_n - U_i)]_N with G_N = phi_a
           const float pi = (a == 0) ? Ui[g].y : (a == 1) ? Ui[g].z : Ui[g].w, pn = (a == 0) ? Un.y : (a == 1) ? Un.z : Un.w;
           const float fl = bit ? nuh * ((pi + pn) - (Un.x - Ui[g].x)) : -nuh * ((pi + pn) - (Ui[g].x - Un.x));
           acc.outflow += (double)fl * dV;
         }
+        m++; pmask |= 1 << (2 * a + bit);
       }
-      m++; pmask |= 1 << (2 * a + bit);
     }
     if (!leaf) continue;
     const float own = fmaf(-nuh, (float)m, 1.f);
@@ -242,16 +269,9 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
         }
       }
     }
-    if (l < A.nl) {
+    if (hd) {
 #pragma unroll
-      for (int g = 0; g < G; g++) {
-        float4* dp = A.dep[l] + (size_t)g * ncell + cell;
-        const float4 d = *dp;
-        if (d.x != 0.f || d.y != 0.f || d.z != 0.f || d.w != 0.f) {
-          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
-          *dp = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-      }
+      for (int g = 0; g < G; g++) A.dep[l][(size_t)g * ncell + cell] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 #pragma unroll
     for (int g = 0; g < G; g++) Unew[(size_t)g * ncell + cell] = ac[g];
@@ -523,7 +543,7 @@ int grid_for(long long work, int block, int cap)
   if (b > cap) b = cap;
   return (int)b;
 }
-constexpr int AMR_GRID_CAP = 148 * 8;            // whole waves of 8 CTAs of 128 threads per SM; each block writes one Partial
+constexpr int AMR_GRID_CAP = 148 * 8;            // (the transport kernel uses 148 * AMR_T_CTAS)            // whole waves of 8 CTAs of 128 threads per SM; each block writes one Partial
 
 }  // namespace
 
@@ -538,7 +558,7 @@ constexpr int AMR_GRID_CAP = 148 * 8;            // whole waves of 8 CTAs of 128
 int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
                          cudaStream_t st)
 {
-  const int nb = grid_for(A.ncell[level], 128, AMR_GRID_CAP);
+  const int nb = grid_for(A.ncell[level], 128, 148 * AMR_T_CTAS);
   AMR_DISPATCH(A.G, (amr_transport_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts)));
   *n_parts = nb;
   return 1;

@@ -34,7 +34,7 @@ struct Layout {
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
   size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
-  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1];   // faces of refined leaves towards a coarser leaf
+  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1], ahasdep[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
 
@@ -111,6 +111,7 @@ void make_layout(const Shape& s, Layout& L)
         L.aslot_coarse[l] = take((size_t)s.nocts[l] * 24 * 4);
         L.aslot_face[l] = take((size_t)s.nocts[l] * 24);
         L.aslot_refs[l] = take((size_t)s.nocts[l] * 6 * 6 * 4);     // 6 neighbour references per oct side
+        L.ahasdep[l] = take((size_t)(s.ncell[l] + 31) / 32 * 4);
       }
       if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
     }
@@ -196,6 +197,7 @@ AmrDev amr_view(const emma_rt* h)
     A.child[l] = l == 0 ? (const int*)(h->arena + h->lay.achild0) : l < s.nl ? h->lv[l].child : nullptr;
     A.nbr[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbr[l]) : nullptr;
     A.nbo[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbo[l]) : nullptr;
+    A.hasdep[l] = (l >= 1 && l < s.nl) ? (const unsigned int*)(h->arena + h->lay.ahasdep[l]) : nullptr;
   }
   return A;
 }
@@ -335,6 +337,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
   std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1), slot_refs_h(s.nl + 1);
   std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
+  std::vector<std::vector<unsigned int>> hasdep_h(s.nl + 1);
   if (s.amr) {
     const int n = s.n;
     auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
@@ -389,6 +392,26 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
         nbo_h[l][i] = (l == 1) ? child0_h[pcell] : child_h[l - 1][pcell];  // oct of level l, or -1: coarser leaf
       }
       CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+    }
+    // leaves of a refined level that touch a split cell of the same level (they receive deposits)
+    for (int l = 1; l < s.nl; l++) {
+      hasdep_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
+      for (auto& kv : h->child_of[l]) {
+        const long long p = kv.first, po = p >> 3;
+        const int k = (int)(p & 7);
+        for (int a = 0; a < 3; a++)
+          for (int side = 0; side < 2; side++) {
+            long long q;
+            if (side != ((k >> a) & 1)) q = (po << 3) | (k ^ (1 << a));
+            else {
+              const int no = nbo_h[l][po * 6 + 2 * a + side];
+              if (no < 0) continue;
+              q = ((long long)no << 3) | (k ^ (1 << a));
+            }
+            if (child_h[l][q] < 0) hasdep_h[l][q >> 5] |= 1u << (q & 31);
+          }
+      }
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.ahasdep[l], hasdep_h[l].data(), hasdep_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
     }
     // faces of refined cells towards a coarser leaf: (fine cell, coarse leaf, face), 4 per oct face
     for (int l = 1; l <= s.nl; l++) {

@@ -221,6 +221,8 @@ struct AmrDev {
                                 // or -1 - bc for a non-periodic box face (levels >= 1)
   const int* nbo[MAXL + 1];     // [nocts][6] derived for the static mesh: the oct of the SAME level behind each face of the
                                 // oct, -1 if that side is a coarser leaf, -2 - bc for a non-periodic box face (levels >= 1)
+  const unsigned int* hasdep[MAXL + 1];   // bitmap over the cells of a level: a leaf with a split face neighbour of its own
+                                          // level, i.e. one that receives deposits (1 <= level < nl)
   float4 inflow[6][MAXG];
 };
 
