@@ -55,6 +55,8 @@ def _errors(orc, gpu, w, masks=None):
     for l in range(w.n_levels + 1):
         for g in range(w.G):
             Uo = orc.read(O.F_U, l, g)
+            if Uo.size == 0:
+                continue
             Ug = gpu.read(E.FIELD_U, l, g).astype(np.float64)
             sc = np.maximum(np.abs(Uo[:, 0]), max(1e-12 * np.abs(Uo[:, 0]).max(), 1e-300))
             rN = np.abs(Ug[:, 0] - Uo[:, 0]) / sc
@@ -158,3 +160,30 @@ def test_amr_refusals_and_io():
     with pytest.raises(E.EmmaRTError):
         crta.read(E.FIELD_U, 1, 0)
     crta.close()
+
+
+@pytest.mark.parametrize("case", ["empty_top_level", "four_groups", "fully_refined"])
+def test_amr_edge_cases(case):
+    """an empty refined level, the maximum group count, and a mesh whose level 0 has no leaves at all (every coarse cell
+    split: the fix list is empty, level 1 is all regular faces; pin M1's geometry)."""
+    rng = np.random.default_rng(17)
+    n = 8
+    if case == "empty_top_level":
+        w0 = make_amr_standard(n=n, G=1, levels=1, seed=3, thresh1=2.0)
+        w = tiny_workload(n, G=1, parent=[w0.parent[0], np.zeros(0, np.int64)], chemistry=0, L=w0.L)
+    elif case == "four_groups":
+        w0 = make_amr_standard(n=n, G=1, levels=2, seed=4, thresh1=2.0, thresh2=2.5)
+        assert len(w0.parent[1]) > 0
+        w = tiny_workload(n, G=4, parent=w0.parent, chemistry=0, L=w0.L, bc=(1, 2, 0, 0, 2, 1))
+    else:
+        w = tiny_workload(n, G=2, parent=[np.arange(n ** 3, dtype=np.int64)], chemistry=0)
+    U = _random_levels(rng, w)
+    orc, gpu = _pair(w, U, chemistry=0)
+    for step in range(2):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        eN, eF = _errors(orc, gpu, w)
+        assert eN <= TOL_NF and eF <= TOL_NF, (case, step, eN, eF)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+    gpu.close()
