@@ -187,3 +187,43 @@ def test_amr_edge_cases(case):
         assert eN <= TOL_NF and eF <= TOL_NF, (case, step, eN, eF)
         assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
     gpu.close()
+
+
+def test_amr_inflow_face_and_non_otsa_isothermal():
+    """(a) a plane-parallel flux entering through -x (reading A20) onto a refined mesh whose octs touch that face;
+    (b) chemistry in the isothermal test mode without OTSA (recombination radiation into group 1) on every level."""
+    n = 12
+    w0 = make_amr_standard(n=n, G=1, levels=2, seed=9, thresh1=2.0, thresh2=2.5)
+    co_x = np.asarray(w0.parent[0]) % n
+    assert (co_x == 0).any() and len(w0.parent[1]) > 0          # refined cells on the inflow face
+    # (a)
+    w = tiny_workload(n, G=2, parent=w0.parent, chemistry=0, L=w0.L, bc=(3, 1, 0, 0, 2, 2))
+    w.inflow = {(0, 0): (1e-4, 1e-4 * w.c_red, 0.0, 0.0), (0, 1): (3e-5, 3e-5 * w.c_red, 0.0, 0.0)}
+    orc, gpu = _pair(w, chemistry=0)
+    for step in range(6):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+    eN, eF = _errors(orc, gpu, w)
+    assert eN <= 3e-5 and eF <= 3e-5, (eN, eF)                  # six steps of 1e-5
+    assert do["photons_outflow"] < 0 and abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-5 * abs(do["photons_outflow"])
+    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-5)
+    gpu.close()
+    # (b)
+    w = make_amr_standard(n=n, G=3, levels=2, seed=9, thresh1=2.0, thresh2=2.5)
+    w.src_Q = w.src_Q * 300.0
+    w.T = [np.full(a.shape, 1.0e4, np.float32) for a in w.T]
+    orc, gpu = _pair(w, thermal=0, otsa=0)
+    prev = 0.0
+    for step in range(8):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        assert budget_residual(dg, prev) <= TOL_BUDGET, (step, dg)
+        prev = dg["photons_total"]
+    assert do["photons_recomb_emitted"] > 0
+    assert dg["photons_recomb_emitted"] == pytest.approx(do["photons_recomb_emitted"], rel=1e-4)
+    for l in range(3):
+        a, b = orc.read(O.F_X, l), gpu.read(E.FIELD_X, l).astype(np.float64)
+        assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, l
+    gpu.close()
