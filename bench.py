@@ -50,7 +50,7 @@ def ncu_traffic(kernel, n):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full summary
     (profiles/traffic.csv; captured at 512^3) -- None for any other grid size or if no capture is recorded."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
-    if n != 512 or not os.path.exists(p):
+    if n != (256 if kernel.startswith("amr_") else 512) or not os.path.exists(p):
         return None
     try:
         import csv
