@@ -7,6 +7,7 @@ M4  brute force: an independent dict-based transcription (tests/brute_amr.py) on
 M5  Fig. 6 call counts of the standard scheme: 4 coarse steps with 2 refined levels = 4 + 24 engine calls
 M6  a resolution jump of 2 across a face is refused
 M7  a beam crossing a refined slab keeps its photons and its speed
+M8  PAPER.md:556: the CRTA front follows the standard scheme's (static HII region with a refined shell)
 """
 import numpy as np
 import pytest
@@ -288,3 +289,49 @@ def test_M7_beam_through_a_refined_slab():
         U = o.read(oracle.F_U, l, 0)
         big = U[:, 0] > 1e-6
         np.testing.assert_allclose(U[big, 1], w.c_red * U[big, 0], rtol=1e-9)
+
+
+def test_M8_crta_front_follows_the_standard_scheme():
+    """PAPER.md:556 (Fig. 11-12): "the front position and velocities of the CRTA calculation follow the ones obtained from
+    the standard procedure".  Static cousin of that HII-region test (workloads.make_hii_region_corner: corner source,
+    reflective + transmissive faces, 3 groups) on a 16^3 base with the shell 1.5 <= r < 7 coarse cells refined once, so that
+    the front travels inside refined cells: the equivalent front radius (ionised volume of the leaves) of the oracle's CRTA
+    mode and of its standard AMR mode agree within 1 % at six epochs, and the standard front, transported on the fine
+    cells, is the sharper one."""
+    from workloads import make_hii_region_corner
+    n = 16
+    w = make_hii_region_corner(n=n)
+    ids = np.arange(n ** 3)
+    r = np.sqrt((ids % n + 0.5) ** 2 + ((ids // n) % n + 0.5) ** 2 + (ids // (n * n) + 0.5) ** 2)
+    p1 = ids[(r >= 1.5) & (r < 7.0)].astype(np.int64)
+    w.parent = [p1]
+    m = 8 * len(p1)
+    w.n0.append(np.full(m, 1e-3, np.float32))
+    w.x.append(np.full(m, 1.2e-3, np.float32))
+    w.T.append(np.full(m, 100.0, np.float32))
+
+    def run(standard):
+        o = oracle.Oracle(w)
+        if standard:
+            assert o.set_amr_transport(True) == oracle.OK
+        radii = []
+        for _ in range(6):
+            rc, _d = o.step(w.dt, 100)
+            assert rc == oracle.OK
+            vol = 0.0
+            for l in (0, 1):
+                x = o.read(oracle.F_X, l)
+                leaf = np.ones(len(x), bool)
+                if l == 0:
+                    leaf[p1] = False
+                vol += ((x[leaf] - 1.2e-3) / (1 - 1.2e-3)).sum() * (w.dx / 2 ** l) ** 3
+            radii.append((6.0 * vol / np.pi) ** (1.0 / 3.0) / w.dx)
+        return np.array(radii), o.read(oracle.F_X, 0).reshape(n, n, n)[0, 0, :]
+
+    r_crta, x_crta = run(False)
+    r_std, x_std = run(True)
+    assert 3.5 < r_std[-1] < 5.0                                  # the front is inside the refined shell
+    np.testing.assert_allclose(r_crta, r_std, rtol=1e-2)
+    assert np.all(np.diff(r_std) > 0)
+    ahead = slice(4, 8)                                           # just ahead of the x = 0.5 point
+    assert np.all(x_std[ahead] < x_crta[ahead])
