@@ -130,6 +130,32 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    if args.amr_standard:
+        # the oracle's standard-AMR mode (serial recursion) on the same recipe at 32^3 + 2 levels
+        import oracle as O
+        from workloads.amr import make_amr_standard
+        ws = make_amr_standard(n=32, G=3, levels=2)
+        orc = O.Oracle(ws)
+        assert orc.set_amr_transport(True) == O.OK
+        lc = [ws.n ** 3] + [8 * len(p) for p in ws.parent]
+        ll = [c - s_ for c, s_ in zip(lc, [len(p) for p in ws.parent] + [0])]
+        steps, warm = max(1, min(args.steps, 6)), min(args.warmup, 1)
+        if warm:
+            orc.step(ws.dt, warm)
+        t0 = time.perf_counter()
+        orc.step(ws.dt, steps)
+        secs = time.perf_counter() - t0
+        val = sum(ll[l] << l for l in range(3)) * 3 * steps / secs
+        sample = "standard-AMR recipe at 32^3 coarse + 2 levels x 3 groups, %d coarse steps, fp64 C oracle (serial recursion)" % steps
+        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+                "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "standard AMR scheme sampled at 32^3 + 2 levels (oracle on host cores)"},
+                "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line), flush=True)
+        return
     n = ORACLE_SAMPLE_N if args.config == 5 else 96
     steps, warm = max(1, min(args.steps, 5)), min(args.warmup, 1)
     # per "step" of this arm: one oracle step on the n^3 sample; the whole run stays within a few minutes

@@ -4,9 +4,12 @@
 // The host (api.cu) runs the recursion advance(l, dt) = [advance(l+1, dt/2) x 2] -> transport(l) -> chemistry(l) ->
 // restriction(l+1 -> l).  This file holds the kernels of one level:
 //   * amr_transport_kernel: Eq. 30 + 32 for the LEAF cells of a refined level, one thread per cell and all G groups.
-//     Neighbours are found through the oct structure the paper describes (each oct points to the 6 cells of
-//     the level below that surround its parent cell); siblings sit in the same 128-byte oct record.  A face towards a
-//     split cell computes nothing (the fine cells behind it deposit).
+//     Neighbours come from the oct structure the paper describes (each oct points to the 6 cells of the
+//     level below that surround its parent cell): the host keeps those pointers (`nbr`, also in the arena) and derives
+//     from them, once for the static mesh, what the kernels read: the same-level neighbour oct of every oct side (`nbo`),
+//     the list of faces towards a coarser leaf with their six resolved coarse references, the leaves that receive
+//     deposits.  Siblings sit in the same 128-byte oct record and are exchanged by warp shuffles.  A face towards a split
+//     cell computes nothing (the fine cells behind it deposit).
 //   * amr_ghost_faces_kernel: the faces towards a coarser leaf, one thread per face from a host-built list: MinMod-limited
 //     linear ghost, flux, the fine cell's change and the same flux / 8 deposited into that leaf (red.global.add.f32).
 //   * level 0 keeps the dense TMA kernel (transport_tma.cu) for the whole block; amr_fix0_kernel then recomputes the
@@ -55,29 +58,6 @@ __device__ NbRef nb_ref0(const AmrDev& A, long long cell, int a, int side)
   NbRef r;
   r.lvl = 0; r.cell = nb; r.flip = -1; r.face = 0;
   r.kind = (A.child[0] && A.child[0][nb] >= 0) ? 1 : 0;
-  return r;
-}
-
-// neighbour of a cell of level l >= 1 through the oct structure
-__device__ NbRef nb_ref(const AmrDev& A, int l, long long cell, int a, int side)
-{
-  if (l == 0) return nb_ref0(A, cell, a, side);
-  const long long oct = cell >> 3;
-  const int k = (int)(cell & 7);
-  const int bit = (k >> a) & 1;
-  NbRef r;
-  r.flip = -1; r.face = 0;
-  long long nb;
-  if (side != bit) nb = (oct << 3) | (k ^ (1 << a));               // sibling in the same oct
-  else {
-    const int p = A.nbr[l][oct * 6 + 2 * a + side];                 // cell of level l-1 next to the parent cell
-    if (p < 0) return box_ghost(-1 - p, a, side, l, cell);
-    const int ch = A.child[l - 1][p];
-    if (ch < 0) { r.kind = 2; r.lvl = l - 1; r.cell = p; return r; }
-    nb = ((long long)ch << 3) | (k ^ (1 << a));
-  }
-  r.lvl = l; r.cell = nb;
-  r.kind = (l < A.nl && A.child[l][nb] >= 0) ? 1 : 0;
   return r;
 }
 
