@@ -18,7 +18,7 @@ using namespace emma;
 namespace {
 
 constexpr size_t ALIGN = 256;
-constexpr int PART_SLOTS = 24576;
+constexpr int PART_SLOTS = 49152;        // a 3-level standard-AMR step: 14 refined sweeps x (888 + 1184) + level 0
 constexpr int TRANSPORT_MAX_BLOCKS = 8192;
 constexpr double E_HI_ERG = 13.6 * 1.602176634e-12;          // "E_13.6" of PAPER.md:266
 

@@ -227,3 +227,52 @@ def test_amr_inflow_face_and_non_otsa_isothermal():
         a, b = orc.read(O.F_X, l), gpu.read(E.FIELD_X, l).astype(np.float64)
         assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, l
     gpu.close()
+
+
+def _nested_cubes(n, boxes):
+    """parents of a mesh of nested cubes: boxes[l] = (lo, hi) in level-l cell coordinates of the cells split on level l."""
+    ids = np.arange(n ** 3)
+    coords = np.stack([ids % n, (ids // n) % n, ids // (n * n)], axis=1)
+    parents = []
+    for lo, hi in boxes:
+        sel = np.flatnonzero(np.all((coords >= lo) & (coords < hi), axis=1)).astype(np.int64)
+        parents.append(sel)
+        k = np.arange(8)
+        off = np.stack([k & 1, (k >> 1) & 1, (k >> 2) & 1], axis=1)
+        coords = (2 * coords[sel][:, None, :] + off[None, :, :]).reshape(-1, 3)
+    return parents
+
+
+def test_amr_three_refined_levels():
+    """the deepest hierarchy the mode accepts: 8^3 base, nested cubes of 216 / 512 / 1728 octs (15 level sweeps per step)."""
+    rng = np.random.default_rng(33)
+    n = 8
+    parents = _nested_cubes(n, [(1, 7), (4, 12), (10, 22)])
+    assert [len(p) for p in parents] == [216, 512, 1728]
+    w = tiny_workload(n, G=2, parent=parents, chemistry=0)
+    U = _random_levels(rng, w)
+    orc, gpu = _pair(w, U, chemistry=0)
+    for step in range(2):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        eN, eF = _errors(orc, gpu, w)
+        assert eN <= TOL_NF and eF <= TOL_NF, (step, eN, eF)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+    gpu.close()
+    # coupled on the same mesh: sources on the finest level, 4 coarse steps
+    w = tiny_workload(n, G=2, parent=parents, src_pos=np.array([[0.51, 0.52, 0.49], [0.47, 0.5, 0.55]]),
+                      src_Q=np.array([[3e47, 1e47], [2e47, 2e47]]))
+    orc, gpu = _pair(w)
+    prev = 0.0
+    for step in range(4):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        assert budget_residual(dg, prev) <= TOL_BUDGET
+        prev = dg["photons_total"]
+    assert orc.source_cell(0)[0] == 3
+    for l in range(4):
+        a, b = orc.read(O.F_X, l), gpu.read(E.FIELD_X, l).astype(np.float64)
+        assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, l
+    gpu.close()
