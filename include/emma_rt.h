@@ -103,8 +103,8 @@ typedef struct {
                                    Eq. 43-48 on the leaves of level l, then split cells := children mean.  Fluxes
                                    through a coarse-fine face are computed by the fine cells from a MinMod-limited
                                    linear ghost and deposited into the coarse leaf.  Needs face jumps <= 1 (else
-                                   EMMA_RT_EINVAL at init), <= 3 refined levels, the Eq. 32 flux; U0 is injected into
-                                   the refined cells at init; FIELD_U/N/F can then be read and U written on any level */
+                                   EMMA_RT_EINVAL at init), <= 3 refined levels; either interface flux
+                                   (emma_rt_set_flux); U0 is injected into the refined cells at init; FIELD_U/N/F can then be read and U written on any level */
   int32_t  reserved0;
 } emma_rt_config;
 

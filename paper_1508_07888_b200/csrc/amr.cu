@@ -18,6 +18,7 @@
 //   * amr_chem_kernel: Eq. 43-48 in place on the leaves of a refined level (chem_math.cuh, same arithmetic as CRTA's).
 //   * restriction, initial injection, sources with chemistry off, outflow of level 0.
 #include "chem_math.cuh"
+#include "hll_math.cuh"
 #include "transport_math.cuh"
 
 #ifndef AMR_T_CTAS
@@ -114,6 +115,95 @@ __device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui,
 __device__ __forceinline__ void red_add4(float4* p, const float4& v)
 {
   atomicAdd(p, v);                                                  // sm_90+: one 16-byte vector reduction (red.global.add.v4.f32)
+}
+
+// ---- HLL variant (reading A19) of the refined-level kernels: face by face, no cancellation algebra ------------------
+// change of the cell (state Ui) caused by the HLL flux through its face (a, side) towards state Un: -/+ nu H
+__device__ __forceinline__ float4 hll_change(int a, int side, const float4& Ui, const Aux& Xi, const float4& Un, const Aux& Xn, float nu)
+{
+  const float4& UL = side ? Ui : Un;
+  const float4& UR = side ? Un : Ui;
+  const Aux& XL = side ? Xi : Xn;
+  const Aux& XR = side ? Xn : Xi;
+  float4 H;
+  if (a == 0) H = hll_face<0>(UL, XL.a, XL.b, XL.lm[0], XL.lp[0], UR, XR.a, XR.b, XR.lm[0], XR.lp[0]);
+  else if (a == 1) H = hll_face<1>(UL, XL.a, XL.b, XL.lm[1], XL.lp[1], UR, XR.a, XR.b, XR.lm[1], XR.lp[1]);
+  else H = hll_face<2>(UL, XL.a, XL.b, XL.lm[2], XL.lp[2], UR, XR.a, XR.b, XR.lm[2], XR.lp[2]);
+  const float w = side ? -nu : nu;
+  return make_float4(w * H.x, w * H.y, w * H.z, w * H.w);
+}
+// A19: keep the state realizable, |phi| <= max(N, 0)
+__device__ __forceinline__ void realizable(float4& U)
+{
+  const float f2 = fmaf(U.y, U.y, fmaf(U.z, U.z, U.w * U.w));
+  const float lim = fmaxf(U.x, 0.f);
+  if (f2 > lim * lim) { const float s = lim * rsqrtf(f2); U.y *= s; U.z *= s; U.w *= s; }
+}
+
+// Eq. 30 with the HLL flux on the leaves of a refined level: the layout of amr_transport_kernel (8 lanes = one oct, sibling
+// states by shuffle, outer faces through nbo), every face evaluated explicitly.  The realizability limiter is applied by
+// the kernel that follows (chemistry or sources), after the ghost-face kernel has added its faces.
+template <int G>
+__global__ void __launch_bounds__(128)
+amr_transport_hll_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, double dV, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const float nu = 2.f * nuh;
+  const long long ncell = A.ncell[l];
+  const float4* __restrict__ Ul = A.U[l];
+  const int* __restrict__ child = (l < A.nl) ? A.child[l] : nullptr;
+  const int* __restrict__ nbo = A.nbo[l];
+  const long long span = (long long)gridDim.x * blockDim.x;
+  for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += span) {
+    const long long cell = base + threadIdx.x;
+    const bool valid = cell < ncell;
+    const bool leaf = valid && !(child && child[cell] >= 0);
+    const bool hd = leaf && l < A.nl && ((A.hasdep[l][cell >> 5] >> (cell & 31)) & 1u);
+    const int k = (int)(cell & 7);
+    const long long oct = cell >> 3;
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      const float4 Ui = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const Aux Xi = make_aux(Ui);
+      float4 ac = Ui;
+      if (hd) {
+        float4* dp = A.dep[l] + (size_t)g * ncell + cell;
+        const float4 d = *dp;
+        ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+        *dp = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int a = 0; a < 3; a++) {
+        const int bit = (k >> a) & 1;
+        const bool sib_leaf = __shfl_xor_sync(0xffffffffu, leaf ? 1 : 0, 1 << a) != 0;
+        float4 Us;
+        Us.x = __shfl_xor_sync(0xffffffffu, Ui.x, 1 << a); Us.y = __shfl_xor_sync(0xffffffffu, Ui.y, 1 << a);
+        Us.z = __shfl_xor_sync(0xffffffffu, Ui.z, 1 << a); Us.w = __shfl_xor_sync(0xffffffffu, Ui.w, 1 << a);
+        if (leaf && sib_leaf) {
+          const float4 d = hll_change(a, 1 - bit, Ui, Xi, Us, make_aux(Us), nu);
+          ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+        }
+        if (!leaf) continue;
+        const int no = nbo[oct * 6 + 2 * a + bit];
+        if (no == -1) continue;
+        float4 Un;
+        bool box = false;
+        if (no >= 0) {
+          const long long nb = ((long long)no << 3) | (k ^ (1 << a));
+          if (child && child[nb] >= 0) continue;
+          Un = Ul[(size_t)g * ncell + nb];
+        } else {
+          Un = nb_load(A, box_ghost(-2 - no, a, bit, l, cell), g, Ui);
+          box = true;
+        }
+        const float4 d = hll_change(a, bit, Ui, Xi, Un, make_aux(Un), nu);
+        ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+        if (box) acc.outflow -= (double)d.x * dV;
+      }
+      if (leaf) Unew[(size_t)g * ncell + cell] = ac;
+    }
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
 }
 
 // U + sgn G_a(U): what a neighbour on the -(sgn = +1) or +(sgn = -1) side of direction a adds to a cell (the algebra of
@@ -264,7 +354,7 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
 // (PAPER.md:436), the Eq. 32 flux, the fine cell's change (added to what amr_transport_kernel wrote) and the same
 // flux / 8 deposited into the coarse leaf (Fig. 3 (i)-(ii)).  Uniform work per thread: the irregular part of the
 // level is taken out of the per-cell kernel, where it made every warp on a patch boundary run the ghost code.
-template <int G>
+template <int G, bool HLL>
 __global__ void __launch_bounds__(128)
 amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, const int* __restrict__ slot_cell,
                        const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face,
@@ -310,9 +400,13 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
       Un.w = fmaf(sg, minmod(Uc.w - Um.w, Up.w - Uc.w), Un.w);
     }
     const float4 Ui = A.U[l][(size_t)g * ncell + cell];
-    float ai, bi;
-    closure_ab(Ui, ai, bi);
-    const float4 d = face_change(a, side, Ui, ai, bi, Un, nuh);
+    float4 d;
+    if (HLL) d = hll_change(a, side, Ui, make_aux(Ui), Un, make_aux(Un), 2.f * nuh);
+    else {
+      float ai, bi;
+      closure_ab(Ui, ai, bi);
+      d = face_change(a, side, Ui, ai, bi, Un, nuh);
+    }
     if (live) red_add4(Unew + (size_t)g * ncell + cell, d);         // a cell can have up to 3 such faces
     // the 4 faces of one oct side are 4 consecutive list entries (aligned lanes) and share the coarse leaf: one deposit
     float4 s4 = d;
@@ -329,7 +423,7 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
 template <int G>
 __global__ void __launch_bounds__(128, 8)
 amr_chem_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, const int* __restrict__ child,
-                int count_total, Partial* __restrict__ parts)
+                int count_total, int limit, Partial* __restrict__ parts)
 {
   Acc acc;
   const long long ncell = L.ncell;
@@ -337,6 +431,14 @@ amr_chem_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, c
     if (child && child[cell] >= 0) { if (cp.record) L.subc[cell] = 0; continue; }
     CellState<G> c;
     load_cell<G>(L, cell, U, ncell, cell, c);
+    if (limit) {                                                      // HLL (A19): the transported state is made realizable
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        float4 u = make_float4(c.N[g], c.px[g], c.py[g], c.pz[g]);
+        realizable(u);
+        c.px[g] = u.y; c.py[g] = u.z; c.pz[g] = u.w;
+      }
+    }
     CellTally tl;
     float rem = cp.dt, dmin = FINF;
     bool ok = true;
@@ -356,7 +458,7 @@ amr_chem_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, c
 template <int G>
 __global__ void __launch_bounds__(128)
 amr_sources_kernel(const LevelDev L, float4* __restrict__ U, const int* __restrict__ child, float dt, int count_total,
-                   Partial* __restrict__ parts)
+                   int limit, Partial* __restrict__ parts)
 {
   Acc acc;
   const long long ncell = L.ncell;
@@ -368,6 +470,7 @@ amr_sources_kernel(const LevelDev L, float4* __restrict__ U, const int* __restri
 #pragma unroll
     for (int g = 0; g < G; g++) {
       float4* p = U + (size_t)g * ncell + cell;
+      if (limit) { float4 u = *p; realizable(u); *p = u; }          // HLL (A19)
       if (S[g] != 0.f) {
         const float add = S[g] * dt;
         p->x += add;
@@ -429,7 +532,7 @@ __global__ void amr_inject_init_kernel(const LevelDev L, const float4* __restric
 // face, without the faces that look at a split cell (Fig. 3 (iii)), plus what the fine cells behind those faces
 // deposited during their two sub-steps.  Recomputed, not corrected: taking a large coarse flux back out of the dense
 // result would leave its rounding error on a possibly much smaller remainder.
-template <int G>
+template <int G, bool HLL>
 __global__ void __launch_bounds__(128)
 amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restrict__ Unew, const int* __restrict__ fix_cell,
                 const unsigned char* __restrict__ fix_mask, int n_fix, float nuh)
@@ -473,23 +576,34 @@ amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restr
     if (ghost[f] == EMMA_RT_BC_INFLOW) Un[f] = A.inflow[f][g];
     else if (ghost[f] == EMMA_RT_BC_REFLECTIVE) { if ((f >> 1) == 0) Un[f].y = -Un[f].y; else if ((f >> 1) == 1) Un[f].z = -Un[f].z; else Un[f].w = -Un[f].w; }
   }
-  float ai, bi;
-  closure_ab(Ui, ai, bi);
   float4 ac = Ui;
+  if (HLL) {
+    const Aux Xi = make_aux(Ui);
 #pragma unroll
-  for (int f = 0; f < 6; f++)
-    if (on[f]) {
-      const float4 d = face_change(f >> 1, f & 1, Ui, ai, bi, Un[f], nuh);
-      ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
-    }
+    for (int f = 0; f < 6; f++)
+      if (on[f]) {
+        const float4 d = hll_change(f >> 1, f & 1, Ui, Xi, Un[f], make_aux(Un[f]), 2.f * nuh);
+        ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+      }
+  } else {
+    float ai, bi;
+    closure_ab(Ui, ai, bi);
+#pragma unroll
+    for (int f = 0; f < 6; f++)
+      if (on[f]) {
+        const float4 d = face_change(f >> 1, f & 1, Ui, ai, bi, Un[f], nuh);
+        ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+      }
+  }
   ac.x += dpv.x; ac.y += dpv.y; ac.z += dpv.z; ac.w += dpv.w;
+  if (HLL) realizable(ac);                                            // A19, after the deposits
   *dp = make_float4(0.f, 0.f, 0.f, 0.f);
   Unew[(size_t)g * nc + cell] = ac;
 }
 
 // net N-flux through the non-periodic box faces of the level-0 LEAVES (the dense pass also counts split cells, whose
 // faces belong to their children here), from the old states
-template <int G>
+template <int G, bool HLL>
 __global__ void __launch_bounds__(128)
 amr_outflow0_kernel(const AmrDev A, const float4* __restrict__ Uold, float nuh, double dV, Partial* __restrict__ parts)
 {
@@ -507,9 +621,14 @@ amr_outflow0_kernel(const AmrDev A, const float4* __restrict__ Uold, float nuh, 
 #pragma unroll
     for (int g = 0; g < G; g++) {
       const float4 Ui = Uold[(size_t)g * nc + cell];
-      float ai, bi;
-      closure_ab(Ui, ai, bi);
-      const float4 d = face_change(a, side, Ui, ai, bi, nb_load(A, r, g, Ui), nuh);
+      const float4 Un = nb_load(A, r, g, Ui);
+      float4 d;
+      if (HLL) d = hll_change(a, side, Ui, make_aux(Ui), Un, make_aux(Un), 2.f * nuh);
+      else {
+        float ai, bi;
+        closure_ab(Ui, ai, bi);
+        d = face_change(a, side, Ui, ai, bi, Un, nuh);
+      }
       acc.outflow -= (double)d.x * dV;
     }
   }
@@ -535,40 +654,42 @@ constexpr int AMR_GRID_CAP = 148 * 8;            // (the transport kernel uses 1
     default: { constexpr int GG = 4; CALL; } break;             \
   }
 
-int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
+int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, int hll, Partial* parts, int* n_parts,
                          cudaStream_t st)
 {
   const int nb = grid_for(A.ncell[level], 128, 148 * AMR_T_CTAS);
-  AMR_DISPATCH(A.G, (amr_transport_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts)));
+  if (hll) { AMR_DISPATCH(A.G, (amr_transport_hll_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts))); }
+  else AMR_DISPATCH(A.G, (amr_transport_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, dV, parts)));
   *n_parts = nb;
   return 1;
 }
 
 int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
-                           const unsigned char* slot_face, const int* slot_refs, int n_slots, cudaStream_t st)
+                           const unsigned char* slot_face, const int* slot_refs, int n_slots, int hll, cudaStream_t st)
 {
   if (n_slots == 0) return 0;
   const int nb = (n_slots + 127) / 128;
-  AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots)));
+  if (hll) { AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, true><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots))); }
+  else AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, false><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots)));
   return 1;
 }
 
-int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, Partial* parts,
-                    int* n_parts, cudaStream_t st)
+int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, int limit,
+                    Partial* parts, int* n_parts, cudaStream_t st)
 {
   const int nb = grid_for(L.ncell, 128, AMR_GRID_CAP);
   const int* child = level < A.nl ? A.child[level] : nullptr;
-  AMR_DISPATCH(A.G, (amr_chem_kernel<GG><<<nb, 128, 0, st>>>(cp, L, A.U[level], child, count_total, parts)));
+  AMR_DISPATCH(A.G, (amr_chem_kernel<GG><<<nb, 128, 0, st>>>(cp, L, A.U[level], child, count_total, limit, parts)));
   *n_parts = nb;
   return 1;
 }
 
-int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, Partial* parts,
+int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, int limit, Partial* parts,
                        int* n_parts, cudaStream_t st)
 {
   const int nb = grid_for(L.ncell, 128, AMR_GRID_CAP);
   const int* child = level < A.nl ? A.child[level] : nullptr;
-  AMR_DISPATCH(A.G, (amr_sources_kernel<GG><<<nb, 128, 0, st>>>(L, A.U[level], child, dt, count_total, parts)));
+  AMR_DISPATCH(A.G, (amr_sources_kernel<GG><<<nb, 128, 0, st>>>(L, A.U[level], child, dt, count_total, limit, parts)));
   *n_parts = nb;
   return 1;
 }
@@ -591,19 +712,21 @@ int launch_amr_inject_init(const LevelDev& Lfine, const AmrDev& A, int level_fin
 }
 
 int launch_amr_fix0(const AmrDev& A, const float4* Uold, float4* Unew, const int* fix_cell, const unsigned char* fix_mask,
-                    int n_fix, float nuh, cudaStream_t st)
+                    int n_fix, float nuh, int hll, cudaStream_t st)
 {
   if (n_fix == 0) return 0;
   const int nb = (int)(((long long)n_fix * A.G + 127) / 128);
-  AMR_DISPATCH(A.G, (amr_fix0_kernel<GG><<<nb, 128, 0, st>>>(A, Uold, Unew, fix_cell, fix_mask, n_fix, nuh)));
+  if (hll) { AMR_DISPATCH(A.G, (amr_fix0_kernel<GG, true><<<nb, 128, 0, st>>>(A, Uold, Unew, fix_cell, fix_mask, n_fix, nuh))); }
+  else AMR_DISPATCH(A.G, (amr_fix0_kernel<GG, false><<<nb, 128, 0, st>>>(A, Uold, Unew, fix_cell, fix_mask, n_fix, nuh)));
   return 1;
 }
 
-int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, Partial* parts, int* n_parts,
+int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, int hll, Partial* parts, int* n_parts,
                         cudaStream_t st)
 {
   const int nb = grid_for(6LL * A.n * A.n, 128, 148 * 2);
-  AMR_DISPATCH(A.G, (amr_outflow0_kernel<GG><<<nb, 128, 0, st>>>(A, Uold, nuh, dV, parts)));
+  if (hll) { AMR_DISPATCH(A.G, (amr_outflow0_kernel<GG, true><<<nb, 128, 0, st>>>(A, Uold, nuh, dV, parts))); }
+  else AMR_DISPATCH(A.G, (amr_outflow0_kernel<GG, false><<<nb, 128, 0, st>>>(A, Uold, nuh, dV, parts)));
   *n_parts = nb;
   return 1;
 }

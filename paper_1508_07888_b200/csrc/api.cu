@@ -626,7 +626,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
 
   if (s.amr) {
     // standard AMR scheme (A21): advance(l, dt) = advance(l+1, dt/2) x 2 -> transport(l) -> chemistry(l) -> restrict(l+1 -> l)
-    if (hll) return fail(h, EMMA_RT_ESTATE, "amr_transport runs the Eq. 32 flux only");
+    const int ihll = hll ? 1 : 0;
     const float nuh = (float)(0.5 * (c * dt / h->dx));           // the same CFL number on every level
     tp.want_total = 0;
     bool open_faces = false;
@@ -654,7 +654,11 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           // dense pass over the whole block (its partials are not used: split cells must not count), then the
           // sparse correction of the leaves that touch a split cell
           h->prof.begin(EMMA_RT_K_TRANSPORT);
-          if (use_tma) {
+          if (hll) {
+            const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+            if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            h->launches += k;
+          } else if (use_tma) {
             const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
             if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
             h->launches += k;
@@ -662,9 +666,9 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           h->prof.end();
           AmrDev A = amr_view(h);
           h->prof.begin(EMMA_RT_K_OTHER);
-          if (open_faces) { h->launches += launch_amr_outflow0(A, h->U(h->cur), nuh, h->lv[0].dV, P + off, &np, h->st); off += np; }
+          if (open_faces) { h->launches += launch_amr_outflow0(A, h->U(h->cur), nuh, h->lv[0].dV, ihll, P + off, &np, h->st); off += np; }
           h->launches += launch_amr_fix0(A, h->U(h->cur), h->U(1 - h->cur), (const int*)(h->arena + h->lay.afix_cell),
-                                         (const unsigned char*)(h->arena + h->lay.afix_mask), h->n_fix, nuh, h->st);
+                                         (const unsigned char*)(h->arena + h->lay.afix_mask), h->n_fix, nuh, ihll, h->st);
           h->prof.end();
           h->cur = 1 - h->cur;
           if (h->cfg.chemistry) {
@@ -673,18 +677,18 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
             off += np;
           } else {
             h->prof.begin(EMMA_RT_K_OTHER);
-            h->launches += launch_amr_sources(h->lv[0], amr_view(h), 0, (float)dt, 1, P + off, &np, h->st);
+            h->launches += launch_amr_sources(h->lv[0], amr_view(h), 0, (float)dt, 1, 0, P + off, &np, h->st);
             h->prof.end();
             off += np;
           }
         } else {
           AmrDev A = amr_view(h);
           h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
-          h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, P + off, &np, h->st);
+          h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, ihll, P + off, &np, h->st);
           h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
                                                 (const int*)(h->arena + h->lay.aslot_coarse[l]),
                                                 (const unsigned char*)(h->arena + h->lay.aslot_face[l]),
-                                                (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], h->st);
+                                                (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], ihll, h->st);
           h->prof.end();
           off += np;
           h->acur[l] = 1 - h->acur[l];
@@ -692,8 +696,8 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           ChemParams cl_cp = cp;
           cl_cp.dt = (float)cl.dt;
           h->prof.begin(EMMA_RT_K_AMR_CHEM);
-          if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, P + off, &np, h->st);
-          else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, P + off, &np, h->st);
+          if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
+          else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
           h->prof.end();
           off += np;
         }
@@ -900,7 +904,6 @@ int emma_rt_set_flux(emma_rt* h, int32_t flux)
 {
   if (!h) return EMMA_RT_EINVAL;
   if (flux != EMMA_RT_FLUX_GLF && flux != EMMA_RT_FLUX_HLL) return fail(h, EMMA_RT_EINVAL, "unknown flux %d", (int)flux);
-  if (flux == EMMA_RT_FLUX_HLL && h->sh.amr) return fail(h, EMMA_RT_ESTATE, "amr_transport runs the Eq. 32 flux only");
   h->flux = flux;
   return EMMA_RT_OK;
 }

@@ -226,20 +226,20 @@ struct AmrDev {
   float4 inflow[6][MAXG];
 };
 
-int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, Partial* parts, int* n_parts,
+int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, int hll, Partial* parts, int* n_parts,
                          cudaStream_t st);
 int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
-                           const unsigned char* slot_face, const int* slot_refs, int n_slots, cudaStream_t st);
-int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, Partial* parts,
-                    int* n_parts, cudaStream_t st);
-int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, Partial* parts,
+                           const unsigned char* slot_face, const int* slot_refs, int n_slots, int hll, cudaStream_t st);
+int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, int limit,
+                    Partial* parts, int* n_parts, cudaStream_t st);
+int launch_amr_sources(const LevelDev& L, const AmrDev& A, int level, float dt, int count_total, int limit, Partial* parts,
                        int* n_parts, cudaStream_t st);
 int launch_amr_restrict(const LevelDev& Lfine, const LevelDev& Lcoarse, const AmrDev& A, int level_fine, int with_gas,
                         cudaStream_t st);
 int launch_amr_inject_init(const LevelDev& Lfine, const AmrDev& A, int level_fine, cudaStream_t st);
 int launch_amr_fix0(const AmrDev& A, const float4* Uold, float4* Unew, const int* fix_cell, const unsigned char* fix_mask,
-                    int n_fix, float nuh, cudaStream_t st);
-int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, Partial* parts, int* n_parts,
+                    int n_fix, float nuh, int hll, cudaStream_t st);
+int launch_amr_outflow0(const AmrDev& A, const float4* Uold, float nuh, double dV, int hll, Partial* parts, int* n_parts,
                         cudaStream_t st);
 
 }  // namespace emma

@@ -21,6 +21,7 @@
 #include "async_copy.cuh"
 #include "emma_rt_internal.cuh"
 #include "transport_math.cuh"
+#include "hll_math.cuh"
 
 namespace emma {
 
@@ -39,62 +40,10 @@ constexpr int AUXB = 2 * SG;                   // aux plane: two sub-planes of o
                                                // (consecutive lanes -> consecutive 16 B: no bank conflicts)
 constexpr size_t SMEM = (size_t)NST * SG + 2 * AUXB + 8 * (NST + 1);
 
-struct Aux {                                   // closure and wave speeds of one cell
-  float a, b;                                  // Pi = a I + b phi (x) phi
-  float lm[3], lp[3];                          // lmin, lmax per direction, in units of c
-};
-
-__device__ __forceinline__ Aux make_aux(const float4& U)
-{
-  Aux A;
-  const float rN = sel_ge(U.x, 1.1754944e-38f, frcp(U.x));           // A2: N <= 0 (or denormal) -> f = 0
-  float rx = U.y * rN, ry = U.z * rN, rz = U.w * rN;
-  const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
-  const float f2 = fminf(f2raw, 1.f);
-  const float xi = fsqrt(fmaf(-3.f, f2, 4.f));
-  const float i2 = frcp(2.f + xi);
-  const float q = f2 * i2;
-  A.a = fmaf(-U.x, q, 0.33333334f * U.x);
-  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
-  if (f2raw > 1.f) { const float s = rsqrtf(f2raw); rx *= s; ry *= s; rz *= s; }   // f clipped to 1: r -> unit vector
-  const float k = 2.f * (1.f - f2) * frcp(xi + 1.f), ixi = frcp(xi), t3 = 3.f * i2;
-  const float sx = fsqrt(fmaxf(k * fmaf(-t3 * rx, rx, xi), 0.f));
-  const float sy = fsqrt(fmaxf(k * fmaf(-t3 * ry, ry, xi), 0.f));
-  const float sz = fsqrt(fmaxf(k * fmaf(-t3 * rz, rz, xi), 0.f));
-  A.lm[0] = (rx - sx) * ixi; A.lp[0] = (rx + sx) * ixi;
-  A.lm[1] = (ry - sy) * ixi; A.lp[1] = (ry + sy) * ixi;
-  A.lm[2] = (rz - sz) * ixi; A.lp[2] = (rz + sz) * ixi;
-  return A;
-}
-
 __device__ __forceinline__ void store_aux(unsigned char* plane, int off, const Aux& A)
 {
   *(float4*)(plane + off) = make_float4(A.a, A.b, A.lm[0], A.lp[0]);
   *(float4*)(plane + SG + off) = make_float4(A.lm[1], A.lp[1], A.lm[2], A.lp[2]);
-}
-
-// flux vector G_d of a cell and the HLL combination for the face between L (towards -d) and R (towards +d)
-template <int D>
-__device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL, float lmL, float lpL,
-                                           const float4& UR, float aR, float bR, float lmR, float lpR)
-{
-  const float pL = comp<D>(UL), pR = comp<D>(UR);
-  const float uL = bL * pL, uR = bR * pR;
-  float4 GL = make_float4(pL, uL * UL.y, uL * UL.z, uL * UL.w);
-  float4 GR = make_float4(pR, uR * UR.y, uR * UR.z, uR * UR.w);
-  if (D == 0) { GL.y += aL; GR.y += aR; } else if (D == 1) { GL.z += aL; GR.z += aR; } else { GL.w += aL; GR.w += aR; }
-  const float lp = fmaxf(0.f, fmaxf(lpL, lpR)), lm = fminf(0.f, fminf(lmL, lmR));
-  const float den = lp - lm;
-  // l+ = l- = 0 (both cells stream exactly along the face): G vanishes there too and H = 0.  The guard also covers a
-  // denormal den (transverse speeds of ~1e-38 from rounding dust in phi), whose approximate reciprocal is inf
-  const float inv = (den > 1e-20f) ? frcp(den) : 0.f;
-  const float wl = lp * inv, wr = -lm * inv, wd = lp * lm * inv;
-  float4 H;
-  H.x = fmaf(wl, GL.x, fmaf(wr, GR.x, wd * (UR.x - UL.x)));
-  H.y = fmaf(wl, GL.y, fmaf(wr, GR.y, wd * (UR.y - UL.y)));
-  H.z = fmaf(wl, GL.z, fmaf(wr, GR.z, wd * (UR.z - UL.z)));
-  H.w = fmaf(wl, GL.w, fmaf(wr, GR.w, wd * (UR.w - UL.w)));
-  return H;
 }
 
 // DIAG: chemistry is off, so this pass owns the step's photon total and non-finite scan.

@@ -3,7 +3,8 @@ the fp64 oracle, element by element on every level.
 
 The oracle's scheme is pinned on the CPU (tests/test_oracle_amr.py M1-M7).  Here: transport alone from random states on
 jump-balanced 1- and 2-level meshes (periodic and open/reflective boxes, G = 1..3), the coupled step with sources and
-chemistry over several coarse steps, the photon budget, the refusals (face jump > 1, HLL), field I/O on refined levels.
+chemistry over several coarse steps, the photon budget, the refusal of a face jump > 1, field I/O on refined levels, and
+the same with the HLL interface flux (reading A19) on every level.
 """
 import numpy as np
 import pytest
@@ -36,10 +37,10 @@ def _random_levels(rng, w, fmax=0.8, lo=-6, hi=-3):
     return out
 
 
-def _pair(w, U=None, **kw):
-    orc = O.Oracle(w, **kw)
+def _pair(w, U=None, flux=None, **kw):
+    orc = O.Oracle(w, flux=flux, **kw)
     assert orc.set_amr_transport(True) == O.OK
-    gpu = E.EmmaRT(w, record_subcycles=1, amr_transport=1, **kw)
+    gpu = E.EmmaRT(w, record_subcycles=1, amr_transport=1, flux=flux, **kw)
     if U is not None:
         for l in range(w.n_levels + 1):
             for g in range(w.G):
@@ -149,7 +150,8 @@ def test_amr_refusals_and_io():
     assert ei.value.code == E.EINVAL
     w = make_amr_standard(n=8, G=1, levels=1, thresh1=2.0)
     gpu = E.EmmaRT(w, amr_transport=1)
-    assert E.lib().emma_rt_set_flux(gpu.h, E.FLUX_HLL) == E.ESTATE
+    assert E.lib().emma_rt_set_flux(gpu.h, E.FLUX_HLL) == E.OK        # both fluxes run in this mode
+    assert E.lib().emma_rt_set_flux(gpu.h, E.FLUX_GLF) == E.OK
     m = gpu.level_cells(1)
     U = np.arange(4 * m, dtype=np.float32).reshape(m, 4)
     assert gpu.write(E.FIELD_U, 1, 0, U) == E.OK
@@ -275,4 +277,53 @@ def test_amr_three_refined_levels():
     for l in range(4):
         a, b = orc.read(O.F_X, l), gpu.read(E.FIELD_X, l).astype(np.float64)
         assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, l
+    gpu.close()
+
+
+@pytest.mark.parametrize("n,G,levels,bc", [(16, 1, 2, (0,) * 6), (12, 3, 2, (1, 1, 2, 1, 0, 0)), (10, 2, 1, (2, 2, 1, 1, 1, 2))])
+def test_amr_hll_transport(n, G, levels, bc):
+    """the HLL flux (A19) on every level of the standard AMR scheme: dense HLL kernel + recomputed fix cells on level 0,
+    explicit faces on the refined levels, the realizability limiter after the deposits."""
+    rng = np.random.default_rng(7 * n + G)
+    w0 = make_amr_standard(n=n, G=1, levels=levels, seed=50 + n, thresh1=2.0, thresh2=2.5)
+    assert 0 < len(w0.parent[0]) < n ** 3 and (levels == 1 or len(w0.parent[1]) > 0)
+    w = tiny_workload(n, G=G, parent=w0.parent, chemistry=0, bc=bc, L=w0.L)
+    U = _random_levels(rng, w, fmax=0.9)
+    orc, gpu = _pair(w, U, flux=E.FLUX_HLL, chemistry=0)
+    for step in range(2):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        eN, eF = _errors(orc, gpu, w)
+        assert eN <= TOL_NF and eF <= 2 * TOL_NF, (step, eN, eF)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+        assert abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-6 * do["photons_total"]
+    gpu.close()
+
+
+def test_amr_hll_coupled_steps():
+    n, n_steps = 12, 8
+    w = make_amr_standard(n=n, G=3, levels=2, seed=31, thresh1=2.0, thresh2=2.5)
+    w.src_Q = w.src_Q * 300.0
+    orc, gpu = _pair(w, flux=E.FLUX_HLL)
+    flips, prev = [], 0.0
+    anc = coarse_ancestors(w)
+    for step in range(1, n_steps + 1):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        assert budget_residual(dg, prev) <= TOL_BUDGET, (step, dg)
+        prev = dg["photons_total"]
+        for l in range(w.n_levels + 1):
+            so = orc.read(O.F_SUBCYCLES, l).astype(np.int64)
+            sg = gpu.read(E.FIELD_SUBCYCLES, l).astype(np.int64)
+            for c in np.flatnonzero(so != sg):
+                flips.append((step, l, int(c), int(anc[l][c])))
+    masks = clean_masks(w, flips, n_steps)
+    assert sum((~m).sum() for m in masks) / sum(m.size for m in masks) <= 0.05, len(flips)
+    for name, fo, fg in (("x", O.F_X, E.FIELD_X), ("T", O.F_T, E.FIELD_T)):
+        for l in range(w.n_levels + 1):
+            a = orc.read(fo, l)[masks[l]]
+            b = gpu.read(fg, l).astype(np.float64)[masks[l]]
+            assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, (name, l)
     gpu.close()
