@@ -191,7 +191,8 @@ def test_amr_edge_cases(case):
     gpu.close()
 
 
-def test_amr_inflow_face_and_non_otsa_isothermal():
+@pytest.mark.parametrize("flux", [E.FLUX_GLF, E.FLUX_HLL])
+def test_amr_inflow_face_and_non_otsa_isothermal(flux):
     """(a) a plane-parallel flux entering through -x (reading A20) onto a refined mesh whose octs touch that face;
     (b) chemistry in the isothermal test mode without OTSA (recombination radiation into group 1) on every level."""
     n = 12
@@ -201,13 +202,23 @@ def test_amr_inflow_face_and_non_otsa_isothermal():
     # (a)
     w = tiny_workload(n, G=2, parent=w0.parent, chemistry=0, L=w0.L, bc=(3, 1, 0, 0, 2, 2))
     w.inflow = {(0, 0): (1e-4, 1e-4 * w.c_red, 0.0, 0.0), (0, 1): (3e-5, 3e-5 * w.c_red, 0.0, 0.0)}
-    orc, gpu = _pair(w, chemistry=0)
+    orc, gpu = _pair(w, flux=flux, chemistry=0)
     for step in range(6):
         rco, do = orc.step(w.dt, 1)
         rcg, dg = gpu.step(w.dt, 1)
         assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
-    eN, eF = _errors(orc, gpu, w)
-    assert eN <= 3e-5 and eF <= 3e-5, (eN, eF)                  # six steps of 1e-5
+    if flux == E.FLUX_GLF:
+        eN, eF = _errors(orc, gpu, w)
+        assert eN <= 3e-5 and eF <= 3e-5, (eN, eF)              # six steps of 1e-5
+    else:
+        # a beam at f = 1 exactly: the HLL transverse speeds c sqrt(2 (1 - f^2)) are sqrt-sensitive to what fp32 resolves of
+        # 1 - f^2 (DESIGN.md 5.6 / tests/test_inflow_shadow.py), so light that leaks sideways at a resolution jump cannot
+        # agree cell by cell between precisions: the difference is bounded relative to the beam instead (measured 1.1e-4)
+        for l in range(w.n_levels + 1):
+            for g in range(w.G):
+                Uo, Ug = orc.read(O.F_U, l, g), gpu.read(E.FIELD_U, l, g).astype(np.float64)
+                assert np.abs(Ug[:, 0] - Uo[:, 0]).max() <= 5e-4 * np.abs(Uo[:, 0]).max(), (l, g)
+                assert np.abs(Ug[:, 1:] - Uo[:, 1:]).max() <= 5e-4 * w.c_red * np.abs(Uo[:, 0]).max(), (l, g)
     assert do["photons_outflow"] < 0 and abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-5 * abs(do["photons_outflow"])
     assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-5)
     gpu.close()
@@ -215,7 +226,7 @@ def test_amr_inflow_face_and_non_otsa_isothermal():
     w = make_amr_standard(n=n, G=3, levels=2, seed=9, thresh1=2.0, thresh2=2.5)
     w.src_Q = w.src_Q * 300.0
     w.T = [np.full(a.shape, 1.0e4, np.float32) for a in w.T]
-    orc, gpu = _pair(w, thermal=0, otsa=0)
+    orc, gpu = _pair(w, flux=flux, thermal=0, otsa=0)
     prev = 0.0
     for step in range(8):
         rco, do = orc.step(w.dt, 1)
