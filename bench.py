@@ -232,7 +232,8 @@ def run_ours(args):
     log("[bench] rank %d: generated %s in %.1f s" % (rank, w.name, time.time() - t0))
 
     amr = 1 if args.amr_standard else 0
-    gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr)
+    flux = E.FLUX_HLL if args.hll else None
+    gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr, flux=flux)
     dt = w.dt
     units_per_step = leaf_count(w) * G            # config 5: n^3 G; config 4: leaf cells x G
     lv_cells = [n ** 3] + [8 * len(p) for p in w.parent]
@@ -325,7 +326,7 @@ def run_ours(args):
         hll["frac"] = hll["GBps"] / peak
         g3.close()
         torch.cuda.empty_cache()
-        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr)
+        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr, flux=flux)
 
     # ---------------- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
     Ke = max(1, min(K, args.e2e_steps))
@@ -397,7 +398,8 @@ def run_ours(args):
                            ("BASELINE config 4: %d^3 coarse + 2 refined levels (CRTA), %d groups, lognormal sigma_ln=1.5, "
                             "%d leaves, %d sources; value counts leaf-cell-group updates" % (n, G, leaf_count(w), len(w.src_pos))),
                            "n_coarse": n, "groups": G, "cells": ncell, "dt_s": dt, "l2": "inputs_exceed_l2",
-                           "schedule": "unfused" if args.unfused else "fused",
+                           "schedule": "unfused" if (args.unfused or args.hll or amr) else "fused",
+                           "flux": "hll" if args.hll else "glf",
                            "parallelism": "replicas" if world > 1 else "single"},
                 "roofline": roofline, "kernels": kern, "transport_only": tr, "transport_only_hll": hll, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": int(launches), "clocks": clk,
@@ -419,6 +421,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[4, 5], help="BASELINE config: 5 (default, the metric's) or 4 (CRTA)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--unfused", action="store_true", help="separate transport and chemistry passes")
+    ap.add_argument("--hll", action="store_true", help="coupled step with the HLL interface flux (two-pass schedule)")
     ap.add_argument("--amr-standard", action="store_true",
                     help="the standard (non-CRTA) AMR scheme on a jump-balanced 256^3 + 2 levels mesh (SURVEY 8f NEXT-2)")
     ap.add_argument("--skip-transport-only", action="store_true")
