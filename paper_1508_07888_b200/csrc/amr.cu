@@ -446,7 +446,7 @@ amr_chem_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, c
     if (!ok) acc.err |= 1u;
     store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
     const double before = acc.total;
-    fold(acc, tl, c.N, G, L.dV);
+    fold(acc, tl, c.N, G, L.dV, L.dV_total);
     if (!count_total) acc.total = before;                            // photons are counted once per coarse step
     acc.dtau_min = fminf(acc.dtau_min, dmin);
     if (!finite_cell<G>(c)) acc.nonfinite++;

@@ -34,7 +34,7 @@ struct Layout {
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
   size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
-  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1], ahasdep[MAXL + 1];   // faces of refined leaves towards a coarser leaf
+  size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1], ahasdep[MAXL + 1], arefined[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
 
@@ -96,7 +96,9 @@ void make_layout(const Shape& s, Layout& L)
     }
   }
   L.refined0 = s.nl > 0 ? take((size_t)(s.ncell[0] + 31) / 32 * 4) : 0;
-  L.queue = s.need_queue ? take(s.ncell[0] * 4) : 0;
+  long long qcells = s.ncell[0];
+  if (s.amr) for (int l = 1; l <= s.nl; l++) qcells = std::max(qcells, s.ncell[l]);   // every level runs the two-pass chemistry
+  L.queue = s.need_queue ? take(qcells * 4) : 0;
   L.qcount = take(256);
   L.parts = take((size_t)PART_SLOTS * sizeof(Partial));
   L.diag = take(sizeof(DiagDev));
@@ -112,6 +114,7 @@ void make_layout(const Shape& s, Layout& L)
         L.aslot_face[l] = take((size_t)s.nocts[l] * 24);
         L.aslot_refs[l] = take((size_t)s.nocts[l] * 6 * 6 * 4);     // 6 neighbour references per oct side
         L.ahasdep[l] = take((size_t)(s.ncell[l] + 31) / 32 * 4);
+        L.arefined[l] = take((size_t)(s.ncell[l] + 31) / 32 * 4);     // split cells of the level (chemistry skips them)
       }
       if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
     }
@@ -180,6 +183,14 @@ int fail(emma_rt* h, int code, const char* fmt, ...)
     cudaError_t e__ = (call);                                                                   \
     if (e__ != cudaSuccess) return fail(h, EMMA_RT_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
   } while (0)
+
+// chem_level0 opens its own profiler spans; inside an AMR sweep the outer AMR_CHEM span already covers it
+Profiler* nullptr_prof(emma_rt* h)
+{
+  static thread_local Profiler off;            // on = false: begin/end do nothing
+  (void)h;
+  return &off;
+}
 
 // device view of the hierarchy in AMR-transport mode, with the buffers that are current right now
 AmrDev amr_view(const emma_rt* h)
@@ -308,6 +319,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     L.n_src = 0;
     const double dxl = h->dx / (double)(1 << l);
     L.dV = dxl * dxl * dxl;
+    L.dV_total = L.dV;
     if (l >= 1) {
       L.parent = (int*)(h->arena + h->lay.parent[l]);
       L.anc0 = (int*)(h->arena + h->lay.anc0[l]);
@@ -337,7 +349,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
   std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1), slot_refs_h(s.nl + 1);
   std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
-  std::vector<std::vector<unsigned int>> hasdep_h(s.nl + 1);
+  std::vector<std::vector<unsigned int>> hasdep_h(s.nl + 1), refined_lv_h(s.nl + 1);
   if (s.amr) {
     const int n = s.n;
     auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
@@ -395,6 +407,9 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     }
     // leaves of a refined level that touch a split cell of the same level (they receive deposits)
     for (int l = 1; l < s.nl; l++) {
+      refined_lv_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
+      for (auto& kv : h->child_of[l]) refined_lv_h[l][kv.first >> 5] |= 1u << (kv.first & 31);
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.arefined[l], refined_lv_h[l].data(), refined_lv_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
       hasdep_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
       for (auto& kv : h->child_of[l]) {
         const long long p = kv.first, po = p >> 3;
@@ -696,7 +711,15 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
           ChemParams cl_cp = cp;
           cl_cp.dt = (float)cl.dt;
           h->prof.begin(EMMA_RT_K_AMR_CHEM);
-          if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
+          if (h->cfg.chemistry && !hll) {
+            // the two-pass chemistry of level 0 (bulk-async main pass + compacted tail, chemistry.cu) on this level's arrays
+            LevelDev Lc = h->lv[l];
+            Lc.refined = l < s.nl ? (unsigned int*)(h->arena + h->lay.arefined[l]) : nullptr;
+            Lc.dV_total = cl.last ? Lc.dV : 0.0;
+            h->launches += launch_chem_level0(cl_cp, Lc, h->Ulev(l), s.ncell[l], (int*)(h->arena + h->lay.queue), h->qcount(),
+                                              P + off, &np, h->sm_count, h->st, nullptr_prof(h));
+            CUDA_TRY(h, cudaMemsetAsync(h->qcount(), 0, 8, h->st));      // queue counters of the next sweep
+          } else if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
           else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
           h->prof.end();
           off += np;

@@ -161,7 +161,9 @@ __device__ __forceinline__ bool substep(const ChemParams& cp, CellState<G>& c, f
   return true;
 }
 
-__device__ __forceinline__ void fold(Acc& a, const CellTally& tl, const float* N, int G, double dV)
+// dV_total: the volume used for the photon total (= dV, or 0 when this sweep is not the one that counts the photons of its
+// level: a refined level of the standard AMR scheme is swept 2^l times per coarse step)
+__device__ __forceinline__ void fold(Acc& a, const CellTally& tl, const float* N, int G, double dV, double dV_total)
 {
   a.absorbed += (double)tl.absorbed * dV;
   a.injected += (double)tl.injected * dV;
@@ -170,7 +172,7 @@ __device__ __forceinline__ void fold(Acc& a, const CellTally& tl, const float* N
   a.nsub_max = max(a.nsub_max, tl.nsub);
   float s = 0.f;
   for (int g = 0; g < G; g++) s += N[g];
-  a.total += (double)s * dV;
+  a.total += (double)s * dV_total;
 }
 
 template <int G>

@@ -74,7 +74,7 @@ chem_main_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, 
         c.x = x1; c.y = y1; c.eps = eps1;
         tl.nsub = 1;
         store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
-        fold(acc, tl, c.N, G, L.dV);
+        fold(acc, tl, c.N, G, L.dV, L.dV_total);
         acc.dtau_min = fminf(acc.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc.nonfinite++;
       } else {
@@ -228,7 +228,7 @@ chem_main_bulk_kernel(const ChemParams cp, const LevelDev L, float4* __restrict_
         c.x = x1; c.y = y1; c.eps = eps1;
         tl.nsub = 1;
         store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
-        fold(acc, tl, c.N, G, L.dV);
+        fold(acc, tl, c.N, G, L.dV, L.dV_total);
         acc.dtau_min = fminf(acc.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc.nonfinite++;
       } else {
@@ -295,7 +295,7 @@ chem_tail_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, 
       if (!ok) acc.err |= 1u;
       if (!ok || rem <= 0.f) {
         store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
-        fold(acc, tl, c.N, G, L.dV);
+        fold(acc, tl, c.N, G, L.dV, L.dV_total);
         acc.dtau_min = fminf(acc.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc.nonfinite++;
         has = false;
@@ -349,7 +349,7 @@ chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow
         L.xs[cell] = encode_x(c.x, c.y);
         L.eps[cell] = c.eps;
         if (cp.record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
-        fold(acc, tl, c.N, G, L.dV);
+        fold(acc, tl, c.N, G, L.dV, L.dV_total);
         acc.dtau_min = fminf(acc.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc.nonfinite++;
       } else {

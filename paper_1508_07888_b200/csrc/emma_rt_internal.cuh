@@ -63,6 +63,7 @@ struct LevelDev {
   float* src_S;            // [n_src][G] photons cm^-3 s^-1
   int n_src;
   double dV;               // cell volume [cm^3]
+  double dV_total;         // = dV; 0 for a sweep that must not add to the photon total (see fold())
 };
 
 struct TransportParams {

@@ -305,7 +305,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
         c.x = x1; c.y = y1; c.eps = eps1;
         tl.nsub = 1;
         store_cell<G>(L, (long long)cell, Uout, (long long)ncell, c, tl, cp.record);
-        fold(acc_d, tl, c.N, G, L.dV);
+        fold(acc_d, tl, c.N, G, L.dV, L.dV_total);
         acc_d.dtau_min = fminf(acc_d.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc_d.nonfinite++;
       } else {
