@@ -119,16 +119,16 @@ __device__ __forceinline__ void red_add4(float4* p, const float4& v)
 
 // ---- HLL variant (reading A19) of the refined-level kernels: face by face, no cancellation algebra ------------------
 // change of the cell (state Ui) caused by the HLL flux through its face (a, side) towards state Un: -/+ nu H
-__device__ __forceinline__ float4 hll_change(int a, int side, const float4& Ui, const Aux& Xi, const float4& Un, const Aux& Xn, float nu)
+__device__ __forceinline__ float4 hll_change(int a, int side, const float4& Ui, const AuxD& Xi, const float4& Un, const AuxD& Xn, float nu)
 {
   const float4& UL = side ? Ui : Un;
   const float4& UR = side ? Un : Ui;
-  const Aux& XL = side ? Xi : Xn;
-  const Aux& XR = side ? Xn : Xi;
+  const AuxD& XL = side ? Xi : Xn;
+  const AuxD& XR = side ? Xn : Xi;
   float4 H;
-  if (a == 0) H = hll_face<0>(UL, XL.a, XL.b, XL.lm[0], XL.lp[0], UR, XR.a, XR.b, XR.lm[0], XR.lp[0]);
-  else if (a == 1) H = hll_face<1>(UL, XL.a, XL.b, XL.lm[1], XL.lp[1], UR, XR.a, XR.b, XR.lm[1], XR.lp[1]);
-  else H = hll_face<2>(UL, XL.a, XL.b, XL.lm[2], XL.lp[2], UR, XR.a, XR.b, XR.lm[2], XR.lp[2]);
+  if (a == 0) H = hll_face<0>(UL, XL.a, XL.b, XL.lm, XL.lp, UR, XR.a, XR.b, XR.lm, XR.lp);
+  else if (a == 1) H = hll_face<1>(UL, XL.a, XL.b, XL.lm, XL.lp, UR, XR.a, XR.b, XR.lm, XR.lp);
+  else H = hll_face<2>(UL, XL.a, XL.b, XL.lm, XL.lp, UR, XR.a, XR.b, XR.lm, XR.lp);
   const float w = side ? -nu : nu;
   return make_float4(w * H.x, w * H.y, w * H.z, w * H.w);
 }
@@ -179,8 +179,12 @@ amr_transport_hll_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ 
         float4 Us;
         Us.x = __shfl_xor_sync(0xffffffffu, Ui.x, 1 << a); Us.y = __shfl_xor_sync(0xffffffffu, Ui.y, 1 << a);
         Us.z = __shfl_xor_sync(0xffffffffu, Ui.z, 1 << a); Us.w = __shfl_xor_sync(0xffffffffu, Ui.w, 1 << a);
+        const AuxD Xa = aux_dir(Xi, a);
+        AuxD Xs;                                                       // the sibling's closure and speeds along a, from its lane
+        Xs.a = __shfl_xor_sync(0xffffffffu, Xa.a, 1 << a); Xs.b = __shfl_xor_sync(0xffffffffu, Xa.b, 1 << a);
+        Xs.lm = __shfl_xor_sync(0xffffffffu, Xa.lm, 1 << a); Xs.lp = __shfl_xor_sync(0xffffffffu, Xa.lp, 1 << a);
         if (leaf && sib_leaf) {
-          const float4 d = hll_change(a, 1 - bit, Ui, Xi, Us, make_aux(Us), nu);
+          const float4 d = hll_change(a, 1 - bit, Ui, Xa, Us, Xs, nu);
           ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
         }
         if (!leaf) continue;
@@ -196,7 +200,7 @@ amr_transport_hll_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ 
           Un = nb_load(A, box_ghost(-2 - no, a, bit, l, cell), g, Ui);
           box = true;
         }
-        const float4 d = hll_change(a, bit, Ui, Xi, Un, make_aux(Un), nu);
+        const float4 d = hll_change(a, bit, Ui, Xa, Un, make_aux_dir(Un, a), nu);
         ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
         if (box) acc.outflow -= (double)d.x * dV;
       }
@@ -401,7 +405,7 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
     }
     const float4 Ui = A.U[l][(size_t)g * ncell + cell];
     float4 d;
-    if (HLL) d = hll_change(a, side, Ui, make_aux(Ui), Un, make_aux(Un), 2.f * nuh);
+    if (HLL) d = hll_change(a, side, Ui, make_aux_dir(Ui, a), Un, make_aux_dir(Un, a), 2.f * nuh);
     else {
       float ai, bi;
       closure_ab(Ui, ai, bi);
@@ -582,7 +586,7 @@ amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restr
 #pragma unroll
     for (int f = 0; f < 6; f++)
       if (on[f]) {
-        const float4 d = hll_change(f >> 1, f & 1, Ui, Xi, Un[f], make_aux(Un[f]), 2.f * nuh);
+        const float4 d = hll_change(f >> 1, f & 1, Ui, aux_dir(Xi, f >> 1), Un[f], make_aux_dir(Un[f], f >> 1), 2.f * nuh);
         ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
       }
   } else {
@@ -623,7 +627,7 @@ amr_outflow0_kernel(const AmrDev A, const float4* __restrict__ Uold, float nuh, 
       const float4 Ui = Uold[(size_t)g * nc + cell];
       const float4 Un = nb_load(A, r, g, Ui);
       float4 d;
-      if (HLL) d = hll_change(a, side, Ui, make_aux(Ui), Un, make_aux(Un), 2.f * nuh);
+      if (HLL) d = hll_change(a, side, Ui, make_aux_dir(Ui, a), Un, make_aux_dir(Un, a), 2.f * nuh);
       else {
         float ai, bi;
         closure_ab(Ui, ai, bi);

@@ -58,4 +58,33 @@ __device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL,
   return H;
 }
 
+// closure and the wave speeds of ONE direction (a face needs nothing else of its neighbour)
+struct AuxD { float a, b, lm, lp; };
+
+__device__ __forceinline__ AuxD make_aux_dir(const float4& U, int d)
+{
+  AuxD A;
+  const float rN = sel_ge(U.x, 1.1754944e-38f, frcp(U.x));
+  float rx = U.y * rN, ry = U.z * rN, rz = U.w * rN;
+  const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
+  const float f2 = fminf(f2raw, 1.f);
+  const float xi = fsqrt(fmaf(-3.f, f2, 4.f));
+  const float i2 = frcp(2.f + xi);
+  const float q = f2 * i2;
+  A.a = fmaf(-U.x, q, 0.33333334f * U.x);
+  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
+  float rd = (d == 0) ? rx : (d == 1) ? ry : rz;
+  if (f2raw > 1.f) rd *= rsqrtf(f2raw);
+  const float k = 2.f * (1.f - f2) * frcp(xi + 1.f), ixi = frcp(xi), t3 = 3.f * i2;
+  const float sd = fsqrt(fmaxf(k * fmaf(-t3 * rd, rd, xi), 0.f));
+  A.lm = (rd - sd) * ixi; A.lp = (rd + sd) * ixi;
+  return A;
+}
+__device__ __forceinline__ AuxD aux_dir(const Aux& X, int d)
+{
+  AuxD A;
+  A.a = X.a; A.b = X.b; A.lm = X.lm[d]; A.lp = X.lp[d];
+  return A;
+}
+
 }  // namespace emma
