@@ -235,6 +235,15 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
   const float4* __restrict__ Ul = A.U[l];
   const int* __restrict__ child = (l < A.nl) ? A.child[l] : nullptr;
   const int* __restrict__ nbo = A.nbo[l];
+  // a level has < 2^31 cells (checked at init): 32-bit cell indices inside a group, one base pointer per group
+  const float4* __restrict__ Ug[G];
+  float4* __restrict__ Vg[G];
+  float4* __restrict__ Dg[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    Ug[g] = Ul + (size_t)g * ncell; Vg[g] = Unew + (size_t)g * ncell;
+    Dg[g] = (l < A.nl) ? A.dep[l] + (size_t)g * ncell : nullptr;
+  }
   const long long span = (long long)gridDim.x * blockDim.x;
   for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += span) {
     const long long cell = base + threadIdx.x;
@@ -242,13 +251,14 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     const bool leaf = valid && !(child && child[cell] >= 0);
     // only leaves next to a split cell of their own level can have received deposits (bitmap built on the host); the
     // deposit is requested together with the cell's own state so that its latency overlaps with the face work
+    const unsigned ci = (unsigned)cell;
     const bool hd = leaf && l < A.nl && ((A.hasdep[l][cell >> 5] >> (cell & 31)) & 1u);
     float4 Ui[G], sum[G];
     float ai[G], bi[G];
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      Ui[g] = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
-      sum[g] = hd ? A.dep[l][(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
+      Ui[g] = valid ? Ug[g][ci] : make_float4(0.f, 0.f, 0.f, 0.f);
+      sum[g] = hd ? Dg[g][ci] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
 #pragma unroll
     for (int g = 0; g < G; g++) {
@@ -264,19 +274,19 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     // outer faces, indices first (all three pointer loads, then all three split tests, in flight together); a face that
     // does not exist on this level reads the cell itself and is masked out, so the state loads below are branch-free
     int no[3];
-    long long nb[3];
+    unsigned nb[3];
     bool reg[3];
 #pragma unroll
     for (int a = 0; a < 3; a++) no[a] = leaf ? nbo[oct * 6 + 2 * a + ((k >> a) & 1)] : -1;
 #pragma unroll
-    for (int a = 0; a < 3; a++) nb[a] = (no[a] >= 0) ? (((long long)no[a] << 3) | (k ^ (1 << a))) : (valid ? cell : 0);
+    for (int a = 0; a < 3; a++) nb[a] = (no[a] >= 0) ? (((unsigned)no[a] << 3) | (unsigned)(k ^ (1 << a))) : (valid ? ci : 0u);
     int chn[3];
 #pragma unroll
     for (int a = 0; a < 3; a++) chn[a] = (child && no[a] >= 0) ? child[nb[a]] : -1;
 #pragma unroll
     for (int a = 0; a < 3; a++) {
       reg[a] = no[a] >= 0 && chn[a] < 0;                             // a leaf of this level behind the face
-      if (!reg[a]) nb[a] = valid ? cell : 0;
+      if (!reg[a]) nb[a] = valid ? ci : 0u;
     }
 #pragma unroll
     for (int a = 0; a < 3; a++) {
@@ -296,7 +306,7 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
       const float wgt = reg[a] ? 1.f : 0.f;
 #pragma unroll
       for (int g = 0; g < G; g++) {
-        const float4 Un = Ul[(size_t)g * ncell + nb[a]];
+        const float4 Un = Ug[g][nb[a]];
         float an, bn;
         closure_ab(Un, an, bn);
         const float4 T = nb_term(Un, an, bn, a, sg);
@@ -345,10 +355,10 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     }
     if (hd) {
 #pragma unroll
-      for (int g = 0; g < G; g++) A.dep[l][(size_t)g * ncell + cell] = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int g = 0; g < G; g++) Dg[g][ci] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 #pragma unroll
-    for (int g = 0; g < G; g++) Unew[(size_t)g * ncell + cell] = ac[g];
+    for (int g = 0; g < G; g++) Vg[g][ci] = ac[g];
   }
   block_reduce_store(acc, parts + blockIdx.x);
 }
