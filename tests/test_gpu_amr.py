@@ -338,3 +338,24 @@ def test_amr_hll_coupled_steps():
             b = gpu.read(fg, l).astype(np.float64)[masks[l]]
             assert (np.abs(b - a) / np.abs(a)).max() <= TOL_XT, (name, l)
     gpu.close()
+
+
+def test_amr_sources_without_chemistry():
+    """chemistry = 0 (A9: Eq. 43 degenerates to N += S dt): in the standard scheme the sources stay on their leaves (they
+    are folded to the coarse cell only under CRTA) and are added once per sweep of their level."""
+    rng = np.random.default_rng(41)
+    w = make_amr_standard(n=12, G=3, levels=2, seed=31, thresh1=2.0, thresh2=2.5)
+    w.chemistry = 0
+    U = _random_levels(rng, w)
+    orc, gpu = _pair(w, U, chemistry=0)
+    assert orc.source_cell(0)[0] == 2                            # the sources sit on the finest level
+    for step in range(3):
+        rco, do = orc.step(w.dt, 1)
+        rcg, dg = gpu.step(w.dt, 1)
+        assert rco == O.OK and rcg == E.OK, (rco, rcg, gpu.last_error())
+        assert dg["photons_injected"] == pytest.approx(do["photons_injected"], rel=1e-6)
+        assert dg["photons_injected"] == pytest.approx(w.src_Q.sum() * w.dt, rel=1e-6)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+    eN, eF = _errors(orc, gpu, w)
+    assert eN <= 2e-5 and eF <= 2e-5, (eN, eF)
+    gpu.close()
