@@ -64,9 +64,10 @@ enum { EMMA_RT_BC_PERIODIC = 0, EMMA_RT_BC_TRANSMISSIVE = 1, EMMA_RT_BC_REFLECTI
 
 /* fields of emma_rt_read / emma_rt_write.  Element type and count per cell in brackets. */
 enum {
-  EMMA_RT_FIELD_U = 0,          /* [float x4] (N,Fx,Fy,Fz) of `group`; level 0 only             (read, write) */
-  EMMA_RT_FIELD_N = 1,          /* [float]    photon density of `group`; level 0 only           (read)        */
-  EMMA_RT_FIELD_F = 2,          /* [float x3] photon flux of `group`; level 0 only              (read)        */
+  EMMA_RT_FIELD_U = 0,          /* [float x4] (N,Fx,Fy,Fz) of `group`; level 0 (any level with amr_transport; after a write
+                                               split cells are re-restricted before the next step)  (read, write) */
+  EMMA_RT_FIELD_N = 1,          /* [float]    photon density of `group`; level 0 (any level with amr_transport) (read)  */
+  EMMA_RT_FIELD_F = 2,          /* [float x3] photon flux of `group`; level 0 (any level with amr_transport)    (read)  */
   EMMA_RT_FIELD_X = 3,          /* [float]    ionised fraction x                                (read, write) */
   EMMA_RT_FIELD_T = 4,          /* [float]    temperature, T = e / (1.5 (1+x) n0 k_B) (A10)     (read, write: uses the x
                                                currently stored, so write X before T)                          */
@@ -169,7 +170,8 @@ EMMA_RT_API int64_t emma_rt_kernel_launches(const emma_rt* h);                 /
  * nullable) the summed CUDA-event durations and launch counts of the emma_rt_step kernels recorded since the last
  * call, clears them, and switches recording on (enable != 0) or off for the steps that follow.  Off by default. */
 enum { EMMA_RT_K_TRANSPORT = 0, EMMA_RT_K_CHEM_MAIN = 1, EMMA_RT_K_CHEM_TAIL = 2, EMMA_RT_K_CHEM_REFINED = 3,
-       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_FUSED = 6, EMMA_RT_K_AMR_TRANSPORT = 7, EMMA_RT_K_AMR_CHEM = 8,
+       EMMA_RT_K_FINALIZE = 4, EMMA_RT_K_OTHER = 5, EMMA_RT_K_FUSED = 6,
+       EMMA_RT_K_AMR_TRANSPORT = 7 /* refined-level transport + ghost faces */, EMMA_RT_K_AMR_CHEM = 8 /* refined-level chemistry */,
        EMMA_RT_K_COUNT = 9 };
 EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out);
 /* Schedule of the coupled step on the unrefined coarse cells (same result up to fp32 rounding order of nothing: both
