@@ -232,7 +232,10 @@ def test_M5_fig6_call_counts_of_the_standard_scheme():
     assert rc == oracle.OK
     tr, ch = o.counters()
     calls_tr = [tr[l] // o.level_cells(l) for l in range(3)]
-    assert calls_tr == [4, 8, 16] and sum(calls_tr) == 28        # 4 on the coarse level, 24 on the refined
+    from .test_oracle_pins import GOLD                           # tests/golden/paper_values.txt, each value with its citation
+    assert calls_tr[0] == int(GOLD["fig6_standard_coarse_calls"])                       # 4 on the coarse level,
+    assert calls_tr[1] + calls_tr[2] == int(GOLD["fig6_standard_refined_calls"])        # 24 on the refined ones,
+    assert calls_tr == [4, 8, 16] and sum(calls_tr) == int(GOLD["fig6_standard_transport_calls"])   # 28 in all
     leaves = [o.level_cells(0) - len(w.parent[0]), o.level_cells(1) - len(w.parent[1]), o.level_cells(2)]
     assert [ch[l] // leaves[l] for l in range(3)] == [4, 8, 16]
 
