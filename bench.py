@@ -223,7 +223,7 @@ def run_ours(args):
     elif args.amr_standard:
         # the standard (non-CRTA) AMR scheme on a jump-balanced config-4-like mesh
         from workloads.amr import make_amr_standard
-        w = make_amr_standard(n=256 if n == 512 else n, G=3, levels=2, seed=replica_seed(4, rank, world))
+        w = make_amr_standard(n=256 if n == 512 else n, G=3, levels=2, seed=replica_seed(4, rank, world), order=args.oct_order)
         n = w.n
     else:
         w = make_config(5, n=n, variant=args.variant, seed=replica_seed(5, rank, world))
@@ -421,6 +421,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[4, 5], help="BASELINE config: 5 (default, the metric's) or 4 (CRTA)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--unfused", action="store_true", help="separate transport and chemistry passes")
+    ap.add_argument("--oct-order", default="id", choices=["id", "morton"],
+                    help="memory order of the octs of --amr-standard: parent-cell id, or Z-order of the parent's coordinates")
     ap.add_argument("--hll", action="store_true", help="coupled step with the HLL interface flux (two-pass schedule)")
     ap.add_argument("--amr-standard", action="store_true",
                     help="the standard (non-CRTA) AMR scheme on a jump-balanced 256^3 + 2 levels mesh (SURVEY 8f NEXT-2)")

@@ -50,11 +50,26 @@ def _children_density(n0_parent, rng):
     return ch.reshape(-1)
 
 
-def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=2.5, thresh2=4.0, levels=2):
-    """n0c: float64 [n^3] coarse densities.  Returns (parents, n0_levels): parents = [p1, p2][:levels]."""
+def _morton(i, j, k, bits=11):
+    """interleaved bits of (i, j, k): the Z-order key of a cell."""
+    key = np.zeros(len(i), np.int64)
+    for b in range(bits):
+        key |= ((i >> b) & 1).astype(np.int64) << (3 * b)
+        key |= ((j >> b) & 1).astype(np.int64) << (3 * b + 1)
+        key |= ((k >> b) & 1).astype(np.int64) << (3 * b + 2)
+    return key
+
+
+def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=2.5, thresh2=4.0, levels=2, order="id"):
+    """n0c: float64 [n^3] coarse densities.  Returns (parents, n0_levels): parents = [p1, p2][:levels].
+    order: the order of the octs of a level in memory (the C-ABI takes them in the order of the parent list): "id" =
+    increasing id of the parent cell; "morton" = along the Z-order curve of the parent cell's coordinates, which keeps
+    the octs of a patch, and so the neighbours a kernel reads together, close in memory."""
     S = _mean27(n0c.reshape(n, n, n))
     mark0 = _dilate26(S > thresh1 * nbar)
     p1 = np.flatnonzero(mark0.reshape(-1)).astype(np.int64)
+    if order == "morton":
+        p1 = p1[np.argsort(_morton(p1 % n, (p1 // n) % n, p1 // (n * n)), kind="stable")]
     n01 = _children_density(n0c[p1], rng)
     if levels == 1 or len(p1) == 0:
         return [p1], [n0c, n01]
@@ -68,11 +83,15 @@ def balanced_two_level_mesh(n0c, n, nbar, rng, thresh1=2.5, thresh2=4.0, levels=
     S1 = np.repeat(np.repeat(np.repeat(S, 2, axis=0), 2, axis=1), 2, axis=2)       # the parent's S on the level-1 grid
     mark1 = exist & (S1 > thresh2 * nbar) & _all26(exist)
     p2 = np.sort(id1[mark1]).astype(np.int64)
+    if order == "morton":
+        kz, ky, kx = np.nonzero(mark1)
+        p2 = id1[kz, ky, kx][np.argsort(_morton(kx, ky, kz), kind="stable")].astype(np.int64)
     n02 = _children_density(n01[p2], rng)
     return [p1, p2], [n0c, n01, n02]
 
 
-def make_amr_standard(n=16, G=3, levels=2, n_steps=4, n_src=None, sigma_ln=1.5, seed=None, thresh1=2.5, thresh2=4.0):
+def make_amr_standard(n=16, G=3, levels=2, n_steps=4, n_src=None, sigma_ln=1.5, seed=None, thresh1=2.5, thresh2=4.0,
+                      order="id"):
     """Config-4-like box on a jump-balanced mesh, for the standard AMR transport: lognormal density,
     sources in the densest leaves of the finest level, x = 1.2e-3, T = 100 K, N = F = 0, periodic."""
     rng = np.random.default_rng(SEED_BASE + 42 if seed is None else seed)
@@ -81,7 +100,7 @@ def make_amr_standard(n=16, G=3, levels=2, n_steps=4, n_src=None, sigma_ln=1.5, 
     w = Workload("amr-standard%d" % n, n, G, dx * n, 0.1 * CGS.c, gr["sigma_N"], gr["sigma_E"], gr["E_mean"], gr["frac"])
     nbar = 1e-3
     n0c = lognormal_density(n, nbar, sigma_ln, rng).reshape(-1).astype(np.float64)
-    parents, n0s = balanced_two_level_mesh(n0c, n, nbar, rng, thresh1, thresh2, levels)
+    parents, n0s = balanced_two_level_mesh(n0c, n, nbar, rng, thresh1, thresh2, levels, order)
     w.parent = parents
     w.n0 = [a.astype(np.float32) for a in n0s]
     w.x = [np.full(a.shape, 1.2e-3, np.float32) for a in w.n0]
