@@ -111,6 +111,8 @@ def lib():
     L.orc_set_amr_transport.argtypes = [C.c_void_p, C.c_int]
     L.orc_write_U.restype = C.c_int
     L.orc_write_U.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+    L.orc_amr_ghost.restype = C.c_int
+    L.orc_amr_ghost.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int64, dp]
     L.orc_restrict_U.restype = C.c_int
     L.orc_restrict_U.argtypes = [C.c_void_p]
     _lib = L
@@ -249,6 +251,15 @@ class Oracle:
     def write_U(self, level, group, U):
         U = np.ascontiguousarray(U, np.float64).reshape(self.level_cells(level), 4)
         return lib().orc_write_U(self.h, int(level), int(group), _dp(U))
+
+    def amr_ghost(self, level, group, v, coarse_cell):
+        """Interpolated state of the virtual level-`level` cell at integer coordinates v inside the coarser leaf (A21)."""
+        vv = (C.c_int * 3)(*[int(t) for t in v])
+        out = np.zeros(4)
+        rc = lib().orc_amr_ghost(self.h, int(level), int(group), vv, int(coarse_cell), _dp(out))
+        if rc != OK:
+            raise ValueError("orc_amr_ghost rc=%d" % rc)
+        return out
 
     def restrict_U(self):
         return lib().orc_restrict_U(self.h)

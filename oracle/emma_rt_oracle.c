@@ -1012,6 +1012,16 @@ int orc_set_amr_transport(orc* o, int on)
   return ORC_OK;
 }
 
+/* test hook: the interpolated state (A21) of the virtual level-`level` cell at integer coordinates v[] that
+ * lies inside the level-(level-1) leaf `coarse_cell` */
+int orc_amr_ghost(orc* o, int level, int group, const int v[3], int64_t coarse_cell, double out[4])
+{
+  if (!o || !o->amr || level < 1 || level > o->n_levels + 1 || group < 0 || group >= o->ph.G) return ORC_EINVAL;
+  if (coarse_cell < 0 || coarse_cell >= o->ncell[level - 1]) return ORC_EINVAL;
+  amr_ghost(o, level, group, v, coarse_cell, out);
+  return ORC_OK;
+}
+
 /* overwrite the radiation of one level and group (tests: random refined states); src is [ncell_l][4] */
 int orc_write_U(orc* o, int level, int group, const double* src)
 {

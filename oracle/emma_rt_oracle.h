@@ -89,6 +89,7 @@ int  orc_set_flux(orc*, int flux);          /* interface flux of the transport s
  * EINVAL if a resolution jump across a face exceeds 1.  Refined cells start with their parent's radiation. */
 int  orc_set_amr_transport(orc*, int on);
 int  orc_write_U(orc*, int level, int group, const double* src);   /* [ncell_l][4]; level > 0 needs amr transport on */
+int  orc_amr_ghost(orc*, int level, int group, const int v[3], int64_t coarse_cell, double out[4]);   /* test hook (A21) */
 int  orc_restrict_U(orc*);                                         /* split cells := children mean, after orc_write_U */
 int  orc_step(orc*, double dt, int n_steps, orc_diag* diag_last);
 int  orc_read(const orc*, int field, int level, int group, double* dst, int64_t n_dst);

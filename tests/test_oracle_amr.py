@@ -7,6 +7,7 @@ M4  brute force: an independent dict-based transcription (tests/brute_amr.py) on
 M5  Fig. 6 call counts of the standard scheme: 4 coarse steps with 2 refined levels = 4 + 24 engine calls
 M6  a resolution jump of 2 across a face is refused
 M7  a beam crossing a refined slab keeps its photons and its speed
+M9  the ghost of a linear field is the field at the centre of the virtual fine cell, all 8 positions
 M8  PAPER.md:556: the CRTA front follows the standard scheme's (static HII region with a refined shell)
 """
 import numpy as np
@@ -338,3 +339,45 @@ def test_M8_crta_front_follows_the_standard_scheme():
     assert np.all(np.diff(r_std) > 0)
     ahead = slice(4, 8)                                           # just ahead of the x = 0.5 point
     assert np.all(x_std[ahead] < x_crta[ahead])
+
+
+def test_M9_ghost_of_a_linear_field_is_exact():
+    """the missing fine neighbour "is interpolated linearly from coarse data at the position of the fine virtual
+    cell".  For a field that is linear in x, y, z (all four components, different gradients) the MinMod slopes are the
+    gradient, so the ghost must equal the field at the centre of the virtual cell -- for each of the 8 positions inside the
+    coarse leaf, on level 0 and on level 1.  Pins the +-1/4 offsets and the axis <-> child-bit mapping independently of any
+    transcription of the scheme."""
+    n = 8
+    # level 1: the block [2,6)^3; level 2: level-1 cells [6,10)^3 (inside, with a level-1 buffer around)
+    ids = np.arange(n ** 3)
+    cx, cy, cz = ids % n, (ids // n) % n, ids // (n * n)
+    p1 = ids[(cx >= 2) & (cx < 6) & (cy >= 2) & (cy < 6) & (cz >= 2) & (cz < 6)].astype(np.int64)
+    co1 = coords_of(n, [p1])[1]
+    sel = np.all((co1 >= 6) & (co1 < 10), axis=1)
+    p2 = np.flatnonzero(sel).astype(np.int64)
+    w = tiny_workload(n, G=1, parent=[p1, p2], chemistry=0, bc=(1,) * 6)
+    o = oracle.Oracle(w, chemistry=0)
+    assert o.set_amr_transport(True) == oracle.OK
+    co = coords_of(n, [p1, p2])
+    grad = np.array([[1.0, 0.3, -0.2, 0.5], [0.7, -0.4, 0.6, 0.1], [-0.5, 0.2, 0.3, -0.6]])     # d/dx, d/dy, d/dz of (N, Fx, Fy, Fz)
+    base = np.array([50.0, 1.0, -2.0, 3.0])
+    field = lambda pos: base[None, :] + pos @ grad                     # pos in units of the coarse cell size
+    for l in range(3):
+        o.write_U(l, 0, field((co[l] + 0.5) / 2 ** l))
+    # level-0 leaf (1,3,3) next to the block: virtual level-1 cells inside it
+    c0 = 1 + n * (3 + n * 3)
+    for k in range(8):
+        v = np.array([2 * 1 + (k & 1), 2 * 3 + ((k >> 1) & 1), 2 * 3 + ((k >> 2) & 1)])
+        np.testing.assert_allclose(o.amr_ghost(1, 0, v, c0), field(((v + 0.5) / 2)[None, :])[0], rtol=1e-13)
+    # level-1 leaf next to the level-2 block: the level-1 cell at (5,7,7) (exists, unsplit); virtual level-2 cells inside it
+    c1 = int(np.flatnonzero(np.all(co[1] == np.array([5, 7, 7]), axis=1))[0])
+    assert c1 not in set(p2.tolist())
+    for k in range(8):
+        v = np.array([2 * 5 + (k & 1), 2 * 7 + ((k >> 1) & 1), 2 * 7 + ((k >> 2) & 1)])
+        np.testing.assert_allclose(o.amr_ghost(2, 0, v, c1), field(((v + 0.5) / 4)[None, :])[0], rtol=1e-13)
+    # an extremum is not extrapolated: MinMod gives a zero slope there
+    U = field((co[0] + 0.5))
+    U[c0] = 1e3
+    o.write_U(0, 0, U)
+    g = o.amr_ghost(1, 0, np.array([2, 6, 6]), c0)
+    np.testing.assert_allclose(g, U[c0], rtol=0, atol=0)
