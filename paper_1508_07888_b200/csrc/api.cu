@@ -213,6 +213,111 @@ AmrDev amr_view(const emma_rt* h)
   return A;
 }
 
+// One emma_rt_step call in AMR-transport mode (reading A21): the recursion advance(l, dt) = advance(l+1, dt/2) x 2
+// -> transport(l) -> chemistry(l) -> restrict(l+1 -> l), flattened into a list of level sweeps per coarse step.
+int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const TransportParams& hp, const ChemParams& cp,
+             bool use_tma, bool hll)
+{
+  const Shape& s = h->sh;
+  const double c = h->cfg.c_red_cm_s;
+  // standard AMR scheme (A21): advance(l, dt) = advance(l+1, dt/2) x 2 -> transport(l) -> chemistry(l) -> restrict(l+1 -> l)
+  const int ihll = hll ? 1 : 0;
+  const float nuh = (float)(0.5 * (c * dt / h->dx));           // the same CFL number on every level
+  tp.want_total = 0;
+  bool open_faces = false;
+  for (int f = 0; f < 6; f++) open_faces = open_faces || h->cfg.bc[f] != EMMA_RT_BC_PERIODIC;
+  if (h->amr_dirty) {                                          // U was written: split cells := children mean
+    for (int l = s.nl; l >= 1; l--) h->launches += launch_amr_restrict(h->lv[l], h->lv[l - 1], amr_view(h), l, 0, h->st);
+    h->amr_dirty = false;
+  }
+  for (int step = 0; step < n_steps; step++) {
+    int off = 0;
+    Partial* P = h->parts();
+    // (level, dt, last sub-step of the level in this coarse step) in execution order, finest first
+    struct Call { int l; double dt; bool last; };
+    std::vector<Call> order;
+    struct Rec { static void go(std::vector<Call>& o, int l, int nl, const long long* nc, double dtl, bool last) {
+      if (l < nl && nc[l + 1] > 0) { go(o, l + 1, nl, nc, 0.5 * dtl, false); go(o, l + 1, nl, nc, 0.5 * dtl, last); }
+      o.push_back({l, dtl, last});
+    } };
+    Rec::go(order, 0, s.nl, s.ncell, dt, true);
+    for (const Call& cl : order) {
+      const int l = cl.l;
+      int np = 0;
+      if (off + 3 * MAX_PART_BLOCKS > PART_SLOTS) return fail(h, EMMA_RT_EINVAL, "too many level sweeps for the partial-sum slots");
+      if (l == 0) {
+        // dense pass over the whole block (its partials are not used: split cells must not count), then the
+        // sparse correction of the leaves that touch a split cell
+        h->prof.begin(EMMA_RT_K_TRANSPORT);
+        if (hll) {
+          const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+          if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+          h->launches += k;
+        } else if (use_tma) {
+          const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+          if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+          h->launches += k;
+        } else h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
+        h->prof.end();
+        AmrDev A = amr_view(h);
+        h->prof.begin(EMMA_RT_K_OTHER);
+        if (open_faces) { h->launches += launch_amr_outflow0(A, h->U(h->cur), nuh, h->lv[0].dV, ihll, P + off, &np, h->st); off += np; }
+        h->launches += launch_amr_fix0(A, h->U(h->cur), h->U(1 - h->cur), (const int*)(h->arena + h->lay.afix_cell),
+                                       (const unsigned char*)(h->arena + h->lay.afix_mask), h->n_fix, nuh, ihll, h->st);
+        h->prof.end();
+        h->cur = 1 - h->cur;
+        if (h->cfg.chemistry) {
+          h->launches += launch_chem_level0(cp, h->lv[0], h->U(h->cur), s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
+                                            P + off, &np, h->sm_count, h->st, &h->prof);
+          off += np;
+        } else {
+          h->prof.begin(EMMA_RT_K_OTHER);
+          h->launches += launch_amr_sources(h->lv[0], amr_view(h), 0, (float)dt, 1, 0, P + off, &np, h->st);
+          h->prof.end();
+          off += np;
+        }
+      } else {
+        AmrDev A = amr_view(h);
+        h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
+        h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, ihll, P + off, &np, h->st);
+        h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
+                                              (const int*)(h->arena + h->lay.aslot_coarse[l]),
+                                              (const unsigned char*)(h->arena + h->lay.aslot_face[l]),
+                                              (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], ihll, h->st);
+        h->prof.end();
+        off += np;
+        h->acur[l] = 1 - h->acur[l];
+        A = amr_view(h);
+        ChemParams cl_cp = cp;
+        cl_cp.dt = (float)cl.dt;
+        h->prof.begin(EMMA_RT_K_AMR_CHEM);
+        if (h->cfg.chemistry && !hll) {
+          // the two-pass chemistry of level 0 (bulk-async main pass + compacted tail, chemistry.cu) on this level's arrays
+          LevelDev Lc = h->lv[l];
+          Lc.refined = l < s.nl ? (unsigned int*)(h->arena + h->lay.arefined[l]) : nullptr;
+          Lc.dV_total = cl.last ? Lc.dV : 0.0;
+          h->launches += launch_chem_level0(cl_cp, Lc, h->Ulev(l), s.ncell[l], (int*)(h->arena + h->lay.queue), h->qcount(),
+                                            P + off, &np, h->sm_count, h->st, nullptr_prof(h));
+          CUDA_TRY(h, cudaMemsetAsync(h->qcount(), 0, 8, h->st));      // queue counters of the next sweep
+        } else if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
+        else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
+        h->prof.end();
+        off += np;
+      }
+      if (l < s.nl && s.ncell[l + 1] > 0) {
+        h->prof.begin(EMMA_RT_K_OTHER);
+        h->launches += launch_amr_restrict(h->lv[l + 1], h->lv[l], amr_view(h), l + 1, h->cfg.chemistry ? 1 : 0, h->st);
+        h->prof.end();
+      }
+    }
+    h->t_sim += dt;
+    h->prof.begin(EMMA_RT_K_FINALIZE);
+    h->launches += launch_finalize(P, off, h->diag(), h->qcount(), h->t_sim, h->st);
+    h->prof.end();
+  }
+  return EMMA_RT_OK;
+}
+
 size_t field_elem_bytes(int field)
 {
   switch (field) {
@@ -640,101 +745,8 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
 
   if (s.amr) {
-    // standard AMR scheme (A21): advance(l, dt) = advance(l+1, dt/2) x 2 -> transport(l) -> chemistry(l) -> restrict(l+1 -> l)
-    const int ihll = hll ? 1 : 0;
-    const float nuh = (float)(0.5 * (c * dt / h->dx));           // the same CFL number on every level
-    tp.want_total = 0;
-    bool open_faces = false;
-    for (int f = 0; f < 6; f++) open_faces = open_faces || h->cfg.bc[f] != EMMA_RT_BC_PERIODIC;
-    if (h->amr_dirty) {                                          // U was written: split cells := children mean
-      for (int l = s.nl; l >= 1; l--) h->launches += launch_amr_restrict(h->lv[l], h->lv[l - 1], amr_view(h), l, 0, h->st);
-      h->amr_dirty = false;
-    }
-    for (int step = 0; step < n_steps; step++) {
-      int off = 0;
-      Partial* P = h->parts();
-      // (level, dt, last sub-step of the level in this coarse step) in execution order, finest first
-      struct Call { int l; double dt; bool last; };
-      std::vector<Call> order;
-      struct Rec { static void go(std::vector<Call>& o, int l, int nl, const long long* nc, double dtl, bool last) {
-        if (l < nl && nc[l + 1] > 0) { go(o, l + 1, nl, nc, 0.5 * dtl, false); go(o, l + 1, nl, nc, 0.5 * dtl, last); }
-        o.push_back({l, dtl, last});
-      } };
-      Rec::go(order, 0, s.nl, s.ncell, dt, true);
-      for (const Call& cl : order) {
-        const int l = cl.l;
-        int np = 0;
-        if (off + 3 * MAX_PART_BLOCKS > PART_SLOTS) return fail(h, EMMA_RT_EINVAL, "too many level sweeps for the partial-sum slots");
-        if (l == 0) {
-          // dense pass over the whole block (its partials are not used: split cells must not count), then the
-          // sparse correction of the leaves that touch a split cell
-          h->prof.begin(EMMA_RT_K_TRANSPORT);
-          if (hll) {
-            const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
-            if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-            h->launches += k;
-          } else if (use_tma) {
-            const int k = launch_transport_tma(tp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
-            if (!k) return fail(h, EMMA_RT_ECUDA, "transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-            h->launches += k;
-          } else h->launches += launch_transport(tp, h->U(h->cur), h->U(1 - h->cur), P + off, &np, h->st);
-          h->prof.end();
-          AmrDev A = amr_view(h);
-          h->prof.begin(EMMA_RT_K_OTHER);
-          if (open_faces) { h->launches += launch_amr_outflow0(A, h->U(h->cur), nuh, h->lv[0].dV, ihll, P + off, &np, h->st); off += np; }
-          h->launches += launch_amr_fix0(A, h->U(h->cur), h->U(1 - h->cur), (const int*)(h->arena + h->lay.afix_cell),
-                                         (const unsigned char*)(h->arena + h->lay.afix_mask), h->n_fix, nuh, ihll, h->st);
-          h->prof.end();
-          h->cur = 1 - h->cur;
-          if (h->cfg.chemistry) {
-            h->launches += launch_chem_level0(cp, h->lv[0], h->U(h->cur), s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
-                                              P + off, &np, h->sm_count, h->st, &h->prof);
-            off += np;
-          } else {
-            h->prof.begin(EMMA_RT_K_OTHER);
-            h->launches += launch_amr_sources(h->lv[0], amr_view(h), 0, (float)dt, 1, 0, P + off, &np, h->st);
-            h->prof.end();
-            off += np;
-          }
-        } else {
-          AmrDev A = amr_view(h);
-          h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
-          h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, ihll, P + off, &np, h->st);
-          h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
-                                                (const int*)(h->arena + h->lay.aslot_coarse[l]),
-                                                (const unsigned char*)(h->arena + h->lay.aslot_face[l]),
-                                                (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], ihll, h->st);
-          h->prof.end();
-          off += np;
-          h->acur[l] = 1 - h->acur[l];
-          A = amr_view(h);
-          ChemParams cl_cp = cp;
-          cl_cp.dt = (float)cl.dt;
-          h->prof.begin(EMMA_RT_K_AMR_CHEM);
-          if (h->cfg.chemistry && !hll) {
-            // the two-pass chemistry of level 0 (bulk-async main pass + compacted tail, chemistry.cu) on this level's arrays
-            LevelDev Lc = h->lv[l];
-            Lc.refined = l < s.nl ? (unsigned int*)(h->arena + h->lay.arefined[l]) : nullptr;
-            Lc.dV_total = cl.last ? Lc.dV : 0.0;
-            h->launches += launch_chem_level0(cl_cp, Lc, h->Ulev(l), s.ncell[l], (int*)(h->arena + h->lay.queue), h->qcount(),
-                                              P + off, &np, h->sm_count, h->st, nullptr_prof(h));
-            CUDA_TRY(h, cudaMemsetAsync(h->qcount(), 0, 8, h->st));      // queue counters of the next sweep
-          } else if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
-          else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
-          h->prof.end();
-          off += np;
-        }
-        if (l < s.nl && s.ncell[l + 1] > 0) {
-          h->prof.begin(EMMA_RT_K_OTHER);
-          h->launches += launch_amr_restrict(h->lv[l + 1], h->lv[l], amr_view(h), l + 1, h->cfg.chemistry ? 1 : 0, h->st);
-          h->prof.end();
-        }
-      }
-      h->t_sim += dt;
-      h->prof.begin(EMMA_RT_K_FINALIZE);
-      h->launches += launch_finalize(P, off, h->diag(), h->qcount(), h->t_sim, h->st);
-      h->prof.end();
-    }
+    const int rc = step_amr(h, dt, n_steps, tp, hp, cp, use_tma, hll);
+    if (rc != EMMA_RT_OK) return rc;
   }
   for (int step = 0; step < (s.amr ? 0 : n_steps); step++) {
     int off = 0, np = 0;
