@@ -318,6 +318,163 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
   return EMMA_RT_OK;
 }
 
+// Index arrays of the AMR-transport mode (reading A21, section 4), built once on the host for the static mesh:
+// the paper's oct neighbour pointers (the 6 cells of level l-1 around the oct's parent cell) and what the
+// kernels read, derived from them: same-level neighbour octs, the level-0 child index, the receivers of deposits, the
+// faces towards a coarser leaf with their six resolved coarse references, the level-0 leaves that touch a split cell.
+// A face jump > 1 is refused here.
+int init_amr_topology(emma_rt* h, const std::vector<std::vector<int>>& parent_h, const std::vector<std::vector<int>>& child_h)
+{
+  const Shape& s = h->sh;
+  std::vector<std::vector<int>> nbr_h(s.nl + 1);
+  std::vector<int> child0_h, fix_cell_h;
+  std::vector<unsigned char> fix_mask_h;
+  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1), slot_refs_h(s.nl + 1);
+  std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
+  std::vector<std::vector<unsigned int>> hasdep_h(s.nl + 1), refined_lv_h(s.nl + 1);
+  const int n = s.n;
+  auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
+  // neighbour of a level-0 cell, or the box-face code
+  auto nb0 = [&](long long cell, int a, int side) -> long long {
+    const long long stride = a == 0 ? 1 : a == 1 ? n : (long long)n * n;
+    const int ca = a == 0 ? (int)(cell % n) : a == 1 ? (int)((cell / n) % n) : (int)(cell / ((long long)n * n));
+    const int cn = ca + (side ? 1 : -1);
+    if (cn < 0 || cn >= n) {
+      if (h->cfg.bc[2 * a + side] != EMMA_RT_BC_PERIODIC) return bc_code(a, side);
+      return cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride;
+    }
+    return cell + (side ? stride : -stride);
+  };
+  for (int l = 1; l <= s.nl; l++) {
+    nbr_h[l].resize((size_t)s.nocts[l] * 6);
+    for (long long o = 0; o < s.nocts[l]; o++) {
+      const long long p = parent_h[l][o];                      // the oct's parent cell, on level l-1
+      for (int a = 0; a < 3; a++)
+        for (int side = 0; side < 2; side++) {
+          long long q;
+          if (l == 1) q = nb0(p, a, side);
+          else {
+            const long long po = p >> 3;                       // the parent cell's own oct (level l-1)
+            const int k = (int)(p & 7), bit = (k >> a) & 1;
+            if (side != bit) q = (po << 3) | (k ^ (1 << a));
+            else {
+              const int pp = nbr_h[l - 1][po * 6 + 2 * a + side];     // cell of level l-2
+              if (pp < 0) q = pp;
+              else {
+                auto it = h->child_of[l - 2].find(pp);
+                if (it == h->child_of[l - 2].end())
+                  return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 across a face of oct %lld of level %d (PAPER.md:75)", o, l);
+                q = ((long long)it->second << 3) | (k ^ (1 << a));
+              }
+            }
+          }
+          nbr_h[l][o * 6 + 2 * a + side] = (int)q;
+        }
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbr[l], nbr_h[l].data(), nbr_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+  }
+  child0_h.assign((size_t)s.ncell[0], -1);
+  for (auto& kv : h->child_of[0]) child0_h[kv.first] = kv.second;
+  CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.achild0, child0_h.data(), child0_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+  // same-level neighbour octs, derived from the neighbour-cell pointers
+  for (int l = 1; l <= s.nl; l++) {
+    nbo_h[l].resize((size_t)s.nocts[l] * 6);
+    for (size_t i = 0; i < nbo_h[l].size(); i++) {
+      const int pcell = nbr_h[l][i];
+      if (pcell < 0) { nbo_h[l][i] = pcell - 1; continue; }              // -1 - bc  ->  -2 - bc
+      nbo_h[l][i] = (l == 1) ? child0_h[pcell] : child_h[l - 1][pcell];  // oct of level l, or -1: coarser leaf
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+  }
+  // leaves of a refined level that touch a split cell of the same level (they receive deposits)
+  for (int l = 1; l < s.nl; l++) {
+    refined_lv_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
+    for (auto& kv : h->child_of[l]) refined_lv_h[l][kv.first >> 5] |= 1u << (kv.first & 31);
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.arefined[l], refined_lv_h[l].data(), refined_lv_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+    hasdep_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
+    for (auto& kv : h->child_of[l]) {
+      const long long p = kv.first, po = p >> 3;
+      const int k = (int)(p & 7);
+      for (int a = 0; a < 3; a++)
+        for (int side = 0; side < 2; side++) {
+          long long q;
+          if (side != ((k >> a) & 1)) q = (po << 3) | (k ^ (1 << a));
+          else {
+            const int no = nbo_h[l][po * 6 + 2 * a + side];
+            if (no < 0) continue;
+            q = ((long long)no << 3) | (k ^ (1 << a));
+          }
+          if (child_h[l][q] < 0) hasdep_h[l][q >> 5] |= 1u << (q & 31);
+        }
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.ahasdep[l], hasdep_h[l].data(), hasdep_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+  }
+  // faces of refined cells towards a coarser leaf: (fine cell, coarse leaf, face), 4 per oct face
+  for (int l = 1; l <= s.nl; l++) {
+    for (long long o = 0; o < s.nocts[l]; o++)
+      for (int f = 0; f < 6; f++) {
+        const int pcell = nbr_h[l][o * 6 + f];
+        if (pcell < 0) continue;
+        const bool split = (l == 1) ? child0_h[pcell] >= 0 : child_h[l - 1][pcell] >= 0;
+        if (split) continue;
+        const int a = f >> 1, side = f & 1;
+        // the six neighbours of the coarse leaf `pcell` on its own level l-1, for the ghost slopes (reading A21)
+        for (int b = 0; b < 3; b++)
+          for (int sd = 0; sd < 2; sd++) {
+            long long q;                                                 // >= 0: cell of level l-1; else a code
+            auto box = [&](int code) { const int bc = -1 - code; return bc == EMMA_RT_BC_INFLOW ? -5 : bc == EMMA_RT_BC_REFLECTIVE ? -2 - b : -1; };
+            if (l == 1) { q = nb0(pcell, b, sd); if (q < 0) q = box((int)q); }
+            else {
+              const long long po = pcell >> 3;
+              const int kk = pcell & 7, bit = (kk >> b) & 1;
+              if (sd != bit) q = (po << 3) | (kk ^ (1 << b));
+              else {
+                const int pp = nbr_h[l - 1][po * 6 + 2 * b + sd];       // cell of level l-2
+                if (pp < 0) q = box(pp);
+                else {
+                  const int ch = (l == 2) ? child0_h[pp] : child_h[l - 2][pp];
+                  q = ch >= 0 ? (((long long)ch << 3) | (kk ^ (1 << b))) : (-16LL - pp);
+                }
+              }
+            }
+            slot_refs_h[l].push_back((int)q);
+          }
+        for (int k = 0; k < 8; k++) {                                    // always 4 entries per oct side (kept aligned)
+          if (((k >> a) & 1) != side) continue;
+          if (l < s.nl && child_h[l][(o << 3) | k] >= 0)
+            return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 at oct %lld of level %d (PAPER.md:75)", o, l);
+          slot_cell_h[l].push_back((int)((o << 3) | k));
+          slot_coarse_h[l].push_back(pcell);
+          slot_face_h[l].push_back((unsigned char)f);
+        }
+      }
+    h->n_slots[l] = (int)slot_cell_h[l].size();
+    if (h->n_slots[l]) {
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_cell[l], slot_cell_h[l].data(), slot_cell_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_coarse[l], slot_coarse_h[l].data(), slot_coarse_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_face[l], slot_face_h[l].data(), slot_face_h[l].size(), cudaMemcpyHostToDevice, h->st));
+      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_refs[l], slot_refs_h[l].data(), slot_refs_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
+    }
+  }
+  // level-0 leaves next to a split cell, with the mask of the faces that look at one (sorted by cell id)
+  std::map<long long, unsigned> fix;
+  for (auto& kv : h->child_of[0])
+    for (int a = 0; a < 3; a++)
+      for (int side = 0; side < 2; side++) {
+        const long long q = nb0(kv.first, a, side);
+        if (q < 0 || child0_h[q] >= 0) continue;
+        fix[q] |= 1u << (2 * a + (1 - side));                   // q sees the split cell through its opposite face
+      }
+  for (auto& kv : fix) { fix_cell_h.push_back((int)kv.first); fix_mask_h.push_back((unsigned char)kv.second); }
+  h->n_fix = (int)fix_cell_h.size();
+  if (h->n_fix) {
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_cell, fix_cell_h.data(), fix_cell_h.size() * 4, cudaMemcpyHostToDevice, h->st));
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_mask, fix_mask_h.data(), fix_mask_h.size(), cudaMemcpyHostToDevice, h->st));
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));   // the staging vectors above go out of scope
+  return EMMA_RT_OK;
+}
+
 size_t field_elem_bytes(int field)
 {
   switch (field) {
@@ -446,155 +603,12 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
     for (auto& kv : h->child_of[0]) refined_h[kv.first >> 5] |= 1u << (kv.first & 31);
     CUDA_TRY(h, cudaMemcpyAsync(h->lv[0].refined, refined_h.data(), refined_h.size() * 4, cudaMemcpyHostToDevice, h->st));
   }
-  // ---- standard AMR transport (A21): the paper's oct neighbour pointers, level-0 child index, fix list
-  std::vector<std::vector<int>> nbr_h(s.nl + 1);
-  std::vector<int> child0_h, fix_cell_h;
-  std::vector<unsigned char> fix_mask_h;
+  // ---- standard AMR transport (A21): oct neighbour pointers and the index arrays derived from them
   h->n_fix = 0; h->amr_dirty = false;
   for (int l = 0; l <= MAXL; l++) { h->acur[l] = 0; h->n_slots[l] = 0; }
-  std::vector<std::vector<int>> slot_cell_h(s.nl + 1), slot_coarse_h(s.nl + 1), nbo_h(s.nl + 1), slot_refs_h(s.nl + 1);
-  std::vector<std::vector<unsigned char>> slot_face_h(s.nl + 1);
-  std::vector<std::vector<unsigned int>> hasdep_h(s.nl + 1), refined_lv_h(s.nl + 1);
   if (s.amr) {
-    const int n = s.n;
-    auto bc_code = [&](int a, int side) { return -1 - h->cfg.bc[2 * a + side]; };       // non-periodic box face
-    // neighbour of a level-0 cell, or the box-face code
-    auto nb0 = [&](long long cell, int a, int side) -> long long {
-      const long long stride = a == 0 ? 1 : a == 1 ? n : (long long)n * n;
-      const int ca = a == 0 ? (int)(cell % n) : a == 1 ? (int)((cell / n) % n) : (int)(cell / ((long long)n * n));
-      const int cn = ca + (side ? 1 : -1);
-      if (cn < 0 || cn >= n) {
-        if (h->cfg.bc[2 * a + side] != EMMA_RT_BC_PERIODIC) return bc_code(a, side);
-        return cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride;
-      }
-      return cell + (side ? stride : -stride);
-    };
-    for (int l = 1; l <= s.nl; l++) {
-      nbr_h[l].resize((size_t)s.nocts[l] * 6);
-      for (long long o = 0; o < s.nocts[l]; o++) {
-        const long long p = parent_h[l][o];                      // the oct's parent cell, on level l-1
-        for (int a = 0; a < 3; a++)
-          for (int side = 0; side < 2; side++) {
-            long long q;
-            if (l == 1) q = nb0(p, a, side);
-            else {
-              const long long po = p >> 3;                       // the parent cell's own oct (level l-1)
-              const int k = (int)(p & 7), bit = (k >> a) & 1;
-              if (side != bit) q = (po << 3) | (k ^ (1 << a));
-              else {
-                const int pp = nbr_h[l - 1][po * 6 + 2 * a + side];     // cell of level l-2
-                if (pp < 0) q = pp;
-                else {
-                  auto it = h->child_of[l - 2].find(pp);
-                  if (it == h->child_of[l - 2].end())
-                    return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 across a face of oct %lld of level %d (PAPER.md:75)", o, l);
-                  q = ((long long)it->second << 3) | (k ^ (1 << a));
-                }
-              }
-            }
-            nbr_h[l][o * 6 + 2 * a + side] = (int)q;
-          }
-      }
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbr[l], nbr_h[l].data(), nbr_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-    }
-    child0_h.assign((size_t)s.ncell[0], -1);
-    for (auto& kv : h->child_of[0]) child0_h[kv.first] = kv.second;
-    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.achild0, child0_h.data(), child0_h.size() * 4, cudaMemcpyHostToDevice, h->st));
-    // same-level neighbour octs, derived from the neighbour-cell pointers
-    for (int l = 1; l <= s.nl; l++) {
-      nbo_h[l].resize((size_t)s.nocts[l] * 6);
-      for (size_t i = 0; i < nbo_h[l].size(); i++) {
-        const int pcell = nbr_h[l][i];
-        if (pcell < 0) { nbo_h[l][i] = pcell - 1; continue; }              // -1 - bc  ->  -2 - bc
-        nbo_h[l][i] = (l == 1) ? child0_h[pcell] : child_h[l - 1][pcell];  // oct of level l, or -1: coarser leaf
-      }
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-    }
-    // leaves of a refined level that touch a split cell of the same level (they receive deposits)
-    for (int l = 1; l < s.nl; l++) {
-      refined_lv_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
-      for (auto& kv : h->child_of[l]) refined_lv_h[l][kv.first >> 5] |= 1u << (kv.first & 31);
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.arefined[l], refined_lv_h[l].data(), refined_lv_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-      hasdep_h[l].assign((size_t)(s.ncell[l] + 31) / 32, 0u);
-      for (auto& kv : h->child_of[l]) {
-        const long long p = kv.first, po = p >> 3;
-        const int k = (int)(p & 7);
-        for (int a = 0; a < 3; a++)
-          for (int side = 0; side < 2; side++) {
-            long long q;
-            if (side != ((k >> a) & 1)) q = (po << 3) | (k ^ (1 << a));
-            else {
-              const int no = nbo_h[l][po * 6 + 2 * a + side];
-              if (no < 0) continue;
-              q = ((long long)no << 3) | (k ^ (1 << a));
-            }
-            if (child_h[l][q] < 0) hasdep_h[l][q >> 5] |= 1u << (q & 31);
-          }
-      }
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.ahasdep[l], hasdep_h[l].data(), hasdep_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-    }
-    // faces of refined cells towards a coarser leaf: (fine cell, coarse leaf, face), 4 per oct face
-    for (int l = 1; l <= s.nl; l++) {
-      for (long long o = 0; o < s.nocts[l]; o++)
-        for (int f = 0; f < 6; f++) {
-          const int pcell = nbr_h[l][o * 6 + f];
-          if (pcell < 0) continue;
-          const bool split = (l == 1) ? child0_h[pcell] >= 0 : child_h[l - 1][pcell] >= 0;
-          if (split) continue;
-          const int a = f >> 1, side = f & 1;
-          // the six neighbours of the coarse leaf `pcell` on its own level l-1, for the ghost slopes (reading A21)
-          for (int b = 0; b < 3; b++)
-            for (int sd = 0; sd < 2; sd++) {
-              long long q;                                                 // >= 0: cell of level l-1; else a code
-              auto box = [&](int code) { const int bc = -1 - code; return bc == EMMA_RT_BC_INFLOW ? -5 : bc == EMMA_RT_BC_REFLECTIVE ? -2 - b : -1; };
-              if (l == 1) { q = nb0(pcell, b, sd); if (q < 0) q = box((int)q); }
-              else {
-                const long long po = pcell >> 3;
-                const int kk = pcell & 7, bit = (kk >> b) & 1;
-                if (sd != bit) q = (po << 3) | (kk ^ (1 << b));
-                else {
-                  const int pp = nbr_h[l - 1][po * 6 + 2 * b + sd];       // cell of level l-2
-                  if (pp < 0) q = box(pp);
-                  else {
-                    const int ch = (l == 2) ? child0_h[pp] : child_h[l - 2][pp];
-                    q = ch >= 0 ? (((long long)ch << 3) | (kk ^ (1 << b))) : (-16LL - pp);
-                  }
-                }
-              }
-              slot_refs_h[l].push_back((int)q);
-            }
-          for (int k = 0; k < 8; k++) {                                    // always 4 entries per oct side (kept aligned)
-            if (((k >> a) & 1) != side) continue;
-            if (l < s.nl && child_h[l][(o << 3) | k] >= 0)
-              return fail(h, EMMA_RT_EINVAL, "resolution jump > 1 at oct %lld of level %d (PAPER.md:75)", o, l);
-            slot_cell_h[l].push_back((int)((o << 3) | k));
-            slot_coarse_h[l].push_back(pcell);
-            slot_face_h[l].push_back((unsigned char)f);
-          }
-        }
-      h->n_slots[l] = (int)slot_cell_h[l].size();
-      if (h->n_slots[l]) {
-        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_cell[l], slot_cell_h[l].data(), slot_cell_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_coarse[l], slot_coarse_h[l].data(), slot_coarse_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_face[l], slot_face_h[l].data(), slot_face_h[l].size(), cudaMemcpyHostToDevice, h->st));
-        CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_refs[l], slot_refs_h[l].data(), slot_refs_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
-      }
-    }
-    // level-0 leaves next to a split cell, with the mask of the faces that look at one (sorted by cell id)
-    std::map<long long, unsigned> fix;
-    for (auto& kv : h->child_of[0])
-      for (int a = 0; a < 3; a++)
-        for (int side = 0; side < 2; side++) {
-          const long long q = nb0(kv.first, a, side);
-          if (q < 0 || child0_h[q] >= 0) continue;
-          fix[q] |= 1u << (2 * a + (1 - side));                   // q sees the split cell through its opposite face
-        }
-    for (auto& kv : fix) { fix_cell_h.push_back((int)kv.first); fix_mask_h.push_back((unsigned char)kv.second); }
-    h->n_fix = (int)fix_cell_h.size();
-    if (h->n_fix) {
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_cell, fix_cell_h.data(), fix_cell_h.size() * 4, cudaMemcpyHostToDevice, h->st));
-      CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.afix_mask, fix_mask_h.data(), fix_mask_h.size(), cudaMemcpyHostToDevice, h->st));
-    }
+    const int rc_topo = init_amr_topology(h, parent_h, child_h);
+    if (rc_topo != EMMA_RT_OK) return rc_topo;
   }
   CUDA_TRY(h, cudaStreamSynchronize(h->st));   // host staging vectors go out of scope below
 
