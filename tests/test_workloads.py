@@ -80,3 +80,29 @@ def test_config4_full_size_refinement_fraction_estimate():
     s = 1.5
     frac = 0.5 * erfc((log(8.0) + s * s / 2) / (s * sqrt(2)))
     assert frac == pytest.approx(0.0163, abs=0.002)
+
+
+def test_amr_standard_mesh_recipe():
+    """workloads.amr: seeded, jump-balanced (the oracle's AMR mode accepts it: PAPER.md:75), children densities average to
+    the parent, and the Z-order option permutes the octs without changing which cells are split."""
+    import oracle as O
+    from workloads.amr import make_amr_standard
+    for seed in (1, 2, 3):
+        w = make_amr_standard(n=12, G=1, levels=2, seed=seed, thresh1=2.0, thresh2=2.5)
+        w2 = make_amr_standard(n=12, G=1, levels=2, seed=seed, thresh1=2.0, thresh2=2.5)
+        assert all(np.array_equal(a, b) for a, b in zip(w.parent, w2.parent))
+        assert all(np.array_equal(a, b) for a, b in zip(w.n0, w2.n0))
+        assert 0 < len(w.parent[0]) < 12 ** 3 and len(w.parent[1]) > 0
+        assert len(set(w.parent[0].tolist())) == len(w.parent[0]) and len(set(w.parent[1].tolist())) == len(w.parent[1])
+        o = O.Oracle(w)
+        assert o.set_amr_transport(True) == O.OK
+        o.close()
+        for l in (1, 2):
+            kids = w.n0[l].astype(np.float64).reshape(-1, 8).mean(axis=1)
+            np.testing.assert_allclose(kids, w.n0[l - 1][w.parent[l - 1]].astype(np.float64), rtol=1e-6)
+        wm = make_amr_standard(n=12, G=1, levels=2, seed=seed, thresh1=2.0, thresh2=2.5, order="morton")
+        assert sorted(wm.parent[0].tolist()) == sorted(w.parent[0].tolist())
+        assert len(wm.parent[1]) == len(w.parent[1])
+        om = O.Oracle(wm)
+        assert om.set_amr_transport(True) == O.OK
+        om.close()
