@@ -48,7 +48,7 @@ def test_transport_one_step_config_like_state(n, G, bc):
     rep = compare(orc, gpu, w)
     assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
     do, dg = diags[0]
-    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6, abs=0)
     assert abs(dg["photons_outflow"] - do["photons_outflow"]) <= 1e-6 * do["photons_total"]
 
 
@@ -82,7 +82,7 @@ def test_transport_many_steps_chunks_and_wrap():
     rep = compare(orc, gpu, w, nf_floor=1e-4)
     assert rep["N"] <= 2e-5 and rep["F"] <= 2e-5, rep
     do, dg = diags[-1]
-    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)    # conservative to rounding
+    assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6, abs=0)    # conservative to rounding
 
 
 def test_P2_single_cell_example_on_gpu():
@@ -96,11 +96,11 @@ def test_P2_single_cell_example_on_gpu():
     assert rc == E.OK
     U = gpu.read(E.FIELD_U).reshape(n, n, n, 4).astype(np.float64)
     nu = 0.2
-    assert U[c, c, c, 0] == pytest.approx((1 - 3 * nu) * N0, rel=1e-6)
-    assert U[c, c, c + 1, 0] == pytest.approx(nu * N0 / 2, rel=1e-6)
-    assert U[c, c, c + 1, 1] == pytest.approx(nu * w.c_red * N0 / 6, rel=1e-6)
-    assert U[c - 1, c, c, 3] == pytest.approx(-nu * w.c_red * N0 / 6, rel=1e-6)
-    assert U[..., 0].sum() == pytest.approx(N0, rel=1e-6)
+    assert U[c, c, c, 0] == pytest.approx((1 - 3 * nu) * N0, rel=1e-6, abs=0)
+    assert U[c, c, c + 1, 0] == pytest.approx(nu * N0 / 2, rel=1e-6, abs=0)
+    assert U[c, c, c + 1, 1] == pytest.approx(nu * w.c_red * N0 / 6, rel=1e-6, abs=0)
+    assert U[c - 1, c, c, 3] == pytest.approx(-nu * w.c_red * N0 / 6, rel=1e-6, abs=0)
+    assert U[..., 0].sum() == pytest.approx(N0, rel=1e-6, abs=0)
 
 
 def test_P3_free_streaming_beam_on_gpu():
@@ -153,8 +153,8 @@ def test_chemistry_off_sources_add_S_dt():
     rep = compare(orc, gpu, w)
     assert rep["N"] <= TOL_NF and rep["F"] <= TOL_NF, rep
     for do, dg in diags:
-        assert dg["photons_injected"] == pytest.approx(do["photons_injected"], rel=1e-6)
-        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6)
+        assert dg["photons_injected"] == pytest.approx(do["photons_injected"], rel=1e-6, abs=0)
+        assert dg["photons_total"] == pytest.approx(do["photons_total"], rel=1e-6, abs=0)
 
 
 # ------------------------------------------------------------------------------------------- coupled, one step
@@ -181,12 +181,12 @@ def test_coupled_one_step_random_state(n, G, otsa):
     assert rep["N"] <= 5e-5 and rep["F"] <= 5e-5, rep
     # diagnostics agree with the oracle's
     for k in ("photons_total", "photons_injected", "photons_absorbed"):
-        assert dg[k] == pytest.approx(do[k], rel=2e-5), k
+        assert dg[k] == pytest.approx(do[k], rel=2e-5, abs=0), k
     if not otsa:
-        assert dg["photons_recomb_emitted"] == pytest.approx(do["photons_recomb_emitted"], rel=1e-4)
+        assert dg["photons_recomb_emitted"] == pytest.approx(do["photons_recomb_emitted"], rel=1e-4, abs=0)
     assert abs(dg["subcycles_total"] - do["subcycles_total"]) <= 1e-3 * do["subcycles_total"]
     assert dg["subcycles_max"] == do["subcycles_max"] or rep["flips"] > 0
-    assert dg["dtau_min"] == pytest.approx(do["dtau_min"], rel=1e-3)
+    assert dg["dtau_min"] == pytest.approx(do["dtau_min"], rel=1e-3, abs=0)
 
 
 def test_isothermal_mode_and_equilibrium_on_gpu():

@@ -46,7 +46,7 @@ def test_closure_trace_and_limits():
         n /= np.linalg.norm(n)
         f = rng.uniform(0, 1.3)                       # > 1 exercises the clip
         P = O.closure([N, *(f * C_RED * N * n)], C_RED)
-        assert np.trace(P) == pytest.approx(N, rel=1e-14)
+        assert np.trace(P) == pytest.approx(N, rel=1e-14, abs=0)
         assert np.allclose(P, P.T, rtol=0, atol=1e-16 * N)
         # eigen-structure: n is an eigenvector with eigenvalue chi N
         chi = O.chi(min(f, 1.0))
@@ -97,9 +97,9 @@ def test_P2_single_cell_worked_example(oracle_mod):
             exp[c + s * dz, c + s * dy, c + s * dx, 1 + d_] = s * fl
     assert np.allclose(U[..., 0], exp[..., 0], rtol=1e-14, atol=0)
     assert np.allclose(U[..., 1:], exp[..., 1:], rtol=1e-14, atol=1e-14 * fl)
-    assert U[..., 0].sum() == pytest.approx(N0, rel=1e-14)
+    assert U[..., 0].sum() == pytest.approx(N0, rel=1e-14, abs=0)
     # reduced flux of the neighbours is 1/3
-    assert abs(U[c, c, c + 1, 1]) / (w.c_red * U[c, c, c + 1, 0]) == pytest.approx(1 / 3, rel=1e-13)
+    assert abs(U[c, c, c + 1, 1]) / (w.c_red * U[c, c, c + 1, 0]) == pytest.approx(1 / 3, rel=1e-13, abs=0)
 
 
 # ---------------------------------------------------------------- P3 free-streaming beam
@@ -135,7 +135,7 @@ def test_P3_free_streaming_beam_binomial(oracle_mod):
     x = np.arange(n)
     cen0 = (prof * x).sum() / prof.sum()
     cen = (U[0, 0, :, 0] * x).sum() / U[0, 0, :, 0].sum()
-    assert cen - cen0 == pytest.approx(k * nu, rel=1e-12)                           # speed = c~
+    assert cen - cen0 == pytest.approx(k * nu, rel=1e-12, abs=0)                           # speed = c~
 
 
 # ---------------------------------------------------------------- P4 photon budget
@@ -163,7 +163,7 @@ def test_P4_photon_budget_closes_every_step(oracle_mod, case):
         rhs = d["photons_injected"] - d["photons_absorbed"] + d["photons_recomb_emitted"] - d["photons_outflow"]
         scale = max(d["photons_total"], d["photons_injected"])
         assert abs((d["photons_total"] - prev) - rhs) <= 1e-12 * scale
-        assert d["photons_injected"] == pytest.approx(w.src_Q.sum() * w.dt, rel=1e-13)   # A12: sum Q dt exactly
+        assert d["photons_injected"] == pytest.approx(w.src_Q.sum() * w.dt, rel=1e-13, abs=0)   # A12: sum Q dt exactly
         saw_out |= d["photons_outflow"] > 0
         if case == "non_otsa":
             assert d["photons_recomb_emitted"] > 0
@@ -187,11 +187,11 @@ def test_P5_absorption_decay_and_dtau_to_zero(oracle_mod):
         assert rc == O.OK and out.nsub == 1 and out.nhalv == 0
         den = 1 + C_RED * gr["sigma_N"][0] * (1 - x) * n0 * dt
         assert np.allclose(U1, U / den, rtol=1e-15)
-        assert out.absorbed == pytest.approx((U[0, 0] - U1[0, 0]), rel=1e-12)       # sink counts what N lost
-        assert O.temperature(e1, x1, n0) == pytest.approx(T, rel=1e-14)            # isothermal mode holds T
+        assert out.absorbed == pytest.approx((U[0, 0] - U1[0, 0]), rel=1e-12, abs=0)       # sink counts what N lost
+        assert O.temperature(e1, x1, n0) == pytest.approx(T, rel=1e-14, abs=0)            # isothermal mode holds T
         x, e, U = x1, e1, U1
     rc, x1, e1, U1, out = O.chem_cell(ph, 1e-9, n0, x, e, U)
-    assert np.allclose(U1, U, rtol=1e-14) and x1 == pytest.approx(x, rel=1e-14)
+    assert np.allclose(U1, U, rtol=1e-14) and x1 == pytest.approx(x, rel=1e-14, abs=0)
 
 
 # ---------------------------------------------------------------- P6 collisional equilibrium
@@ -215,7 +215,7 @@ def test_P6_collisional_ionisation_equilibrium(oracle_mod, otsa):
         for _ in range(400):
             rc, x, e, U, out = O.chem_cell(ph, dt, n0, x, e, U)
             U[:] = 0.0
-        assert x == pytest.approx(xeq, rel=1e-10)
+        assert x == pytest.approx(xeq, rel=1e-10, abs=0)
 
 
 # ---------------------------------------------------------------- P7 photo-ionisation equilibrium
@@ -234,8 +234,8 @@ def test_P7_photoionisation_equilibrium(oracle_mod):
     e = O.energy(T, x, n0)
     for _ in range(3000):
         rc, x, e, U, out = O.chem_cell(ph, 2e13, n0, x, e, U, S=[S])
-    assert x == pytest.approx(xeq, rel=1e-9)
-    assert U[0, 0] == pytest.approx(Neq, rel=1e-9)
+    assert x == pytest.approx(xeq, rel=1e-9, abs=0)
+    assert U[0, 0] == pytest.approx(Neq, rel=1e-9, abs=0)
     assert 0 < xeq < 1
 
 
@@ -249,8 +249,8 @@ def _stromgren_numbers(n0=1e-3, Q=5e48, T=1e4):
 def test_P8_stromgren_textbook_numbers(oracle_mod):
     """north_star: R_s = (3Q / 4 pi n_H^2 alpha_B)^(1/3); with alpha_B(1e4 K) = 2.59e-13 (textbook) this is 5.4 kpc."""
     Rs, trec = _stromgren_numbers()
-    assert O.rates(1e4)["alphaB"] == pytest.approx(2.59e-13, rel=2e-3)       # Osterbrock's case-B value
-    assert O.rates(1e4)["alphaA"] == pytest.approx(4.18e-13, rel=4e-2)       # Osterbrock's case-A value
+    assert O.rates(1e4)["alphaB"] == pytest.approx(2.59e-13, rel=2e-3, abs=0)       # Osterbrock's case-B value
+    assert O.rates(1e4)["alphaA"] == pytest.approx(4.18e-13, rel=4e-2, abs=0)       # Osterbrock's case-A value
     assert Rs / CGS.kpc == pytest.approx(5.4, abs=0.05)
     assert trec / CGS.Myr == pytest.approx(122.3, abs=0.5)
 
@@ -276,7 +276,7 @@ def test_P8_ionised_radius_converges_to_stromgren(oracle_mod):
         r_I = (3 * x.sum() * w.dx ** 3 / (4 * math.pi)) ** (1 / 3)
         r_rec = (3 * (x * x).sum() * w.dx ** 3 / (4 * math.pi)) ** (1 / 3)
         ana = Rs * (1 - math.exp(-frac)) ** (1 / 3)
-        assert r_rec == pytest.approx(ana, rel=0.09), (frac, r_rec / ana)
+        assert r_rec == pytest.approx(ana, rel=0.09, abs=0), (frac, r_rec / ana)
         assert 0.98 * ana < r_I < 1.12 * ana, (frac, r_I / ana)
     assert r_rec / Rs == pytest.approx(0.994, abs=0.03)          # (1 - e^-4)^(1/3) = 0.994
     assert done > 1000
@@ -296,11 +296,11 @@ def test_P8_early_time_config1(oracle_mod):
     Rs = (3 * 5e48 / (4 * math.pi * 1e-6 * aB)) ** (1 / 3)
     t = d["t_sim"]
     V_ana = 4 * math.pi / 3 * Rs ** 3 * (1 - math.exp(-t * aB * 1e-3)) + 1.2e-3 * w.L ** 3
-    assert V_ion == pytest.approx(V_ana, rel=0.08)
+    assert V_ion == pytest.approx(V_ana, rel=0.08, abs=0)
     # P9: no-cooling temperature bound  T <= (Sigma_E/sigma_N) / (3 k_B)   (A8, A10)
     SigE = w.sigma_E[0] * w.E_mean[0] - w.sigma_N[0] * 13.6 * CGS.eV
     Tmax = SigE / w.sigma_N[0] / (3 * CGS.k_B)
-    assert Tmax == pytest.approx(24447, rel=2e-3)
+    assert Tmax == pytest.approx(24447, rel=2e-3, abs=0)
     assert T.max() <= Tmax and T.max() > 0.97 * Tmax
 
 
@@ -309,9 +309,9 @@ def test_A10_temperature_energy_roundtrip(oracle_mod):
     rng = np.random.default_rng(3)
     for _ in range(100):
         T, x, n0 = 10 ** rng.uniform(1, 6), rng.uniform(0, 1), 10 ** rng.uniform(-6, 2)
-        assert O.temperature(O.energy(T, x, n0), x, n0) == pytest.approx(T, rel=1e-15)
+        assert O.temperature(O.energy(T, x, n0), x, n0) == pytest.approx(T, rel=1e-15, abs=0)
     # fully ionised hydrogen: e = 3 n k T (two particles per atom)
-    assert O.energy(1e4, 1.0, 1.0) == pytest.approx(3 * CGS.k_B * 1e4, rel=1e-15)
+    assert O.energy(1e4, 1.0, 1.0) == pytest.approx(3 * CGS.k_B * 1e4, rel=1e-15, abs=0)
 
 
 # ---------------------------------------------------------------- A9: the 10 % rule
@@ -530,10 +530,10 @@ def test_H1_wavespeeds_are_the_extreme_eigenvalues_of_the_flux_jacobian(oracle_m
 def test_H2_wavespeed_limits_and_scaling(oracle_mod):
     c = C_RED
     lo, hi = O.m1_wavespeeds([2.0, 0, 0, 0], c, 1)
-    assert lo == pytest.approx(-c / math.sqrt(3), rel=1e-14) and hi == pytest.approx(c / math.sqrt(3), rel=1e-14)
-    assert O.m1_wavespeeds([1.0, c, 0, 0], c, 0) == pytest.approx((c, c), rel=1e-14)        # free streaming along d
+    assert lo == pytest.approx(-c / math.sqrt(3), rel=1e-14, abs=0) and hi == pytest.approx(c / math.sqrt(3), rel=1e-14, abs=0)
+    assert O.m1_wavespeeds([1.0, c, 0, 0], c, 0) == pytest.approx((c, c), rel=1e-14, abs=0)        # free streaming along d
     assert O.m1_wavespeeds([1.0, c, 0, 0], c, 2) == pytest.approx((0.0, 0.0), abs=1e-9 * c)  # ... across d
-    assert O.m1_wavespeeds([1.0, -3 * c, 0, 0], c, 0) == pytest.approx((-c, -c), rel=1e-14)  # f clipped to 1
+    assert O.m1_wavespeeds([1.0, -3 * c, 0, 0], c, 0) == pytest.approx((-c, -c), rel=1e-14, abs=0)  # f clipped to 1
     assert O.m1_wavespeeds([0.0, 1.0, 0, 0], c, 0) == pytest.approx((-c / math.sqrt(3), c / math.sqrt(3)))  # N<=0: f=0
     # |l| <= c always, lmin <= lmax, and the pair agrees with the independent cancellation-free transcription
     rng = np.random.default_rng(3)
@@ -562,14 +562,14 @@ def test_H3_hll_single_cell_worked_example(oracle_mod):
     assert rc == O.OK
     U = o.read(O.F_U).reshape(n, n, n, 4)
     nu = c * w.dt / w.dx
-    assert U[2, 4, 3, 0] == pytest.approx(1 - math.sqrt(3) * nu, rel=1e-13)
+    assert U[2, 4, 3, 0] == pytest.approx(1 - math.sqrt(3) * nu, rel=1e-13, abs=0)
     for (dz, dy, dx_), comp in (((0, 0, 1), 1), ((0, 0, -1), 1), ((0, 1, 0), 2), ((0, -1, 0), 2), ((1, 0, 0), 3), ((-1, 0, 0), 3)):
         v = U[2 + dz, 4 + dy, 3 + dx_]
         sgn = dz + dy + dx_
-        assert v[0] == pytest.approx(nu / (2 * math.sqrt(3)), rel=1e-13)
-        assert v[comp] == pytest.approx(sgn * nu * c / 6, rel=1e-13)
+        assert v[0] == pytest.approx(nu / (2 * math.sqrt(3)), rel=1e-13, abs=0)
+        assert v[comp] == pytest.approx(sgn * nu * c / 6, rel=1e-13, abs=0)
         assert np.abs(np.delete(v[1:], comp - 1)).max() == 0.0
-    assert U[..., 0].sum() == pytest.approx(1.0, rel=1e-13)
+    assert U[..., 0].sum() == pytest.approx(1.0, rel=1e-13, abs=0)
 
 
 def test_H4_hll_free_streaming_beam_is_exact_upwind(oracle_mod):
@@ -623,7 +623,7 @@ def test_H5_hll_bruteforce_transcription_and_conservation(oracle_mod, n, G, seed
         # radicand differ by ~sqrt(eps)
         assert np.abs(U[..., 0] - Ub[g][..., 0]).max() <= 1e-8 * scale
         assert np.abs(U[..., 1:] - Ub[g][..., 1:]).max() <= 1e-8 * c * scale
-        assert U[..., 0].sum() == pytest.approx(U0[g, :, 0].astype(np.float64).sum(), rel=1e-12)
+        assert U[..., 0].sum() == pytest.approx(U0[g, :, 0].astype(np.float64).sum(), rel=1e-12, abs=0)
 
 
 def test_H6_hll_is_less_diffusive_than_glf(oracle_mod):
@@ -643,7 +643,7 @@ def test_H6_hll_is_less_diffusive_than_glf(oracle_mod):
         N = o.read(O.F_N).reshape(n, n, n)
         inside = N[6:10, 6:10, :].sum()
         leak[name] = 1.0 - inside / N.sum()
-        assert N.sum() == pytest.approx(16.0 * n, rel=1e-12)
+        assert N.sum() == pytest.approx(16.0 * n, rel=1e-12, abs=0)
     assert leak["hll"] < 0.6 * leak["glf"], leak
 
 
