@@ -27,7 +27,8 @@ static const double E_HI = 13.6 * 1.602176634e-12;   /* "E_13.6", PAPER.md:266 *
  * ---------------------------------------------------------------------------------------------- */
 
 /* A2: chi is only described by its limits 1/3 and 1; the formula is Levermore's,
- * from the literature the paper cites.  Interior values: parity unpinned. */
+ * from the literature the paper cites.  Interior values are pinned by tests/test_oracle_literature.py:
+ * chi is the Eddington factor of an isotropic field boosted by beta, f = 4 beta/(3 + beta^2), chi = (1 + 3 beta^2)/(3 + beta^2). */
 double orc_chi(double f)
 {
   return (3.0 + 4.0 * f * f) / (5.0 + 2.0 * sqrt(4.0 - 3.0 * f * f));
@@ -167,7 +168,10 @@ void orc_transport_stencil_flux(int flux, double c, double dt, double dx, const 
 /* ------------------------------------------------------------------------------------------------
  * Atomic rates (A11).  PAPER.md:312 cites Theuns et al. 1998 and Hui & Gnedin 1997 without printing
  * anything; these are literature fits restated as THE definition used by both sides.
- * Coefficients: parity unpinned (only sanity values are pinned in tests).
+ * Pinned by tests/test_oracle_literature.py against other sources: Osterbrock & Ferland's tabulated alpha_A, alpha_B and
+ * recombination-cooling coefficients at 5e3 / 1e4 / 2e4 K, Voronov's (1997) and Cen's (1992) / Theuns et al.'s (1998)
+ * collisional ionisation rate over 5e3 .. 1e6 K, Lambda_ci = 13.6 eV x beta, Cen's excitation cooling, the Rybicki &
+ * Lightman free-free emissivity; a mutation test shows that a slipped exponent or prefactor in any line below fails one.
  * ---------------------------------------------------------------------------------------------- */
 void orc_rates(double T, double* alphaA, double* alphaB, double* beta, double* cool_HI,
                double* cool_HII_A, double* cool_HII_B)

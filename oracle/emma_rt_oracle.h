@@ -6,9 +6,11 @@
  * call it.  It shares no code with paper_1508_07888_b200/ (the CUDA path) and neither includes
  * the other.
  *
- * Unpinned parts:  chi(f) between its two printed limits and the atomic-rate
- * coefficients (PAPER.md:312 cites Theuns et al. 1998 / Hui & Gnedin 1997, neither printed nor in
- * the container) -- "parity unpinned" for orc_chi() interior values and orc_rates() coefficients.
+ * Pins: every function has one.  The two literature formulas the paper cites without printing
+ * -- chi(f) between its printed limits (Levermore via PAPER.md:197) and the atomic rates / cooling
+ * functions -- are pinned against other sources in tests/test_oracle_literature.py (boosted isotropic
+ * field; Osterbrock & Ferland tables, Voronov 1997, Cen 1992 / Theuns et al. 1998, Rybicki & Lightman), as is the
+ * H I cross-section of the group constants (exact hydrogenic closed form).  No function is "parity unpinned".
  */
 #ifndef EMMA_RT_ORACLE_H
 #define EMMA_RT_ORACLE_H
