@@ -28,8 +28,35 @@ if ROOT not in sys.path:
 
 METRIC = "cell_group_updates_per_s"
 UNIT = "cell-group updates/s"
-ORACLE_SAMPLE_N = 128
-ORACLE_SAMPLE_STEPS = 16          # ~10-20 s of host time at 128^3 x 3 groups
+ORACLE_SAMPLE_N = 128             # the oracle's bounded sample of config 5: 128^3 x 3 groups (0.3 s per step on 16 cores)
+ORACLE_SAMPLE_STEPS = 30          # at most this many timed steps (~10 s of host time), after the same warm-up as the GPU arm
+ORACLE_1T_N = 64                  # single-thread figure ("one GPU against one CPU core"): 64^3 x 3 groups
+ORACLE_1T_STEPS = 8
+
+
+def cpu_model():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def time_oracle_single_thread(variant, warmup, config=5):
+    """The same oracle with OMP_NUM_THREADS=1 (a fresh process: OpenMP reads it at start-up) on a smaller sample."""
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "v, secs, cores, d = bench.time_oracle(%d, %d, %d, %r, %d); print(json.dumps([v, secs, cores]))"
+            % (ROOT, ORACLE_1T_N, ORACLE_1T_STEPS, warmup, variant, config))
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True,
+                             text=True, timeout=600, check=True).stdout.strip().splitlines()[-1]
+        v, secs, cores = json.loads(out)
+        return {"value": v, "unit": UNIT, "cores": int(cores), "seconds": secs,
+                "sample": "config 5%s recipe at %d^3 x 3 groups, steps %d..%d" % (variant, ORACLE_1T_N, warmup + 1, warmup + ORACLE_1T_STEPS)}
+    except Exception as e:                                            # a reported baseline, never fatal
+        return {"error": str(e)[:200]}
 
 
 def log(*a):
@@ -157,20 +184,91 @@ def run_reference(args):
         print(json.dumps(line), flush=True)
         return
     n = ORACLE_SAMPLE_N if args.config == 5 else 96
-    steps, warm = max(1, min(args.steps, 5)), min(args.warmup, 1)
-    # per "step" of this arm: one oracle step on the n^3 sample; the whole run stays within a few minutes
+    # per "step" of this arm: one oracle step on the n^3 sample, timed over the SAME step range as the GPU arm (W untimed
+    # warm-up steps from the seeded initial state, then K timed steps, K capped so the run stays within a few minutes)
+    steps, warm = max(1, min(args.steps, ORACLE_SAMPLE_STEPS)), max(0, args.warmup)
     val, secs, cores, d = time_oracle(n, steps, warm, args.variant, args.config)
     label = ("5" + args.variant) if args.config == 5 else "4 (CRTA, 2 refined levels)"
-    sample = "config %s recipe at %d^3 x 3 groups (a bounded sample of the full grid), %d coupled steps, fp64 C oracle with OpenMP" % (
-        label, n, steps)
+    sample = ("config %s recipe at %d^3 x 3 groups (a bounded sample of the full grid), steps %d..%d from the seeded initial state, "
+              "fp64 C oracle with OpenMP" % (label, n, warm + 1, warm + steps))
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "BASELINE config %s sampled at %d^3 (oracle on host cores)" % (label, n)},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model(), "step_range": [warm + 1, warm + steps],
+                             "subcycles_mean_last_step": d["subcycles_total"] / float(n ** 3) if args.config == 5 else None},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+# Issue-rate ceiling of the sub-cycling tail: SASS instructions of chem_tail_kernel<3> per accepted
+# sub-step (rates at T^p 66 incl. 16 MUFU, first guess + commit + loop 64) and per attempt of Eq. 43-48 (97 incl. 4 MUFU),
+# counted with cuobjdump on this build; a B200 issues 4 warp instructions per SM and clock.
+TAIL_INSTR_PER_SUBSTEP = 130
+TAIL_INSTR_PER_ATTEMPT = 97
+
+
+def run_from_initial_state(E, torch, w, dev, K, units_per_step, sm_mhz, **kw):
+    """K coupled steps from step 0 on a fresh handle, NO warm-up: the regime in which cells really sub-cycle (config 5:
+    random initial T).  One step per call with its diagnostics read back, so per-step kernel times and
+    sub-cycle counts are known; the host gap between steps (one 200-byte D2H + event reads) is inside the timing."""
+    gpu = E.EmmaRT(w, device=dev, **kw)
+    gpu.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    steps = []
+    torch.cuda.synchronize(dev)
+    e0.record()
+    for _ in range(K):
+        rc, d = gpu.step(w.dt, 1, diag=True)
+        assert rc == E.OK, (rc, gpu.last_error())
+        steps.append((d, gpu.profile(True)))
+    e1.record()
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    gpu.close()
+    cells = units_per_step // w.G
+    tail_ms = [p["chem_tail"][0] for _, p in steps]
+    main_ms = [p["fused"][0] + p["chem_main"][0] + p["transport"][0] for _, p in steps]
+    # evaluations of Eq. 43-48 in the tail = accepted sub-steps of the deferred cells + their rejected (halved) attempts
+    sub_tail = [d["subcycles_total"] - (cells - d["n_deferred"]) for d, _ in steps]
+    evals = [st + d["halvings_total"] for st, (d, _) in zip(sub_tail, steps)]
+    first = [i for i in range(len(steps)) if tail_ms[i] > 0.05][:6] or [0]
+    ev, tm = sum(evals[i] for i in first), sum(tail_ms[i] for i in first) * 1e-3
+    instr = sum(sub_tail[i] * TAIL_INSTR_PER_SUBSTEP + evals[i] * TAIL_INSTR_PER_ATTEMPT for i in first)
+    peak_lane_instr = 148 * 4 * 32 * (sm_mhz or 1965.0) * 1e6
+    d1 = steps[0][0]
+    return {"steps": K, "warmup": 0, "ms_per_step": ms / K, "value": units_per_step * K / (ms * 1e-3), "unit": UNIT,
+            "chem_tail_ms_first_steps": [float("%.4g" % v) for v in tail_ms[:8]],
+            "transport_chem_pass_ms_first_steps": [float("%.4g" % v) for v in main_ms[:8]],
+            "subcycles_step1": {"mean": d1["subcycles_total"] / float(cells), "max": d1["subcycles_max"],
+                                "deferred": d1["n_deferred"], "halvings": d1["halvings_total"]},
+            "tail": {"steps_counted": [i + 1 for i in first], "evaluations": int(ev), "evaluations_per_s": ev / tm if tm > 0 else None,
+                     "bound": "alu", "issue_ceiling_evaluations_per_s": peak_lane_instr * ev / instr if instr else None,
+                     "frac_of_issue_ceiling": (instr / peak_lane_instr) / tm if tm > 0 else None,
+                     "note": "ceiling = 148 SMs x 4 warp instr/clk x 32 lanes x SM clock / (130 instr per accepted sub-step + 97 "
+                             "per attempt), every lane busy"}}
+
+
+def run_sub_record(E, torch, w, dev, K, W, units_per_step, **kw):
+    """A short device-resident run of another workload (rows a-5 / NEXT-2 of SURVEY.md section 8 at size): W warm-up steps,
+    K timed ones, per-kernel CUDA-event times."""
+    gpu = E.EmmaRT(w, device=dev, **kw)
+    rc, _ = gpu.step(w.dt, W, diag=False)
+    assert rc == E.OK, gpu.last_error()
+    gpu.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    e0.record()
+    rc, d = gpu.step(w.dt, K, diag=True)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    assert rc == E.OK, (rc, gpu.last_error())
+    ms = e0.elapsed_time(e1)
+    prof = gpu.profile(False)
+    gpu.close()
+    return ms, prof, d
 
 
 def replica_seed(config, rank, world):
@@ -328,6 +426,58 @@ def run_ours(args):
         torch.cuda.empty_cache()
         gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr, flux=flux)
 
+    # ---------------- the hard regime: the same workload from the seeded initial state, no warm-up (sub-cycling transient)
+    init_leg = None
+    if args.config == 5 and not amr and not args.skip_initial_state:
+        if gpu is not None:
+            gpu.close()
+            gpu = None
+            torch.cuda.empty_cache()
+        init_leg = run_from_initial_state(E, torch, w, dev, K, units_per_step, clk.get("sm_mhz"),
+                                          fused=0 if args.unfused else 1, flux=flux)
+        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr, flux=flux)
+
+    # ---------------- rows a-5 (CRTA, BASELINE config 4) and NEXT-2 (standard AMR) at size, as short sub-records
+    extra = {}
+    if args.config == 5 and not amr and not args.skip_extra and world == 1:
+        gpu.close()
+        gpu = None
+        torch.cuda.empty_cache()
+        try:
+            w4 = make_config(4)
+            u4 = leaf_count(w4) * w4.G
+            ms4, p4, d4 = run_sub_record(E, torch, w4, dev, min(K, 20), W, u4)
+            extra["config4_crta"] = {
+                "workload": "BASELINE config 4: 256^3 coarse + 2 refined levels (CRTA), 3 groups, %d leaves, %d sources" % (leaf_count(w4), len(w4.src_pos)),
+                "steps": min(K, 20), "warmup": W, "ms_per_step": ms4 / min(K, 20), "value": u4 * min(K, 20) / (ms4 * 1e-3),
+                "unit": "leaf-" + UNIT, "kernels_ms_per_step": {k: v[0] / min(K, 20) for k, v in p4.items() if v[1]},
+                "subcycles_max_last_step": d4["subcycles_max"], "deferred_last_step": d4["n_deferred"]}
+            del w4
+        except Exception as e:                                        # a sub-record never costs the headline line
+            extra["config4_crta"] = {"error": str(e)[:300]}
+        try:
+            from workloads.amr import make_amr_standard
+            wa = make_amr_standard(n=256, G=3, levels=2)
+            ca = [wa.n ** 3] + [8 * len(p) for p in wa.parent]
+            la = [c - s_ for c, s_ in zip(ca, [len(p) for p in wa.parent] + [0])]
+            ua = sum(la[l] << l for l in range(3)) * wa.G
+            Ka = min(K, 10)
+            msa, pa, da = run_sub_record(E, torch, wa, dev, Ka, W, ua, amr_transport=1)
+            ref_sweeps = sum(la[l] << l for l in range(1, 3))
+            extra["amr_standard"] = {
+                "workload": "standard AMR scheme (SURVEY 8f NEXT-2, reading A21): 256^3 + 2 refined levels, 3 groups, cells per level %s, "
+                            "leaves per level %s; a level-l leaf counts 2^l times per coarse step" % (ca, la),
+                "steps": Ka, "warmup": W, "ms_per_step": msa / Ka, "value": ua * Ka / (msa * 1e-3), "unit": "leaf-" + UNIT,
+                "kernels_ms_per_step": {k: v[0] / Ka for k, v in pa.items() if v[1]},
+                "amr_transport": {"algorithmic_bytes_per_step": 32.0 * wa.G * ref_sweeps,
+                                  "GBps": 32.0 * wa.G * ref_sweeps * Ka / (pa["amr_transport"][0] * 1e-3) / 1e9,
+                                  "frac": 32.0 * wa.G * ref_sweeps * Ka / (pa["amr_transport"][0] * 1e-3) / 1e9 / peak}}
+            del wa
+        except Exception as e:
+            extra["amr_standard"] = {"error": str(e)[:300]}
+        torch.cuda.empty_cache()
+        gpu = E.EmmaRT(w, device=dev, fused=0 if args.unfused else 1, amr_transport=amr, flux=flux)
+
     # ---------------- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
     Ke = max(1, min(K, args.e2e_steps))
     hU = [torch.from_numpy(np.ascontiguousarray(w.U0[g])).pin_memory() if w.U0 is not None
@@ -378,18 +528,26 @@ def run_ours(args):
                "sample": "standard-AMR recipe at 32^3 coarse + 2 levels x 3 groups, 6 coarse steps, fp64 C oracle (the AMR "
                          "recursion of the oracle is serial)"}
     elif rank == 0 and world == 1 and not args.skip_cpu_baseline:
-        val, secs, cores, _ = time_oracle(ORACLE_SAMPLE_N if args.config == 5 else 96, ORACLE_SAMPLE_STEPS, 0, args.variant, args.config)
-        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
-               "sample": "config %s recipe at %d^3 x 3 groups, %d coupled steps from the initial state, fp64 C oracle, "
-                         "OpenMP on all host cores" % ("5" + args.variant if args.config == 5 else "4 (CRTA, 2 levels)",
-                                                       ORACLE_SAMPLE_N if args.config == 5 else 96, ORACLE_SAMPLE_STEPS)}
+        osteps = max(1, min(K, ORACLE_SAMPLE_STEPS))
+        on = ORACLE_SAMPLE_N if args.config == 5 else 96
+        val, secs, cores, od = time_oracle(on, osteps, W, args.variant, args.config)
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs, "cpu_model": cpu_model(),
+               "step_range": [W + 1, W + osteps],
+               "sample": "config %s recipe at %d^3 x 3 groups, steps %d..%d from the seeded initial state (the GPU arm's timed "
+                         "range: %d warm-up steps first), fp64 C oracle as it stands, OpenMP on all host cores"
+                         % ("5" + args.variant if args.config == 5 else "4 (CRTA, 2 levels)", on, W + 1, W + osteps, W),
+               # the paper's own convention is one graphics device against ONE CPU core
+               "single_thread": time_oracle_single_thread(args.variant, W) if args.config == 5 else None}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic",
                 "config": {"workload": ("BASELINE config 5%s: %d^3 x %d groups, lognormal sigma_ln=1.0, %d sources, "
-                                        "random x,T, coupled RT+chemistry" % (args.variant, n, G, len(w.src_pos)))
+                                        "random x,T, coupled RT+chemistry; STEADY STATE: timed after %d warm-up steps, ~%.3f accepted "
+                                        "sub-steps per cell (the sub-cycling transient of the random initial T falls in the warm-up: "
+                                        "see coupled_from_initial_state for the same workload from step 0)"
+                                        % (args.variant, n, G, len(w.src_pos), W, diag["subcycles_total"] / float(leaf_count(w))))
                            if args.config == 5 and not amr else
                            ("standard AMR scheme (SURVEY 8f NEXT-2, reading A21): %d^3 coarse + 2 refined levels on a jump-balanced "
                             "config-4-like mesh, %d groups, cells per level %s, leaves per level %s, %d sources; value counts "
@@ -402,6 +560,7 @@ def run_ours(args):
                            "flux": "hll" if args.hll else "glf",
                            "parallelism": "replicas" if world > 1 else "single"},
                 "roofline": roofline, "kernels": kern, "transport_only": tr, "transport_only_hll": hll, "e2e": e2e, "cpu_baseline": cpu,
+                "coupled_from_initial_state": init_leg, "sub_records": extra or None,
                 "gpu_launches": int(launches), "clocks": clk,
                 "subcycles": {"mean_last_step": diag["subcycles_total"] / float(leaf_count(w)), "max_last_step": diag["subcycles_max"],
                               "deferred_last_step": diag["n_deferred"]}}
@@ -428,6 +587,8 @@ def main():
                     help="the standard (non-CRTA) AMR scheme on a jump-balanced 256^3 + 2 levels mesh (SURVEY 8f NEXT-2)")
     ap.add_argument("--skip-transport-only", action="store_true")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
+    ap.add_argument("--skip-initial-state", action="store_true", help="skip the no-warm-up leg (coupled_from_initial_state)")
+    ap.add_argument("--skip-extra", action="store_true", help="skip the config-4 (CRTA) and standard-AMR sub-records")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -27,7 +27,16 @@
  *   - Errors: every entry point returns EMMA_RT_OK or a negative code; nothing throws, aborts or prints.
  *     `emma_rt_last_error` gives a handle-owned message.  There is no CPU fallback: without a CUDA device
  *     `emma_rt_init` returns EMMA_RT_ECUDA.
- *   - Threading: one handle <-> one stream, not re-entrant.
+ *   - Threading: one handle <-> one stream, not re-entrant.  A process may hold handles on several devices: every entry
+ *     point that launches work makes the handle's device current (cudaSetDevice) and leaves it current.
+ *   - Input validation: `emma_rt_init` and `emma_rt_write` with HOST buffers refuse (EMMA_RT_EINVAL) n0 <= 0, T <= 0,
+ *     x outside [0, 1] and non-finite n0, x, T; a non-finite U is accepted and reported by the next step
+ *     (EMMA_RT_ENONFINITE).  Device-buffer writes are stream-ordered and not validated (a NaN stays a NaN).
+ *   - Environment: five tuning knobs for experiments are read ONCE, by `emma_rt_init`, and ignored when unset, not a
+ *     number or out of range: EMMA_RT_TUNE_NZC (z-chunks per tile column of the dense passes, 1..n), EMMA_RT_TUNE_NST
+ *     (stages of the transport TMA ring: 4, 6, 8), EMMA_RT_TUNE_TMA (0: non-TMA transport kernel), EMMA_RT_TUNE_FUSED
+ *     (0: two-pass schedule), EMMA_RT_TUNE_CHEMCTAS (persistent CTAs per SM of the chemistry main pass, 1..32).  None
+ *     changes results beyond fp32 rounding order of nothing (same arithmetic); `emma_rt_step` reads no environment.
  *   - Sync: `emma_rt_step` only enqueues work unless `diag_last != NULL` (then it waits for the stream);
  *     `emma_rt_read` / `emma_rt_write` with host buffers wait for the stream.
  */
@@ -154,6 +163,7 @@ EMMA_RT_API int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos
 EMMA_RT_API double emma_rt_dt_cfl(const emma_rt* h, double courant);
 
 /* Advance n_steps coupled steps of size dt.  dt > dx/(3 c_red) -> EMMA_RT_ECFL, state untouched.
+ * n_steps == 0 with diag_last != NULL: a state query (photons_total and t_sim of the current state, summed on the device).
  * diag_last == NULL: asynchronous.  Otherwise waits and fills *diag_last; returns EMMA_RT_ENONFINITE /
  * EMMA_RT_ESUBCYCLE if the last step saw them (the step still completed). */
 EMMA_RT_API int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last);
@@ -179,17 +189,17 @@ EMMA_RT_API int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int6
  * first trip of the sub-cycle loop (Eq. 43-48), so the radiation field crosses HBM once per step; fused = 0: a
  * transport pass followed by a chemistry pass.  Ignored when chemistry = 0.  Returns EMMA_RT_OK or EINVAL. */
 EMMA_RT_API int emma_rt_set_schedule(emma_rt* h, int32_t fused);
-/* Interface flux of the transport update (Eq. 30).  EMMA_RT_FLUX_GLF (default): the Lax-Friedrichs / GLF flux of Eq. 32
- * (PAPER.md:246).  EMMA_RT_FLUX_HLL: the HLL flux the paper names as its less diffusive successor (PAPER.md:250;
- * DESIGN.md reading A19):  F = [l+ F~_L - l- F~_R + l+ l- (U_R - U_L)] / (l+ - l-),  l+ = max(0, lmax_L, lmax_R),
- * l- = min(0, lmin_L, lmin_R), lmin/lmax the extreme eigenvalues of the M1 flux Jacobian in the face direction.
- * With HLL the coupled step runs the two-pass schedule (the fused pass implements Eq. 32 only).  Returns OK / EINVAL. */
 /* Inflow boundary (reading A20; "the x = 0 boundary is a source of flux of the required
  * rate"): the ghost cells outside a face whose bc is EMMA_RT_BC_INFLOW hold the state U = (N, Fx, Fy, Fz) [photons cm^-3,
  * photons cm^-2 s^-1] given here for `group` (zeros until set); a plane-parallel flux F entering through -x is
  * (F / c_red, F, 0, 0).  face = 0..5 = -x,+x,-y,+y,-z,+z.  With an inflow face the step runs the two-pass schedule and the
  * non-TMA transport kernel.  The net flux through the face counts (negative) in photons_outflow.  Returns OK / EINVAL. */
 EMMA_RT_API int emma_rt_set_inflow(emma_rt* h, int32_t face, int32_t group, const double U[4]);
+/* Interface flux of the transport update (Eq. 30).  EMMA_RT_FLUX_GLF (default): the Lax-Friedrichs / GLF flux of Eq. 32
+ * (PAPER.md:246).  EMMA_RT_FLUX_HLL: the HLL flux the paper names as its less diffusive successor (PAPER.md:250;
+ * DESIGN.md reading A19):  F = [l+ F~_L - l- F~_R + l+ l- (U_R - U_L)] / (l+ - l-),  l+ = max(0, lmax_L, lmax_R),
+ * l- = min(0, lmin_L, lmin_R), lmin/lmax the extreme eigenvalues of the M1 flux Jacobian in the face direction.
+ * With HLL the coupled step runs the two-pass schedule (the fused pass implements Eq. 32 only).  Returns OK / EINVAL. */
 enum { EMMA_RT_FLUX_GLF = 0, EMMA_RT_FLUX_HLL = 1 };
 EMMA_RT_API int emma_rt_set_flux(emma_rt* h, int32_t flux);
 EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */

@@ -13,8 +13,8 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libemma_rt.so")
 SOURCES = ["api.cu", "amr.cu", "transport.cu", "transport_tma.cu", "transport_hll.cu", "chemistry.cu", "fused.cu", "util.cu"]
-HEADERS = [os.path.join(CSRC, "emma_rt_internal.cuh"), os.path.join(CSRC, "transport_math.cuh"), os.path.join(CSRC, "chem_math.cuh"),
-           os.path.join(CSRC, "async_copy.cuh"), os.path.join(INC, "emma_rt.h")]
+import glob
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(INC, "*.h")))     # every header is a dependency
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 

@@ -18,7 +18,8 @@ using namespace emma;
 namespace {
 
 constexpr size_t ALIGN = 256;
-constexpr int PART_SLOTS = 49152;        // a 3-level standard-AMR step: 14 refined sweeps x (888 + 1184) + level 0
+constexpr int PART_SLOTS = 106496;       // worst case of a 3-level standard-AMR step: 15 level sweeps x 3 grids of <= MAX_PART_BLOCKS
+                                         // (transport, chemistry main, tail) + one dense transport grid (9.4 MB)
 constexpr int TRANSPORT_MAX_BLOCKS = 8192;
 constexpr double E_HI_ERG = 13.6 * 1.602176634e-12;          // "E_13.6" of PAPER.md:266
 
@@ -60,8 +61,10 @@ bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
   s.nl = a ? a->n_levels : 0;
   if (s.nl < 0 || s.nl > MAXL) return false;
   s.ncell[0] = (long long)s.n * s.n * s.n; s.nocts[0] = 0;
+  if (s.nl > 0 && (!a->n_octs || !a->parent)) return false;
   for (int l = 1; l <= s.nl; l++) {
-    if (!a->n_octs || a->n_octs[l - 1] < 0 || a->n_octs[l - 1] > s.ncell[l - 1] || 8 * a->n_octs[l - 1] > 2000000000LL)
+    if (a->n_octs[l - 1] > 0 && !a->parent[l - 1]) return false;
+    if (a->n_octs[l - 1] < 0 || a->n_octs[l - 1] > s.ncell[l - 1] || 8 * a->n_octs[l - 1] > 2000000000LL)
       return false;
     s.nocts[l] = a->n_octs[l - 1];
     s.ncell[l] = 8 * s.nocts[l];
@@ -125,10 +128,32 @@ void make_layout(const Shape& s, Layout& L)
   L.total = off;
 }
 
+// Tuning knobs for experiments, read ONCE from the environment by emma_rt_init (documented in include/emma_rt.h) and
+// clamped to their valid ranges; 0 / unset = the built-in choice.
+struct Tune {
+  int nzc = 0;          // EMMA_RT_TUNE_NZC      z-chunks per tile column of the dense passes (0: cost model)
+  int nst = 6;          // EMMA_RT_TUNE_NST      stages of the TMA ring of transport_tma_kernel: 4, 6 or 8
+  int tma = 1;          // EMMA_RT_TUNE_TMA      0: the non-TMA transport kernel (transport.cu)
+  int fused = 1;        // EMMA_RT_TUNE_FUSED    0: two-pass schedule whatever emma_rt_set_schedule says
+  int chem_ctas = 0;    // EMMA_RT_TUNE_CHEMCTAS persistent CTAs per SM of the chemistry main pass (0: occupancy)
+};
+
+int env_int(const char* name, int dflt, int lo, int hi)
+{
+  const char* v = getenv(name);
+  if (!v || !*v) return dflt;
+  char* end = nullptr;
+  const long x = strtol(v, &end, 10);
+  if (end == v || x < lo || x > hi) return dflt;     // out of range or not a number: ignored
+  return (int)x;
+}
+
 }  // namespace
 
 struct emma_rt {
   emma_rt_config cfg;
+  Tune tune;
+  int chem_ctas_per_sm;                        // CTAs of the chemistry main pass that fit on an SM of this device
   Shape sh;
   Layout lay;
   char* arena;
@@ -176,6 +201,25 @@ int fail(emma_rt* h, int code, const char* fmt, ...)
     va_end(ap);
   }
   return code;
+}
+
+// Every entry point that launches work runs through here: the handle's device is made current (a process may hold
+// handles on several GPUs) and nothing thrown by the host-side bookkeeping (std::bad_alloc of its vectors and maps)
+// crosses the C boundary.
+template <class F>
+int guarded(emma_rt* h, bool set_device, F&& f)
+{
+  try {
+    if (h && set_device) {
+      const cudaError_t e = cudaSetDevice(h->cfg.device);
+      if (e != cudaSuccess) return fail(h, EMMA_RT_ECUDA, "cudaSetDevice(%d): %s", h->cfg.device, cudaGetErrorString(e));
+    }
+    return f();
+  } catch (const std::bad_alloc&) {
+    return fail(h, EMMA_RT_ENOMEM, "out of host memory");
+  } catch (...) {
+    return fail(h, EMMA_RT_EINVAL, "internal error (exception)");
+  }
 }
 
 #define CUDA_TRY(h, call)                                                                       \
@@ -230,21 +274,24 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
     for (int l = s.nl; l >= 1; l--) h->launches += launch_amr_restrict(h->lv[l], h->lv[l - 1], amr_view(h), l, 0, h->st);
     h->amr_dirty = false;
   }
+  // (level, dt, last sub-step of the level in this coarse step) in execution order, finest first
+  struct Call { int l; double dt; bool last; };
+  std::vector<Call> order;
+  struct Rec { static void go(std::vector<Call>& o, int l, int nl, const long long* nc, double dtl, bool last) {
+    if (l < nl && nc[l + 1] > 0) { go(o, l + 1, nl, nc, 0.5 * dtl, false); go(o, l + 1, nl, nc, 0.5 * dtl, last); }
+    o.push_back({l, dtl, last});
+  } };
+  Rec::go(order, 0, s.nl, s.ncell, dt, true);
+  // worst-case partial-sum slots of one coarse step, checked BEFORE the first launch so that a refusal leaves the state
+  // untouched: every sweep may use a transport grid, a chemistry main grid and a tail grid
+  if ((long long)order.size() * 3 * MAX_PART_BLOCKS + TRANSPORT_MAX_BLOCKS > PART_SLOTS)
+    return fail(h, EMMA_RT_EINVAL, "too many level sweeps for the partial-sum slots");
   for (int step = 0; step < n_steps; step++) {
     int off = 0;
     Partial* P = h->parts();
-    // (level, dt, last sub-step of the level in this coarse step) in execution order, finest first
-    struct Call { int l; double dt; bool last; };
-    std::vector<Call> order;
-    struct Rec { static void go(std::vector<Call>& o, int l, int nl, const long long* nc, double dtl, bool last) {
-      if (l < nl && nc[l + 1] > 0) { go(o, l + 1, nl, nc, 0.5 * dtl, false); go(o, l + 1, nl, nc, 0.5 * dtl, last); }
-      o.push_back({l, dtl, last});
-    } };
-    Rec::go(order, 0, s.nl, s.ncell, dt, true);
     for (const Call& cl : order) {
       const int l = cl.l;
       int np = 0;
-      if (off + 3 * MAX_PART_BLOCKS > PART_SLOTS) return fail(h, EMMA_RT_EINVAL, "too many level sweeps for the partial-sum slots");
       if (l == 0) {
         // dense pass over the whole block (its partials are not used: split cells must not count), then the
         // sparse correction of the leaves that touch a split cell
@@ -268,7 +315,7 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
         h->cur = 1 - h->cur;
         if (h->cfg.chemistry) {
           h->launches += launch_chem_level0(cp, h->lv[0], h->U(h->cur), s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
-                                            P + off, &np, h->sm_count, h->st, &h->prof);
+                                            P + off, &np, h->sm_count, h->chem_ctas_per_sm, h->st, &h->prof);
           off += np;
         } else {
           h->prof.begin(EMMA_RT_K_OTHER);
@@ -297,7 +344,7 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
           Lc.refined = l < s.nl ? (unsigned int*)(h->arena + h->lay.arefined[l]) : nullptr;
           Lc.dV_total = cl.last ? Lc.dV : 0.0;
           h->launches += launch_chem_level0(cl_cp, Lc, h->Ulev(l), s.ncell[l], (int*)(h->arena + h->lay.queue), h->qcount(),
-                                            P + off, &np, h->sm_count, h->st, nullptr_prof(h));
+                                            P + off, &np, h->sm_count, h->chem_ctas_per_sm, h->st, nullptr_prof(h));
           CUDA_TRY(h, cudaMemsetAsync(h->qcount(), 0, 8, h->st));      // queue counters of the next sweep
         } else if (h->cfg.chemistry) h->launches += launch_amr_chem(cl_cp, h->lv[l], A, l, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
         else h->launches += launch_amr_sources(h->lv[l], A, l, (float)cl.dt, cl.last ? 1 : 0, ihll, P + off, &np, h->st);
@@ -491,8 +538,10 @@ int upload_field(emma_rt* h, int field, int level, int group, const void* src, b
   const size_t eb = field_elem_bytes(field);
   float4* Ug = (field == EMMA_RT_FIELD_U) ? h->Ulev(level) + (size_t)group * nc : nullptr;
   if (field == EMMA_RT_FIELD_U && h->sh.amr) h->amr_dirty = true;
+  unsigned int* bad_dev = h->qcount() + 32;                            // invalid-value counter of the import kernel
   if (src_is_device) {
-    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, 0, nc, src, h->st);
+    // stream-ordered, no host wait: values are not validated here (a NaN stays a NaN and is reported by the next step)
+    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, 0, nc, src, nullptr, h->st);
     CUDA_TRY(h, cudaGetLastError());
     return EMMA_RT_OK;
   }
@@ -502,18 +551,29 @@ int upload_field(emma_rt* h, int field, int level, int group, const void* src, b
   for (long long off = 0; off < nc; off += chunk) {
     const long long cnt = std::min(chunk, nc - off);
     CUDA_TRY(h, cudaMemcpyAsync(scratch, (const char*)src + (size_t)off * eb, (size_t)cnt * eb, cudaMemcpyHostToDevice, h->st));
-    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, off, cnt, scratch, h->st);
+    h->launches += launch_import(field, h->lv[level], Ug, (float)h->cfg.c_red_cm_s, off, cnt, scratch, bad_dev, h->st);
     CUDA_TRY(h, cudaGetLastError());
   }
+  if (field == EMMA_RT_FIELD_U) {
+    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+    return EMMA_RT_OK;
+  }
+  // n0 <= 0, T <= 0, x outside [0, 1] or anything non-finite would only surface as inf / NaN one step later: refuse now
+  CUDA_TRY(h, cudaMemcpyAsync(&h->diag_pinned->err_last, bad_dev, 4, cudaMemcpyDeviceToHost, h->st));
   CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  const unsigned int n_bad = h->diag_pinned->err_last;
+  if (n_bad) {
+    CUDA_TRY(h, cudaMemsetAsync(bad_dev, 0, 4, h->st));
+    return fail(h, EMMA_RT_EINVAL, "%u invalid value(s) in field %d of level %d (need finite n0 > 0, T > 0, 0 <= x <= 1)", n_bad, field, level);
+  }
   return EMMA_RT_OK;
 }
 
 }  // namespace
 
-extern "C" {
+namespace {
 
-size_t emma_rt_arena_bytes(const emma_rt_config* cfg, const emma_rt_amr* amr)
+size_t arena_bytes_impl(const emma_rt_config* cfg, const emma_rt_amr* amr)
 {
   Shape s;
   if (!make_shape(cfg, amr, s)) return 0;
@@ -522,7 +582,7 @@ size_t emma_rt_arena_bytes(const emma_rt_config* cfg, const emma_rt_amr* amr)
   return L.total;
 }
 
-int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, const emma_rt_fields* fields,
+int init_impl(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, const emma_rt_fields* fields,
                  void* arena_dev, size_t arena_bytes)
 {
   if (!out) return EMMA_RT_EINVAL;
@@ -547,6 +607,19 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   cudaDeviceProp prop;
   CUDA_TRY(h, cudaGetDeviceProperties(&prop, cfg->device));
   h->sm_count = prop.multiProcessorCount;
+  // function attributes belong to the device's context: set them for every handle (a second handle on another GPU of the
+  // same process needs its own), and take the occupancy of the persistent chemistry pass on THIS device
+  CUDA_TRY(h, configure_transport_tma());
+  CUDA_TRY(h, configure_transport_hll());
+  CUDA_TRY(h, configure_fused(s.G));
+  CUDA_TRY(h, configure_chemistry(s.G, &h->chem_ctas_per_sm));
+  h->tune.nzc = env_int("EMMA_RT_TUNE_NZC", 0, 1, 4096);
+  h->tune.nst = env_int("EMMA_RT_TUNE_NST", 6, 4, 8);
+  if (h->tune.nst != 4 && h->tune.nst != 8) h->tune.nst = 6;
+  h->tune.tma = env_int("EMMA_RT_TUNE_TMA", 1, 0, 1);
+  h->tune.fused = env_int("EMMA_RT_TUNE_FUSED", 1, 0, 1);
+  h->tune.chem_ctas = env_int("EMMA_RT_TUNE_CHEMCTAS", 0, 1, 32);
+  if (h->tune.chem_ctas > 0) h->chem_ctas_per_sm = h->tune.chem_ctas;
   CUDA_TRY(h, cudaMallocHost((void**)&h->diag_pinned, sizeof(DiagDev)));
   for (int b = 0; b < 2; b++) {
     const int r = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps[b]);
@@ -632,7 +705,7 @@ int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* am
   return EMMA_RT_OK;
 }
 
-int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos, const double* Q)
+int set_sources_impl(emma_rt* h, int64_t n_src, const double* pos, const double* Q)
 {
   if (!h) return EMMA_RT_EINVAL;
   const Shape& s = h->sh;
@@ -689,12 +762,7 @@ int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos, const doub
   return EMMA_RT_OK;
 }
 
-double emma_rt_dt_cfl(const emma_rt* h, double courant)
-{
-  return h ? courant * h->dx / (3.0 * h->cfg.c_red_cm_s) : 0.0;
-}
-
-int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
+int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
 {
   if (!h) return EMMA_RT_EINVAL;
   if (!(dt > 0.0) || n_steps < 0) return fail(h, EMMA_RT_EINVAL, "dt must be > 0 and n_steps >= 0");
@@ -714,7 +782,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   auto pick_zchunks = [&](TransportParams& q, int per, int per_sm) -> bool {
     const long long slots = (long long)per_sm * h->sm_count;
     int best = 1; double best_cost = 1e300;
-    const int env_nzc = getenv("EMMA_RT_TUNE_NZC") ? atoi(getenv("EMMA_RT_TUNE_NZC")) : 0;
+    const int env_nzc = h->tune.nzc;
     for (int nzc = 1; nzc <= std::max(1, s.n / 8); nzc++) {
       const int zc = (s.n + nzc - 1) / nzc;
       const int nz = (s.n + zc - 1) / zc;
@@ -724,15 +792,15 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
       const double cost = (double)((blocks + slots - 1) / slots) * (zc + 3);
       if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = nzc; }
     }
-    if (env_nzc > 0) best = env_nzc;
+    if (env_nzc > 0 && env_nzc <= s.n) best = env_nzc;
     q.zchunk = (s.n + best - 1) / best;
     q.nzc = (s.n + q.zchunk - 1) / q.zchunk;
     return (long long)per * q.nzc <= TRANSPORT_MAX_BLOCKS;
   };
   if (!pick_zchunks(tp, tp.tiles_x * tp.tiles_y * s.G, 2)) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
-  tp.nst = getenv("EMMA_RT_TUNE_NST") ? atoi(getenv("EMMA_RT_TUNE_NST")) : 6;
-  tp.pf = getenv("EMMA_RT_TUNE_PF") ? atoi(getenv("EMMA_RT_TUNE_PF")) : 2;
-  const bool use_tma = !any_inflow && (getenv("EMMA_RT_TUNE_TMA") ? atoi(getenv("EMMA_RT_TUNE_TMA")) != 0 : true);
+  tp.nst = h->tune.nst;
+  tp.pf = 2;
+  const bool use_tma = !any_inflow && h->tune.tma != 0;
   tp.want_total = h->cfg.chemistry ? 0 : 1;
   tp.nu = (float)(c * dt / h->dx);
   tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
@@ -753,7 +821,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   const bool hll = h->flux == EMMA_RT_FLUX_HLL;
   TransportParams hp = tp;                     // HLL pass (transport_hll.cu): one group per CTA, one CTA per SM
   if (hll && !pick_zchunks(hp, hp.tiles_x * hp.tiles_y * s.G, hll_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
-  const bool fused = !hll && !any_inflow && h->cfg.chemistry && h->fused && (getenv("EMMA_RT_TUNE_FUSED") ? atoi(getenv("EMMA_RT_TUNE_FUSED")) != 0 : true);
+  const bool fused = !hll && !any_inflow && h->cfg.chemistry && h->fused && h->tune.fused != 0;
   TransportParams fp = tp;
   fp.tiles_y = (s.n + fused_tile_y() - 1) / fused_tile_y();
   if (fused && !pick_zchunks(fp, fp.tiles_x * fp.tiles_y, fused_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
@@ -781,7 +849,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
       off += np;
       for (int l = s.nl; l >= 1; l--) {
         h->prof.begin(EMMA_RT_K_CHEM_REFINED);
-        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->st);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->sm_count, h->st);
         h->prof.end();
         off += np;
       }
@@ -812,12 +880,12 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
       // 2-4. CRTA: deepest refined level first (inject -> leaf chemistry -> restrict), then the unrefined coarse cells
       for (int l = s.nl; l >= 1; l--) {
         h->prof.begin(EMMA_RT_K_CHEM_REFINED);
-        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->st);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->sm_count, h->st);
         h->prof.end();
         off += np;
       }
       h->launches += launch_chem_level0(cp, h->lv[0], U, s.ncell[0], (int*)(h->arena + h->lay.queue), h->qcount(),
-                                        P + off, &np, h->sm_count, h->st, &h->prof);
+                                        P + off, &np, h->sm_count, h->chem_ctas_per_sm, h->st, &h->prof);
       off += np;
     } else {
       h->prof.begin(EMMA_RT_K_OTHER);
@@ -833,19 +901,16 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   }
   CUDA_TRY(h, cudaGetLastError());
   if (!diag_last) return EMMA_RT_OK;
-  if (n_steps == 0) {                          // state query: photons currently in the box
-    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  if (n_steps == 0) {                          // state query: photons currently in the box (summed on the device)
     memset(diag_last, 0, sizeof *diag_last);
     diag_last->t_sim = h->t_sim;
     diag_last->dtau_min = INFINITY;
-    std::vector<float> N((size_t)s.ncell[0]);
-    double tot = 0;
-    for (int g = 0; g < s.G; g++) {
-      int rc = emma_rt_read(h, EMMA_RT_FIELD_N, 0, g, N.data(), N.size() * 4, 0);
-      if (rc != EMMA_RT_OK) return rc;
-      for (float v : N) tot += (double)v;
-    }
-    diag_last->photons_total = tot * h->lv[0].dV;
+    double* tot_dev = (double*)(h->qcount() + 16);                     // scratch double inside the counter block
+    h->launches += launch_sum_N(h->U(h->cur), (long long)s.G * s.ncell[0], h->lv[0].dV, h->parts(), tot_dev, h->st);
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync(&h->diag_pinned->d.photons_total, tot_dev, sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    CUDA_TRY(h, cudaStreamSynchronize(h->st));
+    diag_last->photons_total = h->diag_pinned->d.photons_total;
     return EMMA_RT_OK;
   }
   CUDA_TRY(h, cudaMemcpyAsync(h->diag_pinned, h->diag(), sizeof(DiagDev), cudaMemcpyDeviceToHost, h->st));
@@ -856,7 +921,7 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   return EMMA_RT_OK;
 }
 
-int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
+int read_impl(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
 {
   if (!h || !dst) return EMMA_RT_EINVAL;
   const Shape& s = h->sh;
@@ -888,7 +953,7 @@ int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* 
   return EMMA_RT_OK;
 }
 
-int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const void* src, size_t bytes, int32_t src_is_device)
+int write_impl(emma_rt* h, int32_t field, int32_t level, int32_t group, const void* src, size_t bytes, int32_t src_is_device)
 {
   if (!h || !src) return EMMA_RT_EINVAL;
   const Shape& s = h->sh;
@@ -901,15 +966,7 @@ int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const
   return upload_field(h, field, level, group, src, src_is_device != 0);
 }
 
-int64_t emma_rt_level_cells(const emma_rt* h, int32_t level)
-{
-  if (!h || level < 0 || level > h->sh.nl) return -1;
-  return h->sh.ncell[level];
-}
-
-int64_t emma_rt_kernel_launches(const emma_rt* h) { return h ? h->launches : 0; }
-
-int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out)
+int profile_impl(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out)
 {
   if (!h) return EMMA_RT_EINVAL;
   CUDA_TRY(h, cudaStreamSynchronize(h->st));
@@ -929,6 +986,67 @@ int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launche
   h->prof.on = enable != 0;
   return EMMA_RT_OK;
 }
+
+}  // namespace
+
+extern "C" {
+
+size_t emma_rt_arena_bytes(const emma_rt_config* cfg, const emma_rt_amr* amr)
+{
+  try { return arena_bytes_impl(cfg, amr); } catch (...) { return 0; }
+}
+
+int emma_rt_init(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, const emma_rt_fields* fields,
+                 void* arena_dev, size_t arena_bytes)
+{
+  // *out is set as soon as the handle exists, so a failure (also an exception) leaves a handle whose message can be read
+  if (out) *out = nullptr;
+  try {
+    return init_impl(out, cfg, amr, fields, arena_dev, arena_bytes);
+  } catch (const std::bad_alloc&) {
+    return fail(out ? *out : nullptr, EMMA_RT_ENOMEM, "out of host memory");
+  } catch (...) {
+    return fail(out ? *out : nullptr, EMMA_RT_EINVAL, "internal error (exception)");
+  }
+}
+
+int emma_rt_set_sources(emma_rt* h, int64_t n_src, const double* pos_box, const double* Q)
+{
+  return guarded(h, true, [&] { return set_sources_impl(h, n_src, pos_box, Q); });
+}
+
+int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
+{
+  return guarded(h, true, [&] { return step_impl(h, dt, n_steps, diag_last); });
+}
+
+int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
+{
+  return guarded(h, true, [&] { return read_impl(h, field, level, group, dst, bytes, dst_is_device); });
+}
+
+int emma_rt_write(emma_rt* h, int32_t field, int32_t level, int32_t group, const void* src, size_t bytes, int32_t src_is_device)
+{
+  return guarded(h, true, [&] { return write_impl(h, field, level, group, src, bytes, src_is_device); });
+}
+
+int emma_rt_profile(emma_rt* h, int32_t enable, double* ms_out, int64_t* launches_out)
+{
+  return guarded(h, true, [&] { return profile_impl(h, enable, ms_out, launches_out); });
+}
+
+double emma_rt_dt_cfl(const emma_rt* h, double courant)
+{
+  return h ? courant * h->dx / (3.0 * h->cfg.c_red_cm_s) : 0.0;
+}
+
+int64_t emma_rt_level_cells(const emma_rt* h, int32_t level)
+{
+  if (!h || level < 0 || level > h->sh.nl) return -1;
+  return h->sh.ncell[level];
+}
+
+int64_t emma_rt_kernel_launches(const emma_rt* h) { return h ? h->launches : 0; }
 
 int emma_rt_set_schedule(emma_rt* h, int32_t fused)
 {

@@ -1,6 +1,6 @@
-// async_copy.cuh -- mbarrier + TMA (cp.async.bulk.tensor) helpers of the sm_100a kernels that feed shared-memory
-// rings asynchronously (fused.cu).  One elected thread issues the copies; every consumer waits on the stage's
-// mbarrier phase.
+// async_copy.cuh -- the one copy of the mbarrier + TMA (cp.async.bulk / cp.async.bulk.tensor) helpers of the sm_100a
+// kernels that feed shared-memory rings asynchronously (transport_tma.cu, transport_hll.cu, fused.cu, chemistry.cu).
+// Elected threads issue the copies; every consumer waits on the stage's mbarrier phase.
 #pragma once
 #include <cuda.h>
 
@@ -60,6 +60,13 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
       :: "r"(dst), "l"(map), "r"(bar), "r"(cx), "r"(cy), "r"(cz) : "memory");
+}
+
+// a contiguous run of bytes (multiple of 16, 16-byte aligned on both sides) -> shared memory, completion on an mbarrier
+__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar)
+{
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
 }  // namespace acp

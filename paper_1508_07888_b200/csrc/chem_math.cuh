@@ -3,6 +3,7 @@
 // conditioning notes (x and 1-x both carried, per-atom energies, rates through lg2/ex2).
 #pragma once
 #include "emma_rt_internal.cuh"
+#include "transport_math.cuh"
 
 namespace emma {
 
@@ -63,6 +64,15 @@ __device__ __forceinline__ Rates rates_at(float T, int otsa, float x, float n0)
     r.rec = (aA - aB) * x * x * n0 * n0;              // A6: recombination radiation, group 1 only
   }
   return r;
+}
+
+// First guess of the chemical step, abs(e / (H - Lambda)) (reading A9), `if_zero` when H = Lambda.  d is
+// (H - Lambda) per atom at state p.  One approximate reciprocal instead of an IEEE division: the guess only picks the
+// starting dtau of the halving loop and feeds the dtau_min diagnostic (held to 1e-3 against the oracle).
+__device__ __forceinline__ float first_guess(float eps, float d, float if_zero)
+{
+  const float ad = fabsf(d);
+  return (ad == 0.f) ? if_zero : fabsf(eps) * frcp(ad);
 }
 
 // Eq. 44 with the factor chosen by attempt(): m > 0 -> F' = F m (m = 1/(1 + k dtau), strong sink);
@@ -131,7 +141,7 @@ __device__ __forceinline__ bool substep(const ChemParams& cp, CellState<G>& c, f
 #pragma unroll
     for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
     const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);      // (H - Lambda)/n0 at state p
-    const float guess = (d == 0.f) ? rem : fabsf(c.eps / d);                        // PAPER.md:290 (A9: abs)
+    const float guess = first_guess(c.eps, d, rem);                                 // PAPER.md:290 (A9: abs)
     dtau_min = fminf(dtau_min, guess);
     dtau = fminf(rem, guess);
   }
@@ -224,13 +234,19 @@ __device__ __forceinline__ void load_cell(const LevelDev& L, long long cell, con
   load_sources<G>(L, cell, c.S);
 }
 
+// 0 * v is +-0 for a finite v and NaN for an infinite or NaN v, so one packed FMA per pair of values accumulates
+// "anything non-finite" into s (IEEE arithmetic: nothing here is folded away without fast-math)
 template <int G>
 __device__ __forceinline__ bool finite_cell(const CellState<G>& c)
 {
-  float s = fabsf(c.eps) + fabsf(c.x);
+  float s0 = 0.f, s1 = 0.f;
+  fma2(s0, s1, c.eps, c.x, 0.f, 0.f, s0, s1);
 #pragma unroll
-  for (int g = 0; g < G; g++) s += fabsf(c.N[g]) + fabsf(c.px[g]) + fabsf(c.py[g]) + fabsf(c.pz[g]);
-  return s < FINF;
+  for (int g = 0; g < G; g++) {
+    fma2(s0, s1, c.N[g], c.px[g], 0.f, 0.f, s0, s1);
+    fma2(s0, s1, c.py[g], c.pz[g], 0.f, 0.f, s0, s1);
+  }
+  return (s0 + s1) == 0.f;
 }
 
 template <int G>

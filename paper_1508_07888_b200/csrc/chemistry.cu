@@ -17,8 +17,7 @@
 // rule, are appended to a queue with one warp-aggregated atomic and left untouched.  `chem_tail_kernel` then runs
 // persistent warps over that (compacted) queue: each lane owns one queued cell, advances it one accepted sub-step
 // per loop trip and refills from the queue as soon as its cell is done, so lanes stay busy while any work is left.
-#include <stdlib.h>
-
+#include "async_copy.cuh"
 #include "chem_math.cuh"
 #include "emma_rt_internal.cuh"
 
@@ -27,111 +26,18 @@ namespace emma {
 namespace {
 
 // ------------------------------------------------------------------------------------------------------------
-// level 0, pass 1: every unrefined coarse cell gets one attempt with dtau = dt (HBM-bound)
-// ------------------------------------------------------------------------------------------------------------
-template <int G>
-__global__ void __launch_bounds__(256)
-chem_main_kernel(const ChemParams cp, const LevelDev L, float4* __restrict__ U, long long ncell,
-                 int* __restrict__ queue, unsigned int* __restrict__ qcount, Partial* __restrict__ parts)
-{
-  Acc acc;
-  const int lane = threadIdx.x & 31;
-  for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += (long long)gridDim.x * blockDim.x) {
-    const long long cell = base + threadIdx.x;
-    bool valid = cell < ncell;
-    if (valid && L.refined) valid = !((L.refined[cell >> 5] >> (cell & 31)) & 1u);   // split cells: CRTA kernels
-    bool defer = false;
-    if (valid) {
-      CellState<G> c;
-      load_cell<G>(L, cell, U, ncell, cell, c);
-      CellTally tl;
-      float dmin = FINF;
-      // fast path == the first trip of the sub-cycle loop when it covers the whole step
-      const float T = c.eps * frcp(KB15 * (1.f + c.x));
-      const Rates r = rates_at(T, cp.otsa, c.x, c.n0);
-      bool go = true;
-      if (cp.thermal) {
-        float hsum = 0.f;
-#pragma unroll
-        for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
-        const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
-        const float guess = (d == 0.f) ? cp.dt : fabsf(c.eps / d);
-        go = guess >= cp.dt;
-        if (go) dmin = guess;
-      }
-      float N1[G], iden[G], x1, y1, eps1;
-      if (go) go = attempt<G>(cp, c, r, cp.dt, N1, iden, x1, y1, eps1);
-      if (go) {
-        const float k = c.y * c.n0 * cp.dt;
-#pragma unroll
-        for (int g = 0; g < G; g++) {
-          tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);
-          tl.injected = fmaf(c.S[g], cp.dt, tl.injected);
-          c.N[g] = N1[g];
-          c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);
-        }
-        tl.recomb = r.rec * cp.dt;
-        c.x = x1; c.y = y1; c.eps = eps1;
-        tl.nsub = 1;
-        store_cell<G>(L, cell, U, ncell, c, tl, cp.record);
-        fold(acc, tl, c.N, G, L.dV, L.dV_total);
-        acc.dtau_min = fminf(acc.dtau_min, dmin);
-        if (!finite_cell<G>(c)) acc.nonfinite++;
-      } else {
-        defer = true;
-      }
-    }
-    // warp-aggregated append of the deferred cells (north_star item 3: warp-level work compaction)
-    const unsigned m = __ballot_sync(0xffffffffu, defer);
-    if (m) {
-      const int leader = __ffs(m) - 1;
-      unsigned b = 0;
-      if (lane == leader) b = atomicAdd(qcount, (unsigned)__popc(m));
-      b = __shfl_sync(0xffffffffu, b, leader);
-      if (defer) {
-        queue[b + __popc(m & ((1u << lane) - 1u))] = (int)cell;
-        acc.ndefer++;
-      }
-    }
-  }
-  block_reduce_store(acc, parts + blockIdx.x);
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// level 0, pass 1, bulk-async variant: the same arithmetic, but the inputs of a chunk of 256 cells (G float4 runs of
-// 4 KB and the n0, xs, eps runs of 1 KB) are brought into a ring of shared-memory stages by cp.async.bulk copies that
-// complete on mbarriers, NSTC-1 chunks ahead of the compute and at no register cost.  chem_main_kernel keeps ~60 B per
-// thread in flight and waits on long-scoreboard stalls (profiles/r1b_summary.md: 14 of 18.5 cycles per issue).
+// level 0, pass 1: every unrefined coarse cell gets one attempt with dtau = dt (HBM-bound).  The inputs of a chunk of 256
+// cells (G float4 runs of 4 KB and the n0, xs, eps runs of 1 KB) are brought into a ring of shared-memory stages by
+// cp.async.bulk copies that complete on mbarriers, NSTC-1 chunks ahead of the compute and at no register cost (a plain
+// one-load-per-thread version kept ~60 B per thread in flight and waited on long-scoreboard stalls,
+// profiles/r1b_summary.md: 14 of 18.5 cycles per issue).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int CH = 256;                                               // cells per chunk = threads per CTA
 constexpr int NSTC = 4;                                               // stages of the ring
 template <int G> constexpr int chem_stage_bytes() { return CH * 16 * G + CH * 4 * 3; }
 template <int G> constexpr int chem_smem_bytes() { return NSTC * chem_stage_bytes<G>() + 8 * NSTC; }
 
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
-{
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-  unsigned done;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-  } while (!done);
-}
-__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar)
-{
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
+using namespace acp;
 
 template <int G>
 __global__ void __launch_bounds__(CH)
@@ -163,8 +69,7 @@ chem_main_bulk_kernel(const ChemParams cp, const LevelDev L, float4* __restrict_
   };
   if (t == 0) {
     for (int s = 0; s < NSTC; s++) mbar_init(bar0 + 8 * s, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_fence_init();
   }
   __syncthreads();
   if (t == 0)
@@ -209,7 +114,7 @@ chem_main_bulk_kernel(const ChemParams cp, const LevelDev L, float4* __restrict_
 #pragma unroll
         for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
         const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
-        const float guess = (d == 0.f) ? cp.dt : fabsf(c.eps / d);
+        const float guess = first_guess(c.eps, d, cp.dt);
         go = guess >= cp.dt;
         if (go) dmin = guess;
       }
@@ -442,31 +347,15 @@ int chem_tail_G(const ChemParams& cp, const LevelDev& L0, float4* U, long long n
 
 template <int G>
 int chem_level0_G(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue, unsigned int* qcount,
-                  Partial* parts, int* n_parts, int sm_count, cudaStream_t st, Profiler* pf)
+                  Partial* parts, int* n_parts, int sm_count, int ctas_per_sm, cudaStream_t st, Profiler* pf)
 {
-  long long want = (ncell + 255) / 256;
-  int nb = (int)(want < (long long)sm_count * 8 ? want : (long long)sm_count * 8);
-  if (nb > MAX_PART_BLOCKS) nb = MAX_PART_BLOCKS;
-  const bool bulk = getenv("EMMA_RT_TUNE_CHEMBULK") ? atoi(getenv("EMMA_RT_TUNE_CHEMBULK")) != 0 : true;
-  if (bulk) {
-    static bool configured = false;
-    if (!configured) {
-      if (cudaFuncSetAttribute(chem_main_bulk_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               chem_smem_bytes<G>()) != cudaSuccess) return 0;
-      configured = true;
-    }
-    static int occ = 0;                                               // persistent CTAs: as many as fit per SM
-    if (!occ && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, chem_main_bulk_kernel<G>, CH, chem_smem_bytes<G>()) != cudaSuccess) return 0;
-    const int per_sm = getenv("EMMA_RT_TUNE_CHEMCTAS") ? atoi(getenv("EMMA_RT_TUNE_CHEMCTAS")) : (occ > 0 ? occ : 1);
-    nb = (int)(want < (long long)sm_count * per_sm ? want : (long long)sm_count * per_sm);
-    pf->begin(EMMA_RT_K_CHEM_MAIN);
-    chem_main_bulk_kernel<G><<<nb, CH, chem_smem_bytes<G>(), st>>>(cp, L0, U, ncell, queue, qcount, parts);
-    pf->end();
-  } else {
-    pf->begin(EMMA_RT_K_CHEM_MAIN);
-    chem_main_kernel<G><<<nb, 256, 0, st>>>(cp, L0, U, ncell, queue, qcount, parts);
-    pf->end();
-  }
+  const long long want = (ncell + CH - 1) / CH;
+  long long cap = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);      // persistent CTAs: as many as fit per SM
+  if (cap > MAX_PART_BLOCKS) cap = MAX_PART_BLOCKS;
+  const int nb = (int)(want < cap ? want : cap);
+  pf->begin(EMMA_RT_K_CHEM_MAIN);
+  chem_main_bulk_kernel<G><<<nb, CH, chem_smem_bytes<G>(), st>>>(cp, L0, U, ncell, queue, qcount, parts);
+  pf->end();
   *n_parts = nb;
   if (!cp.thermal) return 1;                                          // isothermal mode never defers
   int nt = 0;
@@ -475,16 +364,37 @@ int chem_level0_G(const ChemParams& cp, const LevelDev& L0, float4* U, long long
   return 2;
 }
 
+template <int G>
+cudaError_t chem_configure_G(int* occ)
+{
+  cudaError_t e = cudaFuncSetAttribute(chem_main_bulk_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, chem_smem_bytes<G>());
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, chem_main_bulk_kernel<G>, CH, chem_smem_bytes<G>());
+}
+
 }  // namespace
 
+// Per-device set-up of the chemistry kernels for G groups (called by emma_rt_init with the handle's device current):
+// opts the bulk main pass into its dynamic shared memory and returns how many of its CTAs fit on an SM.
+cudaError_t configure_chemistry(int G, int* ctas_per_sm)
+{
+  switch (G) {
+    case 1: return chem_configure_G<1>(ctas_per_sm);
+    case 2: return chem_configure_G<2>(ctas_per_sm);
+    case 3: return chem_configure_G<3>(ctas_per_sm);
+    default: return chem_configure_G<4>(ctas_per_sm);
+  }
+}
+
 int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
-                       unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, cudaStream_t st, Profiler* pf)
+                       unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, int ctas_per_sm, cudaStream_t st,
+                       Profiler* pf)
 {
   switch (cp.G) {
-    case 1: return chem_level0_G<1>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
-    case 2: return chem_level0_G<2>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
-    case 3: return chem_level0_G<3>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
-    default: return chem_level0_G<4>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, st, pf);
+    case 1: return chem_level0_G<1>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, ctas_per_sm, st, pf);
+    case 2: return chem_level0_G<2>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, ctas_per_sm, st, pf);
+    case 3: return chem_level0_G<3>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, ctas_per_sm, st, pf);
+    default: return chem_level0_G<4>(cp, L0, U, ncell, queue, qcount, parts, n_parts, sm_count, ctas_per_sm, st, pf);
   }
 }
 
@@ -503,14 +413,13 @@ int launch_chem_tail(const ChemParams& cp, const LevelDev& L0, float4* U, long l
 }
 
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U, long long ncell0,
-                        Partial* parts, int* n_parts, cudaStream_t st)
+                        Partial* parts, int* n_parts, int sm_count, cudaStream_t st)
 {
   const LevelDev& L = lv[level];
   if (L.ncell == 0) { *n_parts = 0; return 0; }
   long long want = (L.ncell + 127) / 128;
-  static int sms = 0;                                                 // persistent grid: whole waves of 8 CTAs per SM
-  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-  const long long cap = (sms > 0 && (long long)sms * 8 <= MAX_PART_BLOCKS) ? (long long)sms * 8 : MAX_PART_BLOCKS;
+  // persistent grid: whole waves of 8 CTAs per SM
+  const long long cap = (sm_count > 0 && (long long)sm_count * 8 <= MAX_PART_BLOCKS) ? (long long)sm_count * 8 : MAX_PART_BLOCKS;
   int nb = (int)(want < cap ? want : cap);
   const float4* Ut_above = (level < n_levels) ? lv[level + 1].Ut : nullptr;
   const long long nocts_above = (level < n_levels) ? lv[level + 1].nocts : 0;

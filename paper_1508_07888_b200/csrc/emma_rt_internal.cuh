@@ -119,8 +119,14 @@ int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int t
 int launch_transport_tma(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st);
 int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
-                       unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, cudaStream_t st,
+                       unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, int ctas_per_sm, cudaStream_t st,
                        Profiler* pf);
+// per-device set-up of the kernels that need more than 48 KB of dynamic shared memory; called by emma_rt_init for every
+// handle with the handle's device current (function attributes belong to the device's context, not to the process)
+cudaError_t configure_transport_tma();
+cudaError_t configure_transport_hll();
+cudaError_t configure_fused(int G);
+cudaError_t configure_chemistry(int G, int* ctas_per_sm);
 int launch_chem_tail(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
                      unsigned int* qcount, Partial* parts, int* n_parts, int sm_count, cudaStream_t st, Profiler* pf);
 int launch_fused(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, const ChemParams& cp,
@@ -131,7 +137,7 @@ int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in,
                          int* n_parts, cudaStream_t st);
 int hll_ctas_per_sm();
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U,
-                        long long ncell0, Partial* parts, int* n_parts, cudaStream_t st);
+                        long long ncell0, Partial* parts, int* n_parts, int sm_count, cudaStream_t st);
 int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts,
                           int* n_parts, cudaStream_t st);
 int launch_finalize(const Partial* parts, int n_parts, DiagDev* diag, unsigned int* qcount, double t_sim,
@@ -141,7 +147,9 @@ int launch_restrict_init(const LevelDev* lv, int level, cudaStream_t st);
 int launch_export(int field, const LevelDev& L, const float4* Ug, float c_red, long long off, long long cnt,
                   void* dst, cudaStream_t st);
 int launch_import(int field, const LevelDev& L, float4* Ug, float c_red, long long off, long long cnt,
-                  const void* src, cudaStream_t st);
+                  const void* src, unsigned int* bad, cudaStream_t st);
+// sum of n float4.x values times dV -> *out (fp64, fixed summation order); scratch = >= 1024 Partial slots
+int launch_sum_N(const float4* U, long long n, double dV, Partial* scratch, double* out, cudaStream_t st);
 int launch_set_bits(unsigned int* mask, const int* cells, int n, cudaStream_t st);
 
 // ---- small device helpers -----------------------------------------------------------------------------------

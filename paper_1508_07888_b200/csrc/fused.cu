@@ -19,7 +19,6 @@
 // pair of closure planes (plane j's, and plane j-1's whose slots receive plane j+1's as they are consumed); one
 // __syncthreads per plane.
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "async_copy.cuh"
 #include "chem_math.cuh"
@@ -87,8 +86,9 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const int oxp = (tx < wx - 1) ? own + 16 : STAGE_ROWS + COLB + ty * 16;
   const int oym = own - ROWB;
   const int oyp = (ty + 1 < wy) ? own + ROWB : TOPROW + tx * 16;
-  // halo closures: the 2 wy + 2 wx halo cells of each of the G groups are dealt round-robin over the warps (task
-  // h -> warp h % 16, lane h / 16), at most one per thread, so that every warp carries the same extra work
+  // halo closures: the 2 wy + 2 wx halo cells of each of the G groups are dealt in order, task h -> thread h: whole
+  // warps (288 tasks = 9 of the 16 warps at G = 3) so that the others skip the work altogether, and consecutive lanes
+  // read consecutive cells (no bank conflicts).  The split-phase plane barrier lets the lighter warps run ahead.
   // (with 32 x 8 tiles and G = 4 there are more halo cells than threads: a second task for some)
   auto halo_task = [&](int h) -> int {         // byte offset (inside a stage) of halo task h, or -1
     const int nh = 2 * wy + 2 * wx;
@@ -98,8 +98,8 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
                 : (q < 2 * wy + wx) ? (q - 2 * wy) * 16 : TOPROW + (q - 2 * wy - wx) * 16;
     return g * SG + o;
   };
-  const int hoff = halo_task((t & 31) * (NT / 32) + (t >> 5));
-  const int hoff2 = ((2 * TY + 2 * TX) * G > NT) ? halo_task(NT + (t & 31) * (NT / 32) + (t >> 5)) : -1;
+  const int hoff = halo_task(t);
+  const int hoff2 = ((2 * TY + 2 * TX) * G > NT) ? halo_task(NT + t) : -1;
   float sxm = 1.f, sxp = 1.f, sym = 1.f, syp = 1.f;     // reflective faces: sign of the face-normal flux (A13)
   if (BCGEN) {
     if (tx == 0 && x0 == 0 && p.bc[0] == EMMA_RT_BC_REFLECTIVE) sxm = -1.f;
@@ -147,6 +147,8 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const float c0 = p.c0, c1 = p.c1;
   const size_t plane = (size_t)n * n, ncell = plane * n;
   Acc acc_d;
+  double t_abs = 0.0, t_tot = 0.0, t_inj = 0.0, t_rec = 0.0;          // fast-path tallies, per unit volume
+  unsigned n_fast = 0;                                               // cells finished here (one accepted sub-step each)
 
   // closures of plane in stage `st` into closure plane `ab`: my own cell (all groups) and my halo cell
   auto stage_closures = [&](const unsigned char* st, unsigned char* ab, bool halo) {
@@ -284,7 +286,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
 #pragma unroll
           for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
           const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
-          const float guess = (d == 0.f) ? cp.dt : fabsf(c.eps / d);          // PAPER.md:290 (A9)
+          const float guess = first_guess(c.eps, d, cp.dt);                    // PAPER.md:290 (A9)
           go = guess >= cp.dt;
           if (go) dmin = guess;
         }
@@ -292,20 +294,31 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
       float N1[G], iden[G], x1, y1, eps1;
       if (go) go = attempt<G>(cp, c, r, cp.dt, N1, iden, x1, y1, eps1);
       if (go) {
+        // commit.  The tallies of A15 are summed per thread in fp64 and scaled by the (one) cell volume at the end;
+        // the injected term exists in source cells only, the recombination term without OTSA only.
         CellTally tl;
         const float k = c.y * c.n0 * cp.dt;
+        float sumN = 0.f;
 #pragma unroll
         for (int g = 0; g < G; g++) {
           tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);
-          tl.injected = fmaf(c.S[g], cp.dt, tl.injected);
           c.N[g] = N1[g];
+          sumN += N1[g];
           c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);
         }
-        tl.recomb = r.rec * cp.dt;
         c.x = x1; c.y = y1; c.eps = eps1;
         tl.nsub = 1;
         store_cell<G>(L, (long long)cell, Uout, (long long)ncell, c, tl, cp.record);
-        fold(acc_d, tl, c.N, G, L.dV, L.dV_total);
+        t_abs += (double)tl.absorbed;
+        t_tot += (double)sumN;
+        if ((srcw >> (cell & 31)) & 1u) {
+          float inj = 0.f;
+#pragma unroll
+          for (int g = 0; g < G; g++) inj = fmaf(c.S[g], cp.dt, inj);
+          t_inj += (double)inj;
+        }
+        if (!cp.otsa) t_rec += (double)(r.rec * cp.dt);
+        n_fast++;
         acc_d.dtau_min = fminf(acc_d.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc_d.nonfinite++;
       } else {
@@ -332,6 +345,8 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   }
   flush_deferred();
 
+  acc_d.absorbed = t_abs * L.dV; acc_d.injected = t_inj * L.dV; acc_d.recomb = t_rec * L.dV; acc_d.total = t_tot * L.dV_total;
+  acc_d.nsub = n_fast; acc_d.nsub_max = n_fast ? 1u : 0u;
   acc_d.outflow *= (double)p.nu * p.dV;
   block_reduce_store(acc_d, parts + blockIdx.x);
 }
@@ -340,18 +355,31 @@ template <int G>
 int launch_G(const TransportParams& p, const TransportMaps& maps, float4* Uout, const ChemParams& cp, const LevelDev& L0,
              int* queue, unsigned int* qcount, Partial* parts, int nblk, bool bcgen, cudaStream_t st)
 {
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(fused_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<G>()) != cudaSuccess) return 0;
-    if (cudaFuncSetAttribute(fused_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<G>()) != cudaSuccess) return 0;
-    configured = true;
-  }
   if (bcgen) fused_kernel<G, true><<<nblk, NT, fused_smem<G>(), st>>>(p, maps, Uout, cp, L0, queue, qcount, parts);
   else fused_kernel<G, false><<<nblk, NT, fused_smem<G>(), st>>>(p, maps, Uout, cp, L0, queue, qcount, parts);
   return 1;
 }
 
+template <int G>
+cudaError_t configure_G()
+{
+  cudaError_t e = cudaFuncSetAttribute(fused_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<G>());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(fused_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<G>());
+}
+
 }  // namespace
+
+// Per-device set-up (emma_rt_init, handle's device current): dynamic shared memory opt-in of the kernels for G groups
+cudaError_t configure_fused(int G)
+{
+  switch (G) {
+    case 1: return configure_G<1>();
+    case 2: return configure_G<2>();
+    case 3: return configure_G<3>();
+    default: return configure_G<4>();
+  }
+}
 
 // CTAs resident per SM of the fused pass (one: its ring fills the shared memory) -- for the z-chunk cost model
 int fused_ctas_per_sm() { return CTAS_PER_SM; }

@@ -263,17 +263,21 @@ template <bool DIAG, bool BCGEN>
 cudaError_t launch_variant(const TransportParams& p, const TransportMaps& maps, float4* Uout, Partial* parts, int nblk,
                            cudaStream_t st)
 {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(transport_hll_kernel<DIAG, BCGEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
   transport_hll_kernel<DIAG, BCGEN><<<nblk, NT, SMEM, st>>>(p, maps, Uout, parts);
   return cudaSuccess;
 }
 
 }  // namespace
+
+// Per-device set-up (emma_rt_init, handle's device current): dynamic shared memory opt-in
+cudaError_t configure_transport_hll()
+{
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(transport_hll_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(transport_hll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(transport_hll_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(transport_hll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+}
 
 int hll_ctas_per_sm() { return 2; }
 

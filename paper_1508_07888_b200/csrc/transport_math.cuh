@@ -37,6 +37,14 @@ __device__ __forceinline__ float sel_ge(float x, float lo, float v)
   return d;
 }
 
+// 1 / x when x > 1, else 1 (the reciprocal is issued under the predicate)
+__device__ __forceinline__ float rcp_if_gt1(float x)
+{
+  float d;
+  asm("{\n\t.reg .pred p;\n\tsetp.gt.f32 p, %1, 0f3F800000;\n\tmov.f32 %0, 0f3F800000;\n\t@p rcp.approx.ftz.f32 %0, %1;\n\t}" : "=f"(d) : "f"(x));
+  return d;
+}
+
 __device__ __forceinline__ void closure_ab(const float4& U, float& a, float& b)
 {
   // A2: N <= 0 -> f = 0.  A denormal N (light that has just reached a dark cell) counts as 0: rcp.ftz of it is inf.
@@ -45,11 +53,14 @@ __device__ __forceinline__ void closure_ab(const float4& U, float& a, float& b)
   const float f2raw = fmaf(rx, rx, fmaf(ry, ry, rz * rz));
   const float f2 = fminf(f2raw, 1.f);          // A2: f clipped to [0,1]
   const float s = fsqrt(fmaf(-3.f, f2, 4.f));
-  const float q = f2 * frcp(2.f + s);
+  const float r2s = frcp(2.f + s);
+  const float q = f2 * r2s;
   a = fmaf(-U.x, q, 0.33333334f * U.x);
+  // b = 3 q / (N f^2) = 3 / ((2 + s) N) * (f2 / f2raw): the last factor is 1 unless f was clipped (rare), so the
+  // reciprocal of f2raw is predicated on the clip and costs no MUFU cycle otherwise.
   // A1: |F| = 0 -> no n(x)n term; below f^2 = 1e-30 the term (<= f^2 N) is far under fp32 resolution of a
   // (f2raw is +inf or NaN only for non-finite inputs, which the diagnostics report)
-  b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
+  b = sel_ge(f2raw, 1.0000001e-30f, 3.f * r2s * rN * rcp_if_gt1(f2raw));
 }
 
 // map an index that may be one cell outside [0,n) through the boundary condition of that face (A13)

@@ -18,6 +18,7 @@
 // __syncthreads per plane.
 #include <cuda.h>
 
+#include "async_copy.cuh"
 #include "emma_rt_internal.cuh"
 #include "transport_math.cuh"
 
@@ -37,34 +38,7 @@ constexpr int COLB = TY * 16;                  // bytes of one halo column
 constexpr int STAGE_BYTES = STAGE_ROWS + 2 * COLB;     // = bytes one plane's five boxes deliver
 constexpr int AB_BYTES = STAGE_BYTES / 2;      // closure plane: float2 (a, b) at half the byte offset of the cell
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
-{
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-  unsigned done;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-  } while (!done);
-}
-// one box of a rank-3 tensor (x in floats, y, z' = group * n + z) -> shared memory, completion on an mbarrier
-__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int cx, int cy, int cz)
-{
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-      :: "r"(dst), "l"(map), "r"(bar), "r"(cx), "r"(cy), "r"(cz) : "memory");
-}
+using namespace acp;
 
 struct TileT {                                 // per-thread constants of the march
   int own0;                                    // byte offset of my first cell inside a stage (second = own0 + ROWB)
@@ -150,8 +124,7 @@ transport_tma_kernel(const TransportParams p, const __grid_constant__ TransportM
 
   if (t == 0) {
     for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_fence_init();
   }
   __syncthreads();
   if (t == 0) {
@@ -327,13 +300,6 @@ template <int NST, bool DIAG, bool BCGEN>
 cudaError_t launch_variant(const TransportParams& p, const TransportMaps& maps, float4* Uout, Partial* parts, int nblk,
                            cudaStream_t st)
 {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(transport_tma_kernel<NST, DIAG, BCGEN>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>());
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
   transport_tma_kernel<NST, DIAG, BCGEN><<<nblk, NT, smem_bytes<NST>(), st>>>(p, maps, Uout, parts);
   return cudaSuccess;
 }
@@ -348,7 +314,26 @@ cudaError_t launch_nst(const TransportParams& p, const TransportMaps& maps, floa
   return launch_variant<NST, false, false>(p, maps, Uout, parts, nblk, st);
 }
 
+template <int NST>
+cudaError_t configure_nst()
+{
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(transport_tma_kernel<NST, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>())) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(transport_tma_kernel<NST, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>())) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(transport_tma_kernel<NST, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>())) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(transport_tma_kernel<NST, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<NST>());
+}
+
 }  // namespace
+
+// Per-device set-up (emma_rt_init, handle's device current): dynamic shared memory opt-in of every ring depth
+cudaError_t configure_transport_tma()
+{
+  cudaError_t e;
+  if ((e = configure_nst<4>()) != cudaSuccess) return e;
+  if ((e = configure_nst<NST_DEFAULT>()) != cudaSuccess) return e;
+  return configure_nst<8>();
+}
 
 // Tensor maps of one radiation buffer U[G][n][n][n] float4, seen as a rank-3 fp32 tensor (4n, n, G n).
 // Returns 0 on success, the CUresult (or -1 when the driver entry point is missing) otherwise.

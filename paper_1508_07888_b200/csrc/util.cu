@@ -63,15 +63,18 @@ __global__ void export_kernel(int field, const LevelDev L, const float4* __restr
 }
 
 __global__ void import_kernel(int field, const LevelDev L, float4* __restrict__ Ug, float c_red, long long off,
-                              long long cnt, const void* __restrict__ src)
+                              long long cnt, const void* __restrict__ src, unsigned int* __restrict__ bad)
 {
   const float rc = 1.f / c_red;
+  unsigned int n_bad = 0;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
     const long long cell = off + i;
     switch (field) {
       case EMMA_RT_FIELD_U: { const float4 u = ((const float4*)src)[i]; Ug[cell] = make_float4(u.x, u.y * rc, u.z * rc, u.w * rc); break; }
       case EMMA_RT_FIELD_X: {
-        const float x = fminf(fmaxf(((const float*)src)[i], 0.f), 1.f);
+        const float xin = ((const float*)src)[i];
+        if (!(xin >= 0.f && xin <= 1.f)) n_bad++;                      // also NaN
+        const float x = (xin != xin) ? xin : fminf(fmaxf(xin, 0.f), 1.f);
         // 1-x is exact in fp32 for x in [0.5, 1] (Sterbenz), so the neutral fraction of the input is kept exactly
         L.xs[cell] = (x <= 0.5f) ? x : __int_as_float(__float_as_int(1.f - x) | 0x80000000);
         break;
@@ -79,13 +82,42 @@ __global__ void import_kernel(int field, const LevelDev L, float4* __restrict__ 
       case EMMA_RT_FIELD_T: {
         float x, y;
         decode_x(L.xs[cell], x, y);
+        const float Tin = ((const float*)src)[i];
+        if (!(Tin > 0.f && Tin < __int_as_float(0x7f800000))) n_bad++;
         // A10 in fp64, rounded once: eps = e/n0 = (3/2)(1+x) k_B T
-        L.eps[cell] = (float)(1.5 * 1.380649e-16 * (1.0 + (double)x) * (double)((const float*)src)[i]);
+        L.eps[cell] = (float)(1.5 * 1.380649e-16 * (1.0 + (double)x) * (double)Tin);
         break;
       }
-      case EMMA_RT_FIELD_N0: L.n0[cell] = ((const float*)src)[i]; break;
+      case EMMA_RT_FIELD_N0: {
+        const float v = ((const float*)src)[i];
+        if (!(v > 0.f && v < __int_as_float(0x7f800000))) n_bad++;
+        L.n0[cell] = v;
+        break;
+      }
     }
   }
+  if (bad && n_bad) atomicAdd(bad, n_bad);                             // rare: only invalid inputs get here
+}
+
+// sum of U[i].x over i < n, times dV: per-block fp64 partials in index order, then one block adds them in index order
+__global__ void __launch_bounds__(256)
+sum_N_kernel(const float4* __restrict__ U, long long n, double dV, Partial* __restrict__ parts)
+{
+  Acc a;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    a.total += (double)U[i].x;
+  a.total *= dV;
+  block_reduce_store(a, parts + blockIdx.x);
+}
+__global__ void __launch_bounds__(256)
+sum_parts_kernel(const Partial* __restrict__ parts, int n_parts, double* __restrict__ out)
+{
+  __shared__ Partial s_tot;
+  Acc a;
+  for (int i = threadIdx.x; i < n_parts; i += blockDim.x) a.total += parts[i].total;
+  block_reduce_store(a, &s_tot);
+  __syncthreads();
+  if (threadIdx.x == 0) *out = s_tot.total;
 }
 
 __global__ void set_bits_kernel(unsigned int* mask, const int* __restrict__ cells, int n)
@@ -119,13 +151,22 @@ int launch_export(int field, const LevelDev& L, const float4* Ug, float c_red, l
   return 1;
 }
 
+int launch_sum_N(const float4* U, long long n, double dV, Partial* scratch, double* out, cudaStream_t st)
+{
+  const long long want = (n + 255) / 256;
+  const int nb = (int)(want < 1024 ? (want > 0 ? want : 1) : 1024);
+  sum_N_kernel<<<nb, 256, 0, st>>>(U, n, dV, scratch);
+  sum_parts_kernel<<<1, 256, 0, st>>>(scratch, nb, out);
+  return 2;
+}
+
 int launch_import(int field, const LevelDev& L, float4* Ug, float c_red, long long off, long long cnt, const void* src,
-                  cudaStream_t st)
+                  unsigned int* bad, cudaStream_t st)
 {
   if (cnt <= 0) return 0;
   long long want = (cnt + 255) / 256;
   const int nb = (int)(want < 148 * 16 ? want : 148 * 16);
-  import_kernel<<<nb, 256, 0, st>>>(field, L, Ug, c_red, off, cnt, src);
+  import_kernel<<<nb, 256, 0, st>>>(field, L, Ug, c_red, off, cnt, src, bad);
   return 1;
 }
 

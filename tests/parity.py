@@ -57,19 +57,26 @@ def run_pair(w, n_steps, track_signatures=True, chemistry=None, thermal=None, ot
     return orc, gpu, flips, diags
 
 
-def clean_masks(w, flips, n_steps):
-    """Per level: True for cells farther than FLIP_RADIUS (L1, coarse cells, periodic) from every flip."""
+def clean_masks(w, flips, n_steps, radius=None):
+    """Per level: True for cells farther than `radius` (default FLIP_RADIUS; L1, coarse cells, periodic) from every flip.
+    A flip of step s has had n_steps - s steps to spread, so its radius is min(radius, n_steps - s).  The L1 balls are grown by
+    repeated 6-neighbour dilation of the seed grid (cost independent of the number of flips)."""
     n = w.n
-    near = np.zeros(n ** 3, bool)
+    RM = FLIP_RADIUS if radius is None else int(radius)
+    near = np.zeros((n, n, n), bool)                                  # [iz, iy, ix]
     if flips:
-        idx = np.arange(n ** 3)
-        X, Y, Z = idx % n, (idx // n) % n, idx // (n * n)
+        seeds = [np.zeros((n, n, n), bool) for _ in range(RM + 1)]
         for (step, _l, _c, c0) in flips:
-            R = min(FLIP_RADIUS, n_steps - step)
-            cx, cy, cz = c0 % n, (c0 // n) % n, c0 // (n * n)
-            d = (np.minimum(abs(X - cx), n - abs(X - cx)) + np.minimum(abs(Y - cy), n - abs(Y - cy))
-                 + np.minimum(abs(Z - cz), n - abs(Z - cz)))
-            near |= d <= R
+            R = max(0, min(RM, n_steps - step))
+            seeds[R][c0 // (n * n), (c0 // n) % n, c0 % n] = True
+        for R in range(RM, -1, -1):                                   # near = U_R dilate^R(seeds[R])
+            if R < RM and near.any():
+                grown = near.copy()
+                for ax in range(3):
+                    grown |= np.roll(near, 1, ax) | np.roll(near, -1, ax)
+                near = grown
+            near |= seeds[R]
+    near = near.reshape(-1)
     anc = coarse_ancestors(w)
     return [~near[a] for a in anc]
 
@@ -83,11 +90,28 @@ def absorption_condition(w, dt):
     return [1.0 + w.c_red * w.sigma_N[g] * y * w.n0[0].astype(np.float64) * dt for g in range(w.G)]
 
 
-def compare(orc, gpu, w, flips=None, n_steps=0, nf_floor=1e-12, nf_cond=None):
+def flip_distance(w, flips, rmax=12):
+    """L1 distance (coarse cells, periodic) of every coarse cell to the nearest flip, capped at rmax + 1."""
+    n = w.n
+    cur = np.zeros((n, n, n), bool)
+    for (_s, _l, _c, c0) in flips:
+        cur[c0 // (n * n), (c0 // n) % n, c0 % n] = True
+    dist = np.full((n, n, n), rmax + 1, np.int16)
+    dist[cur] = 0
+    for r in range(1, rmax + 1):
+        grown = cur.copy()
+        for ax in range(3):
+            grown |= np.roll(cur, 1, ax) | np.roll(cur, -1, ax)
+        dist[grown & ~cur] = r
+        cur = grown
+    return dist.reshape(-1)
+
+
+def compare(orc, gpu, w, flips=None, n_steps=0, nf_floor=1e-12, nf_cond=None, radius=None):
     """Error report.  Keys: N, F (A17 norms, clean coarse cells), x, T, xn (clean cells, all levels), *_near (cells
     within FLIP_RADIUS of a flip), flips, cells, near_cells.  nf_cond: optional per-group arrays dividing the N, F
     errors (see absorption_condition)."""
-    clean = clean_masks(w, flips or [], n_steps)
+    clean = clean_masks(w, flips or [], n_steps, radius)
     rep = {"flips": len(flips or []), "cells": int(sum(m.size for m in clean)),
            "near_cells": int(sum((~m).sum() for m in clean))}
     c = w.c_red

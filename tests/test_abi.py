@@ -56,6 +56,35 @@ def test_arena_bytes_validation_and_size(L):
     assert 2 * 3 * 512 ** 3 * 16 < big < 20e9
 
 
+def test_null_amr_arrays_are_refused_not_dereferenced(L):
+    """A refined description whose n_octs / parent arrays (or one level's parent list) are NULL is invalid: 0, no crash."""
+    cfg = B.make_config(8, 1, 1e22, 3e9, [1e-18], [1e-18], [4e-11])
+    a = B.Amr()
+    a.n_levels, a.n_octs, a.parent = 1, None, None
+    assert L.emma_rt_arena_bytes(C.byref(cfg), C.byref(a)) == 0
+    n_octs = (C.c_int64 * 1)(3)
+    a.n_octs = C.cast(n_octs, C.POINTER(C.c_int64))
+    assert L.emma_rt_arena_bytes(C.byref(cfg), C.byref(a)) == 0
+    par = (C.c_void_p * 1)(None)
+    a.parent = C.cast(par, C.POINTER(C.c_void_p))
+    assert L.emma_rt_arena_bytes(C.byref(cfg), C.byref(a)) == 0      # n_octs[0] = 3 with a NULL parent list
+    # init refuses the same without touching a device
+    h = C.c_void_p()
+    assert L.emma_rt_init(C.byref(h), C.byref(cfg), C.byref(a), None, None, 0) == E.EINVAL and not h.value
+
+
+def test_step_reads_no_environment(L):
+    """The tuning variables are read once, at init (include/emma_rt.h): no getenv outside emma_rt_init's helper."""
+    src = open(os.path.join(ROOT, "paper_1508_07888_b200", "csrc", "api.cu")).read()
+    assert src.count("getenv(") == 1
+    for f in os.listdir(os.path.join(ROOT, "paper_1508_07888_b200", "csrc")):
+        if f != "api.cu":
+            assert "getenv(" not in open(os.path.join(ROOT, "paper_1508_07888_b200", "csrc", f)).read(), f
+    hdr = open(os.path.join(ROOT, "include", "emma_rt.h")).read()
+    for v in re.findall(r'env_int\("(EMMA_RT_TUNE_[A-Z]+)"', src):
+        assert v in hdr, v
+
+
 def test_null_handle_calls_fail_cleanly(L):
     assert L.emma_rt_step(None, 1.0, 1, None) == E.EINVAL
     assert L.emma_rt_set_sources(None, 0, None, None) == E.EINVAL
