@@ -318,6 +318,8 @@ def run_ours(args):
         # BASELINE config 4: 256^3 coarse + 2 refined levels (CRTA); transport on the coarse level, chemistry on leaves
         w = make_config(4, n=None if n == 512 else n, seed=replica_seed(4, rank, world))
         n = w.n
+        if args.boost_sources != 1.0:               # brighter sources: the refined leaves around them sub-cycle hard (row a-5)
+            w.src_Q = w.src_Q * args.boost_sources
     elif args.amr_standard:
         # the standard (non-CRTA) AMR scheme on a jump-balanced config-4-like mesh
         from workloads.amr import make_amr_standard
@@ -588,6 +590,7 @@ def main():
     ap.add_argument("--skip-transport-only", action="store_true")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     ap.add_argument("--skip-initial-state", action="store_true", help="skip the no-warm-up leg (coupled_from_initial_state)")
+    ap.add_argument("--boost-sources", type=float, default=1.0, help="--config 4 only: multiply every source's Q (divergent sub-cycling on the refined levels)")
     ap.add_argument("--skip-extra", action="store_true", help="skip the config-4 (CRTA) and standard-AMR sub-records")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -32,6 +32,7 @@ struct Layout {
   size_t parent[MAXL + 1], anc0[MAXL + 1], child[MAXL + 1], Ut[MAXL + 1];
   size_t srcmask[MAXL + 1], src_cell[MAXL + 1], src_S[MAXL + 1];
   size_t queue, qcount, parts, diag;
+  size_t crta_oct[MAXL + 1], crta_side[MAXL + 1];   // deferred octs of the refined levels under CRTA (chemistry.cu)
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
   size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
@@ -44,6 +45,7 @@ struct Shape {
   long long ncell[MAXL + 1], nocts[MAXL + 1];
   long long max_src;
   bool record, need_queue, amr;
+  long long crta_cap[MAXL + 1];                 // octs the side buffer of a refined level holds (0: none)
 };
 
 bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
@@ -74,6 +76,9 @@ bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
   s.need_queue = c->chemistry != 0 && c->thermal != 0;
   if (c->amr_transport != 0 && c->amr_transport != 1) return false;
   s.amr = c->amr_transport == 1 && s.nl > 0;
+  for (int l = 0; l <= MAXL; l++) s.crta_cap[l] = 0;
+  if (!s.amr && s.need_queue)                   // a side-buffer slot for every oct: any number of octs can be deferred
+    for (int l = 1; l <= s.nl; l++) s.crta_cap[l] = s.nocts[l];
   if (s.amr && s.nl > 3) return false;          // partial-sum slots: 2^(nl+1) - 1 level sweeps per step
   return true;
 }
@@ -101,8 +106,14 @@ void make_layout(const Shape& s, Layout& L)
   L.refined0 = s.nl > 0 ? take((size_t)(s.ncell[0] + 31) / 32 * 4) : 0;
   long long qcells = s.ncell[0];
   if (s.amr) for (int l = 1; l <= s.nl; l++) qcells = std::max(qcells, s.ncell[l]);   // every level runs the two-pass chemistry
+  for (int l = 1; l <= s.nl; l++) qcells = std::max(qcells, 8 * s.crta_cap[l]);
   L.queue = s.need_queue ? take(qcells * 4) : 0;
   L.qcount = take(256);
+  for (int l = 1; l <= s.nl; l++)
+    if (s.crta_cap[l] > 0) {
+      L.crta_oct[l] = take((size_t)s.crta_cap[l] * 4);
+      L.crta_side[l] = take((size_t)s.G * s.crta_cap[l] * 8 * sizeof(float4));
+    }
   L.parts = take((size_t)PART_SLOTS * sizeof(Partial));
   L.diag = take(sizeof(DiagDev));
   if (s.amr) {
@@ -186,6 +197,16 @@ struct emma_rt {
     return (float4*)(arena + lay.aU[other ? 1 - acur[l] : acur[l]][l]);
   }
   Partial* parts() const { return (Partial*)(arena + lay.parts); }
+  CrtaQueue crta_queue(int l) const
+  {
+    CrtaQueue q;
+    q.cap = (int)sh.crta_cap[l];
+    q.oct_list = q.cap ? (int*)(arena + lay.crta_oct[l]) : nullptr;
+    q.side = q.cap ? (float4*)(arena + lay.crta_side[l]) : nullptr;
+    q.lqueue = q.cap ? (int*)(arena + lay.queue) : nullptr;
+    q.counters = (unsigned int*)(arena + lay.qcount);
+    return q;
+  }
   unsigned int* qcount() const { return (unsigned int*)(arena + lay.qcount); }
   DiagDev* diag() const { return (DiagDev*)(arena + lay.diag); }
 };
@@ -849,7 +870,7 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
       off += np;
       for (int l = s.nl; l >= 1; l--) {
         h->prof.begin(EMMA_RT_K_CHEM_REFINED);
-        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->sm_count, h->st);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], h->crta_queue(l), P + off, &np, h->sm_count, h->st);
         h->prof.end();
         off += np;
       }
@@ -880,7 +901,7 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
       // 2-4. CRTA: deepest refined level first (inject -> leaf chemistry -> restrict), then the unrefined coarse cells
       for (int l = s.nl; l >= 1; l--) {
         h->prof.begin(EMMA_RT_K_CHEM_REFINED);
-        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], P + off, &np, h->sm_count, h->st);
+        h->launches += launch_chem_refined(cp, h->lv, l, s.nl, U, s.ncell[0], h->crta_queue(l), P + off, &np, h->sm_count, h->st);
         h->prof.end();
         off += np;
       }

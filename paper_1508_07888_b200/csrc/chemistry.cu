@@ -223,19 +223,58 @@ __device__ __forceinline__ float oct_sum(float v)
   return v;
 }
 
+// Deferred octs of a refined level (row a-5; SURVEY.md section 7 hard part 6: the dense, source-hosting leaves need 10-60
+// evaluations of Eq. 43-48 while their warp-mates need one).  A leaf whose single fast-path attempt does not finish the
+// step makes its OCT deferred: the oct takes a slot, its finished members park their final radiation in the slot's side
+// buffer, its unfinished members go to the compacted leaf queue of chem_crta_tail_kernel (one lane per leaf, refilled as
+// soon as a leaf is done), and crta_restrict_kernel averages the slot afterwards.  Leaves keep no radiation between steps
+// (A14), so the side buffer is the only per-leaf radiation there is; it has a slot for every oct of the level (16 G bytes
+// per refined cell: 0.6 GB at config 4), so every leaf takes the same path in every run -- fast path here or tail there --
+// whatever order the slots are handed out in.  No atomics on data, fixed summation order: bit-reproducible.
+template <int G>
+__device__ __forceinline__ void oct_restrict_store(const CellState<G>& c, float e_den, bool leader, const LevelDev& L,
+                                                   const LevelDev& Lbelow, long long oct, float4* __restrict__ U0,
+                                                   long long ncell0, int level)
+{
+  // restriction: mean of the 8 children (A14)
+  float4 m[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    m[g].x = 0.125f * oct_sum(c.N[g]); m[g].y = 0.125f * oct_sum(c.px[g]);
+    m[g].z = 0.125f * oct_sum(c.py[g]); m[g].w = 0.125f * oct_sum(c.pz[g]);
+  }
+  const float xm = 0.125f * oct_sum(c.x), ym = 0.125f * oct_sum(c.y), em = 0.125f * oct_sum(e_den);
+  if (leader) {
+    const long long pc = L.parent[oct];                               // split cell on the level below
+    if (level == 1) {
+#pragma unroll
+      for (int g = 0; g < G; g++) U0[(size_t)g * ncell0 + pc] = m[g];
+    } else {
+#pragma unroll
+      for (int g = 0; g < G; g++) L.Ut[(size_t)g * L.nocts + oct] = m[g];
+    }
+    Lbelow.xs[pc] = encode_x(xm, ym);
+    Lbelow.eps[pc] = em / Lbelow.n0[pc];
+  }
+}
+
 template <int G>
 __global__ void __launch_bounds__(128, 8)
 chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow, const float4* __restrict__ Ut_above,
-                    long long nocts_above, float4* __restrict__ U0, long long ncell0, int level,
+                    long long nocts_above, float4* __restrict__ U0, long long ncell0, int level, const CrtaQueue q,
                     Partial* __restrict__ parts)
 {
   Acc acc;
   const long long ncell = L.ncell;                                    // multiple of 8
+  const int lane = threadIdx.x & 31;
+  const unsigned oct_mask = 0xffu << (lane & 24);                     // the 8 lanes of my oct
   for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += (long long)gridDim.x * blockDim.x) {
     const long long cell = base + threadIdx.x;
     const bool valid = cell < ncell;                                  // uniform per 8-lane group
     CellState<G> c;
-    float e_den = 0.f;                                                // energy per volume for the restriction
+    CellTally tl;
+    float rem = 0.f, dmin = FINF;
+    bool leaf = false;
 #pragma unroll
     for (int g = 0; g < G; g++) { c.N[g] = c.px[g] = c.py[g] = c.pz[g] = 0.f; }
     c.x = c.y = c.eps = c.n0 = 0.f;
@@ -244,21 +283,41 @@ chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow
       oct = cell >> 3;
       const int ch = L.child ? L.child[cell] : -1;
       if (ch < 0) {
-        // leaf: starts from the coarse ancestor's post-transport radiation (piecewise-constant injection)
+        // leaf: starts from the coarse ancestor's post-transport radiation (piecewise-constant injection); the first
+        // trip of the sub-cycle loop when it covers the whole step (as chem_main_bulk_kernel)
+        leaf = true;
         load_cell<G>(L, cell, U0, ncell0, (long long)L.anc0[oct], c);
-        CellTally tl;
-        float rem = cp.dt, dmin = FINF;
-        bool ok = true;
-        while (ok && rem > 0.f) ok = substep<G>(cp, c, rem, tl, dmin);
-        if (!ok) acc.err |= 1u;
-        L.xs[cell] = encode_x(c.x, c.y);
-        L.eps[cell] = c.eps;
-        if (cp.record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
-        fold(acc, tl, c.N, G, L.dV, L.dV_total);
-        acc.dtau_min = fminf(acc.dtau_min, dmin);
-        if (!finite_cell<G>(c)) acc.nonfinite++;
+        rem = cp.dt;
+        const float T = c.eps * frcp(KB15 * (1.f + c.x));
+        const Rates r = rates_at(T, cp.otsa, c.x, c.n0);
+        bool go = true;
+        if (cp.thermal) {
+          float hsum = 0.f;
+#pragma unroll
+          for (int g = 0; g < G; g++) hsum = fmaf(cp.csigE[g], c.N[g], hsum);
+          const float d = c.y * hsum - c.n0 * c.x * fmaf(c.y, r.cHI, c.x * r.cHII);
+          const float guess = first_guess(c.eps, d, cp.dt);
+          go = guess >= cp.dt;
+          if (go) dmin = guess;
+        }
+        float N1[G], iden[G], x1, y1, eps1;
+        if (go) go = attempt<G>(cp, c, r, cp.dt, N1, iden, x1, y1, eps1);
+        if (go) {
+          const float k = c.y * c.n0 * cp.dt;
+#pragma unroll
+          for (int g = 0; g < G; g++) {
+            tl.absorbed = fmaf(cp.csig[g] * k, N1[g], tl.absorbed);
+            tl.injected = fmaf(c.S[g], cp.dt, tl.injected);
+            c.N[g] = N1[g];
+            c.px[g] = decay(c.px[g], iden[g]); c.py[g] = decay(c.py[g], iden[g]); c.pz[g] = decay(c.pz[g], iden[g]);
+          }
+          tl.recomb = r.rec * cp.dt;
+          c.x = x1; c.y = y1; c.eps = eps1;
+          tl.nsub = 1;
+          rem = 0.f;
+        }
       } else {
-        // split cell: restricted values were written by the kernel of the level above
+        // split cell: restricted values were written by the kernels of the level above
 #pragma unroll
         for (int g = 0; g < G; g++) {
           const float4 u = Ut_above[(size_t)g * nocts_above + ch];
@@ -268,30 +327,135 @@ chem_refined_kernel(const ChemParams cp, const LevelDev L, const LevelDev Lbelow
         decode_x(L.xs[cell], c.x, c.y);
         if (cp.record) L.subc[cell] = 0;
       }
-      e_den = c.eps * c.n0;
     }
-    // restriction: mean of the 8 children (A14)
-    float4 m[G];
-#pragma unroll
-    for (int g = 0; g < G; g++) {
-      m[g].x = 0.125f * oct_sum(c.N[g]); m[g].y = 0.125f * oct_sum(c.px[g]);
-      m[g].z = 0.125f * oct_sum(c.py[g]); m[g].w = 0.125f * oct_sum(c.pz[g]);
-    }
-    const float xm = 0.125f * oct_sum(c.x), ym = 0.125f * oct_sum(c.y), em = 0.125f * oct_sum(e_den);
-    if (valid && (cell & 7) == 0) {
-      const long long pc = L.parent[oct];                             // split cell on the level below
-      if (level == 1) {
-#pragma unroll
-        for (int g = 0; g < G; g++) U0[(size_t)g * ncell0 + pc] = m[g];
-      } else {
-#pragma unroll
-        for (int g = 0; g < G; g++) L.Ut[(size_t)g * L.nocts + oct] = m[g];
+    // ---- octs with an unfinished leaf: take a slot of the side buffer (one atomic per such oct)
+    const bool unfinished = leaf && rem > 0.f;
+    const unsigned um = __ballot_sync(0xffffffffu, unfinished);
+    int slot = -1;
+    if (um) {
+      const bool oct_defers = (um & oct_mask) != 0u;
+      if (oct_defers && (lane & 7) == 0) slot = (int)atomicAdd(q.counters + 2, 1u);
+      slot = __shfl_sync(0xffffffffu, slot, lane & 24);              // < q.cap: there is a slot for every oct
+      if (oct_defers && (lane & 7) == 0) q.oct_list[slot] = (int)oct;
+      // unfinished leaves of deferred octs -> the compacted leaf queue (one warp-aggregated atomic)
+      const bool enq = unfinished && slot >= 0;
+      const unsigned em = __ballot_sync(0xffffffffu, enq);
+      if (em) {
+        const int leader = __ffs(em) - 1;
+        unsigned b = 0;
+        if (lane == leader) b = atomicAdd(q.counters, (unsigned)__popc(em));
+        b = __shfl_sync(0xffffffffu, b, leader);
+        if (enq) {
+          q.lqueue[b + __popc(em & ((1u << lane) - 1u))] = slot * 8 + (int)(cell & 7);
+          acc.ndefer++;
+        }
       }
-      Lbelow.xs[pc] = encode_x(xm, ym);
-      Lbelow.eps[pc] = em / Lbelow.n0[pc];
+    }
+    const bool deferred_oct = slot >= 0;
+    if (leaf && rem <= 0.f) {                                         // this leaf is finished (here)
+      L.xs[cell] = encode_x(c.x, c.y);
+      L.eps[cell] = c.eps;
+      if (cp.record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
+      fold(acc, tl, c.N, G, L.dV, L.dV_total);
+      acc.dtau_min = fminf(acc.dtau_min, dmin);
+      if (!finite_cell<G>(c)) acc.nonfinite++;
+    }
+    if (deferred_oct && valid && !(leaf && rem > 0.f)) {              // finished member of a deferred oct: park its radiation
+#pragma unroll
+      for (int g = 0; g < G; g++)
+        q.side[(size_t)g * q.cap * 8 + (size_t)slot * 8 + (cell & 7)] = make_float4(c.N[g], c.px[g], c.py[g], c.pz[g]);
+    }
+    oct_restrict_store<G>(c, c.eps * c.n0, valid && (cell & 7) == 0 && !deferred_oct, L, Lbelow, oct, U0, ncell0, level);
+  }
+  block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// persistent warps over the compacted queue of unfinished refined leaves (the refined-level twin of chem_tail_kernel):
+// each lane owns one leaf, advances it one accepted sub-step per trip, refills when done
+template <int G>
+__global__ void __launch_bounds__(128)
+chem_crta_tail_kernel(const ChemParams cp, const LevelDev L, const float4* __restrict__ U0, long long ncell0,
+                      const CrtaQueue q, Partial* __restrict__ parts)
+{
+  Acc acc;
+  const unsigned nq = q.counters[0];
+  const int lane = threadIdx.x & 31;
+  CellState<G> c;
+  CellTally tl;
+  float rem = 0.f, dmin = FINF;
+  long long cell = -1;
+  int entry = 0;
+  bool has = false, exhausted = false;
+  for (;;) {
+    const unsigned want = __ballot_sync(0xffffffffu, !has && !exhausted);
+    if (want) {
+      const int leader = __ffs(want) - 1;
+      unsigned b = 0;
+      if (lane == leader) b = atomicAdd(q.counters + 1, (unsigned)__popc(want));
+      b = __shfl_sync(0xffffffffu, b, leader);
+      if (!has && !exhausted) {
+        const unsigned idx = b + __popc(want & ((1u << lane) - 1u));
+        if (idx < nq) {
+          entry = q.lqueue[idx];
+          cell = (long long)q.oct_list[entry >> 3] * 8 + (entry & 7);
+          load_cell<G>(L, cell, U0, ncell0, (long long)L.anc0[cell >> 3], c);
+          tl = CellTally();
+          rem = cp.dt; dmin = FINF;
+          has = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(0xffffffffu, has)) break;
+    if (has) {
+      const bool ok = substep<G>(cp, c, rem, tl, dmin);
+      if (!ok) acc.err |= 1u;
+      if (!ok || rem <= 0.f) {
+        L.xs[cell] = encode_x(c.x, c.y);
+        L.eps[cell] = c.eps;
+        if (cp.record) L.subc[cell] = min(tl.nsub, 65535u) | (min(tl.nhalv, 65535u) << 16);
+#pragma unroll
+        for (int g = 0; g < G; g++) q.side[(size_t)g * q.cap * 8 + entry] = make_float4(c.N[g], c.px[g], c.py[g], c.pz[g]);
+        fold(acc, tl, c.N, G, L.dV, L.dV_total);
+        acc.dtau_min = fminf(acc.dtau_min, dmin);
+        if (!finite_cell<G>(c)) acc.nonfinite++;
+        has = false;
+      }
     }
   }
   block_reduce_store(acc, parts + blockIdx.x);
+}
+
+// children mean of the deferred octs, after the tail: 8 lanes per slot
+template <int G>
+__global__ void __launch_bounds__(128)
+crta_restrict_kernel(const LevelDev L, const LevelDev Lbelow, float4* __restrict__ U0, long long ncell0, int level,
+                     const CrtaQueue q)
+{
+  const long long total = 8LL * min(q.counters[2], (unsigned)q.cap);
+  const int lane = threadIdx.x & 31;
+  for (long long base = (long long)blockIdx.x * blockDim.x + (threadIdx.x - lane); base < total; base += (long long)gridDim.x * blockDim.x) {
+    const long long i = base + lane;                                  // warp-uniform trip count: the shuffles below are safe
+    const bool valid = i < total;
+    CellState<G> c;
+#pragma unroll
+    for (int g = 0; g < G; g++) { c.N[g] = c.px[g] = c.py[g] = c.pz[g] = 0.f; }
+    c.x = c.y = c.eps = c.n0 = 0.f;
+    long long oct = 0;
+    if (valid) {
+      oct = q.oct_list[i >> 3];
+      const long long cell = oct * 8 + (i & 7);
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        const float4 u = q.side[(size_t)g * q.cap * 8 + i];
+        c.N[g] = u.x; c.px[g] = u.y; c.py[g] = u.z; c.pz[g] = u.w;
+      }
+      c.n0 = L.n0[cell]; c.eps = L.eps[cell];
+      decode_x(L.xs[cell], c.x, c.y);
+    }
+    oct_restrict_store<G>(c, c.eps * c.n0, valid && (i & 7) == 0, L, Lbelow, oct, U0, ncell0, level);
+  }
 }
 
 // chemistry off: Eq. 43 degenerates to N += S dt in the source cells (A9); sources are folded to the coarse level
@@ -413,24 +577,41 @@ int launch_chem_tail(const ChemParams& cp, const LevelDev& L0, float4* U, long l
 }
 
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U, long long ncell0,
-                        Partial* parts, int* n_parts, int sm_count, cudaStream_t st)
+                        const CrtaQueue& q, Partial* parts, int* n_parts, int sm_count, cudaStream_t st)
 {
   const LevelDev& L = lv[level];
   if (L.ncell == 0) { *n_parts = 0; return 0; }
   long long want = (L.ncell + 127) / 128;
   // persistent grid: whole waves of 8 CTAs per SM
   const long long cap = (sm_count > 0 && (long long)sm_count * 8 <= MAX_PART_BLOCKS) ? (long long)sm_count * 8 : MAX_PART_BLOCKS;
-  int nb = (int)(want < cap ? want : cap);
+  const int nb = (int)(want < cap ? want : cap);
   const float4* Ut_above = (level < n_levels) ? lv[level + 1].Ut : nullptr;
   const long long nocts_above = (level < n_levels) ? lv[level + 1].nocts : 0;
-  switch (cp.G) {
-    case 1: chem_refined_kernel<1><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
-    case 2: chem_refined_kernel<2><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
-    case 3: chem_refined_kernel<3><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
-    default: chem_refined_kernel<4><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, parts); break;
+  const bool tail = cp.thermal && q.cap > 0;                          // isothermal mode never leaves a leaf unfinished
+  int nt = 0;
+  if (tail) {
+    nt = sm_count * 8;
+    if (nt > MAX_PART_BLOCKS) nt = MAX_PART_BLOCKS;
+    cudaMemsetAsync(q.counters, 0, 3 * sizeof(unsigned int), st);
   }
-  *n_parts = nb;
-  return 1;
+  long long rwant = ((long long)q.cap * 8 + 127) / 128;
+  const int nr = (int)(rwant < cap ? rwant : cap);
+#define CRTA_LAUNCH(GG)                                                                                                       \
+  chem_refined_kernel<GG><<<nb, 128, 0, st>>>(cp, L, lv[level - 1], Ut_above, nocts_above, U, ncell0, level, q, parts);          \
+  if (tail) {                                                                                                                 \
+    chem_crta_tail_kernel<GG><<<nt, 128, 0, st>>>(cp, L, U, ncell0, q, parts + nb);                                             \
+    crta_restrict_kernel<GG><<<nr, 128, 0, st>>>(L, lv[level - 1], U, ncell0, level, q);                                        \
+  }
+  switch (cp.G) {
+    case 1: { CRTA_LAUNCH(1) } break;
+    case 2: { CRTA_LAUNCH(2) } break;
+    case 3: { CRTA_LAUNCH(3) } break;
+    default: { CRTA_LAUNCH(4) } break;
+  }
+#undef CRTA_LAUNCH
+  if (tail) cudaMemsetAsync(q.counters, 0, 3 * sizeof(unsigned int), st);   // the level-0 passes share the queue and its counters
+  *n_parts = nb + nt;
+  return tail ? 3 : 1;
 }
 
 int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts, int* n_parts,

@@ -66,6 +66,15 @@ struct LevelDev {
   double dV_total;         // = dV; 0 for a sweep that must not add to the photon total (see fold())
 };
 
+// Deferred octs of a refined level under CRTA (chemistry.cu: chem_refined_kernel and its tail)
+struct CrtaQueue {
+  int cap;                       // octs the side buffer holds
+  int* oct_list;                 // [cap] slot -> oct of this level
+  float4* side;                  // [G][cap * 8] radiation of the members of a deferred oct after the step
+  int* lqueue;                   // [<= cap * 8] deferred leaves: slot * 8 + child
+  unsigned int* counters;        // [0] leaves queued, [1] leaves taken by the tail, [2] octs deferred
+};
+
 struct TransportParams {
   int n, G;
   int bc[6];
@@ -137,7 +146,7 @@ int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in,
                          int* n_parts, cudaStream_t st);
 int hll_ctas_per_sm();
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U,
-                        long long ncell0, Partial* parts, int* n_parts, int sm_count, cudaStream_t st);
+                        long long ncell0, const CrtaQueue& q, Partial* parts, int* n_parts, int sm_count, cudaStream_t st);
 int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts,
                           int* n_parts, cudaStream_t st);
 int launch_finalize(const Partial* parts, int n_parts, DiagDev* diag, unsigned int* qcount, double t_sim,
