@@ -489,7 +489,9 @@ def run_ours(args):
     h2d = sum(t.numel() * 4 for t in hU) + hx.numel() * 4 + hT.numel() * 4
     d2h = h2d
 
-    def e2e_step():
+    use_host = args.config == 5 and not amr and not args.unfused and not args.hll
+
+    def e2e_serial():
         for g in range(G):
             assert gpu.write(E.FIELD_U, 0, g, hU[g]) == E.OK
         assert gpu.write(E.FIELD_X, 0, 0, hx) == E.OK
@@ -501,6 +503,13 @@ def run_ours(args):
         assert gpu.read_into(E.FIELD_X, 0, 0, hx) == E.OK
         assert gpu.read_into(E.FIELD_T, 0, 0, hT) == E.OK
 
+    def e2e_step():
+        if use_host:                                              # host state in, host state out, slab-pipelined (one C-ABI call)
+            rc, _ = gpu.step_host(dt, hU, hx, hT, diag=False)
+            assert rc == E.OK, gpu.last_error()
+        else:
+            e2e_serial()
+
     e2e_step()                                                # warm-up (page-locks, first-touch)
     barrier()
     t0 = time.perf_counter()
@@ -510,7 +519,17 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, dist, "cuda")
     e2e = {"value": units_per_step * Ke * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
-           "d2h_bytes_per_step": d2h, "steps": Ke, "ms_per_step": 1e3 * e2e_s / Ke}
+           "d2h_bytes_per_step": d2h, "steps": Ke, "ms_per_step": 1e3 * e2e_s / Ke,
+           "api": "emma_rt_step_host (z-slab pipeline: H2D, fused pass, D2H on three streams)" if use_host
+                  else "emma_rt_write x5 -> emma_rt_step -> emma_rt_read x5",
+           "link_GBps_each_way": h2d / (e2e_s / Ke) / 1e9}
+    if use_host:                                                  # the same bytes through the serial calls, for comparison
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(2):
+            e2e_serial()
+        barrier()
+        e2e["serial_write_step_read_ms_per_step"] = 1e3 * (time.perf_counter() - t0) / 2
     gpu.close()
 
     # ---------------- oracle on the host cores, bounded sample (rank 0, N = 1 only)

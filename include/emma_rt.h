@@ -168,6 +168,24 @@ EMMA_RT_API double emma_rt_dt_cfl(const emma_rt* h, double courant);
  * EMMA_RT_ESUBCYCLE if the last step saw them (the step still completed). */
 EMMA_RT_API int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last);
 
+/* One coupled step for a caller whose state lives in HOST memory -- the paper's own mode of operation, whose host <-> device
+ * traffic took ~70 % of its GPU engines' time.  Equivalent, bit for bit, to
+ *     emma_rt_write(U_g, X, T from `in`) -> emma_rt_step(h, dt, 1, diag) -> emma_rt_read(U_g, X, T into `out`),
+ * but the grid goes through the device in z-slabs on three streams: the upload of slab k+1, the fused transport +
+ * chemistry pass over slab k and the download of slab k-1 overlap, so both directions of the link are busy at once.
+ * `in` and `out` are level-0 host arrays (U[g]: n^3 x (N,Fx,Fy,Fz) per group; x, T: n^3), pinned for the copies to be
+ * asynchronous (pageable memory works, serialised); `out` may be the same arrays as `in`.  n0 and the sources stay on the
+ * device.  Needs a uniform grid (n_levels = 0), chemistry = 1, the GLF flux, the fused schedule and no inflow face, else
+ * EMMA_RT_ESTATE.  Waits for completion; afterwards the device holds the new state too.  Errors as emma_rt_step, plus
+ * EMMA_RT_EINVAL for invalid x / T in `in` (see "Input validation"; the step has then run on the clamped values). */
+typedef struct {
+  float* const* U;              /* [n_groups] -> n^3 x 4 floats */
+  float* x;                     /* n^3 */
+  float* T;                     /* n^3 */
+} emma_rt_host_state;
+EMMA_RT_API int emma_rt_step_host(emma_rt* h, double dt, const emma_rt_host_state* in, const emma_rt_host_state* out,
+                                  emma_rt_diag* diag_last /* nullable */);
+
 /* Copy a field of one level (and group) out of / into the library.  dst/src holds exactly n_cells(level) elements
  * of the field's type; `bytes` must match.  *_is_device != 0: the pointer is a device pointer on the same device
  * and the copy is stream-ordered; otherwise it is a host pointer and the call waits for the stream. */

@@ -17,7 +17,7 @@ FIELD_U, FIELD_N, FIELD_F, FIELD_X, FIELD_T, FIELD_E, FIELD_N0, FIELD_SUBCYCLES,
 _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYCLES: (1, np.uint32)}
 
 EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources", "emma_rt_dt_cfl", "emma_rt_step",
-                    "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
+                    "emma_rt_step_host", "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
                     "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_set_inflow", "emma_rt_last_error", "emma_rt_free"]
 FLUX_GLF, FLUX_HLL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
@@ -47,6 +47,10 @@ class Amr(C.Structure):
 class Fields(C.Structure):
     _fields_ = [("U0", C.POINTER(C.c_void_p)), ("n0", C.POINTER(C.c_void_p)), ("x", C.POINTER(C.c_void_p)),
                 ("T", C.POINTER(C.c_void_p))]
+
+
+class HostState(C.Structure):
+    _fields_ = [("U", C.POINTER(C.c_void_p)), ("x", C.c_void_p), ("T", C.c_void_p)]
 
 
 class Diag(C.Structure):
@@ -86,6 +90,8 @@ def lib():
     L.emma_rt_dt_cfl.argtypes = [C.c_void_p, C.c_double]
     L.emma_rt_step.restype = C.c_int
     L.emma_rt_step.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.POINTER(Diag)]
+    L.emma_rt_step_host.restype = C.c_int
+    L.emma_rt_step_host.argtypes = [C.c_void_p, C.c_double, C.POINTER(HostState), C.POINTER(HostState), C.POINTER(Diag)]
     L.emma_rt_read.restype = C.c_int
     L.emma_rt_read.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t, C.c_int32]
     L.emma_rt_write.restype = C.c_int
@@ -252,6 +258,27 @@ class EmmaRT:
 
     def step(self, dt, n_steps=1, diag=True):
         return emma_rt_step(self.h, dt, n_steps, diag)
+
+    def step_host(self, dt, U, x, T, U_out=None, x_out=None, T_out=None, diag=True):
+        """One coupled step on HOST state (emma_rt_step_host): U = list of G arrays [n^3, 4], x, T = [n^3]; numpy arrays or
+        (pinned) torch CPU tensors, float32, contiguous.  Outputs default to the inputs (in place).  Returns (rc, diag)."""
+        def ptr(a):
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"]
+                return a.ctypes.data
+            assert a.dtype == self._torch.float32 and a.is_contiguous() and not a.is_cuda
+            return a.data_ptr()
+
+        def state(Us, xs, Ts):
+            hs = HostState()
+            arr = (C.c_void_p * self.G)(*[ptr(u) for u in Us])
+            hs.U, hs.x, hs.T = C.cast(arr, C.POINTER(C.c_void_p)), ptr(xs), ptr(Ts)
+            return hs, arr
+        si, keep_i = state(U, x, T)
+        so, keep_o = state(U if U_out is None else U_out, x if x_out is None else x_out, T if T_out is None else T_out)
+        d = Diag()
+        rc = lib().emma_rt_step_host(self.h, float(dt), C.byref(si), C.byref(so), C.byref(d) if diag else None)
+        return rc, (d.as_dict() if diag else None)
 
     def level_cells(self, level):
         return lib().emma_rt_level_cells(self.h, level)

@@ -32,6 +32,7 @@ struct Layout {
   size_t parent[MAXL + 1], anc0[MAXL + 1], child[MAXL + 1], Ut[MAXL + 1];
   size_t srcmask[MAXL + 1], src_cell[MAXL + 1], src_S[MAXL + 1];
   size_t queue, qcount, parts, diag;
+  size_t host_stage;                                // one exported slab of emma_rt_step_host: U (G float4) + x + T
   size_t crta_oct[MAXL + 1], crta_side[MAXL + 1];   // deferred octs of the refined levels under CRTA (chemistry.cu)
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
@@ -45,7 +46,8 @@ struct Shape {
   long long ncell[MAXL + 1], nocts[MAXL + 1];
   long long max_src;
   bool record, need_queue, amr;
-  long long crta_cap[MAXL + 1];                 // octs the side buffer of a refined level holds (0: none)
+  long long crta_cap[MAXL + 1];
+  int slab_planes;                              // planes per slab of emma_rt_step_host (0: not available)                 // octs the side buffer of a refined level holds (0: none)
 };
 
 bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
@@ -76,6 +78,8 @@ bool make_shape(const emma_rt_config* c, const emma_rt_amr* a, Shape& s)
   s.need_queue = c->chemistry != 0 && c->thermal != 0;
   if (c->amr_transport != 0 && c->amr_transport != 1) return false;
   s.amr = c->amr_transport == 1 && s.nl > 0;
+  // emma_rt_step_host streams the state through the device in z-slabs: ~32 slabs, at least 8 planes each
+  s.slab_planes = (s.nl == 0 && c->chemistry != 0) ? std::min(s.n, std::max(8, s.n / 32)) : 0;
   for (int l = 0; l <= MAXL; l++) s.crta_cap[l] = 0;
   if (!s.amr && s.need_queue)                   // a side-buffer slot for every oct: any number of octs can be deferred
     for (int l = 1; l <= s.nl; l++) s.crta_cap[l] = s.nocts[l];
@@ -114,6 +118,7 @@ void make_layout(const Shape& s, Layout& L)
       L.crta_oct[l] = take((size_t)s.crta_cap[l] * 4);
       L.crta_side[l] = take((size_t)s.G * s.crta_cap[l] * 8 * sizeof(float4));
     }
+  L.host_stage = s.slab_planes ? take((size_t)s.slab_planes * s.n * s.n * (16 * (size_t)s.G + 8)) : 0;
   L.parts = take((size_t)PART_SLOTS * sizeof(Partial));
   L.diag = take(sizeof(DiagDev));
   if (s.amr) {
@@ -188,6 +193,9 @@ struct emma_rt {
   int n_fix;                                   // level-0 leaves with a split face neighbour
   int n_slots[MAXL + 1];                       // faces of the leaves of a refined level towards a coarser leaf
   bool amr_dirty;                              // U was written: restrict bottom-up before the next step
+  cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of emma_rt_step_host (created at its first call)
+  std::vector<cudaEvent_t> ev_in, ev_c;          // per slab: inputs on the device / slab computed
+  cudaEvent_t ev_start = nullptr;
   char err[256];
 
   float4* U(int b) const { return (float4*)(arena + lay.U[b]); }
@@ -783,6 +791,35 @@ int set_sources_impl(emma_rt* h, int64_t n_src, const double* pos, const double*
   return EMMA_RT_OK;
 }
 
+// geometry- and physics-constants of one step of size dt (everything but the z-chunking of a particular kernel)
+void base_params(const emma_rt* h, double dt, TransportParams& tp, ChemParams& cp, bool& any_inflow)
+{
+  const Shape& s = h->sh;
+  const double c = h->cfg.c_red_cm_s;
+  tp.n = s.n; tp.G = s.G;
+  any_inflow = false;
+  for (int f = 0; f < 6; f++) { tp.bc[f] = h->cfg.bc[f]; any_inflow = any_inflow || h->cfg.bc[f] == EMMA_RT_BC_INFLOW; }
+  memcpy(tp.inflow, h->inflow, sizeof tp.inflow);
+  tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
+  tp.z_lo = 0; tp.z_hi = s.n;
+  tp.zchunk = s.n; tp.nzc = 1;
+  tp.nst = h->tune.nst;
+  tp.pf = 2;
+  tp.want_total = h->cfg.chemistry ? 0 : 1;
+  tp.nu = (float)(c * dt / h->dx);
+  tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
+  tp.c1 = (float)(0.5 * (c * dt / h->dx));
+  tp.dV = h->lv[0].dV;
+  memset(&cp, 0, sizeof cp);
+  cp.G = s.G; cp.otsa = h->cfg.otsa; cp.thermal = h->cfg.thermal; cp.max_halvings = h->cfg.max_halvings;
+  cp.record = s.record ? 1 : 0;
+  cp.dt = (float)dt; cp.e_tol = (float)h->cfg.e_tol;
+  for (int g = 0; g < s.G; g++) {
+    cp.csig[g] = (float)(c * h->cfg.sigma_N[g]);
+    cp.csigE[g] = (float)(c * (h->cfg.sigma_E[g] * h->cfg.E_mean[g] - h->cfg.sigma_N[g] * E_HI_ERG));   // PAPER.md:266
+  }
+}
+
 int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
 {
   if (!h) return EMMA_RT_EINVAL;
@@ -792,11 +829,9 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
   if (3.0 * c * dt > h->dx * (1.0 + 1e-12)) return fail(h, EMMA_RT_ECFL, "dt = %g exceeds dx/(3 c) = %g (A4)", dt, h->dx / (3 * c));
 
   TransportParams tp;
-  tp.n = s.n; tp.G = s.G;
+  ChemParams cp;
   bool any_inflow = false;
-  for (int f = 0; f < 6; f++) { tp.bc[f] = h->cfg.bc[f]; any_inflow = any_inflow || h->cfg.bc[f] == EMMA_RT_BC_INFLOW; }
-  memcpy(tp.inflow, h->inflow, sizeof tp.inflow);
-  tp.tiles_x = (s.n + 31) / 32; tp.tiles_y = (s.n + 15) / 16;
+  base_params(h, dt, tp, cp, any_inflow);
   // z chunks.  Every CTA costs (its planes + ~3 planes of prologue) and the SMs hold `per_sm` CTAs each, so a launch
   // takes ceil(blocks / (per_sm SMs)) rounds of (zchunk + 3) plane-times: pick the chunk count that minimises that
   // (at 512^3 x 3 one chunk per column is 1536 CTAs = 5.19 rounds, i.e. 14 % of the last round idle).
@@ -819,24 +854,7 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
     return (long long)per * q.nzc <= TRANSPORT_MAX_BLOCKS;
   };
   if (!pick_zchunks(tp, tp.tiles_x * tp.tiles_y * s.G, 2)) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
-  tp.nst = h->tune.nst;
-  tp.pf = 2;
   const bool use_tma = !any_inflow && h->tune.tma != 0;
-  tp.want_total = h->cfg.chemistry ? 0 : 1;
-  tp.nu = (float)(c * dt / h->dx);
-  tp.c0 = (float)(1.0 - 3.0 * (c * dt / h->dx));
-  tp.c1 = (float)(0.5 * (c * dt / h->dx));
-  tp.dV = h->lv[0].dV;
-
-  ChemParams cp;
-  memset(&cp, 0, sizeof cp);
-  cp.G = s.G; cp.otsa = h->cfg.otsa; cp.thermal = h->cfg.thermal; cp.max_halvings = h->cfg.max_halvings;
-  cp.record = s.record ? 1 : 0;
-  cp.dt = (float)dt; cp.e_tol = (float)h->cfg.e_tol;
-  for (int g = 0; g < s.G; g++) {
-    cp.csig[g] = (float)(c * h->cfg.sigma_N[g]);
-    cp.csigE[g] = (float)(c * (h->cfg.sigma_E[g] * h->cfg.E_mean[g] - h->cfg.sigma_N[g] * E_HI_ERG));   // PAPER.md:266
-  }
 
   // fused schedule (fused.cu): all G groups of a tile in one CTA, one CTA per SM
   const bool hll = h->flux == EMMA_RT_FLUX_HLL;
@@ -942,6 +960,139 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
   return EMMA_RT_OK;
 }
 
+// One coupled step for a caller whose state lives in HOST memory (include/emma_rt.h: emma_rt_step_host).  Same kernels
+// and arithmetic as write(U, X, T) -> step(dt, 1) -> read(U, X, T), but the grid goes through the device in z-slabs on
+// three streams, so the upload of slab k+1, the fused pass over slab k and the download of slab k-1 overlap: both copy
+// engines are busy at once (PCIe is full duplex) and the compute hides behind them.  The paper's own GPU engines spent
+// ~70 % of their time in exactly this traffic.
+int step_host_impl(emma_rt* h, double dt, const emma_rt_host_state* in, const emma_rt_host_state* out, emma_rt_diag* diag_last)
+{
+  if (!h || !in || !out || !in->U || !in->x || !in->T || !out->U || !out->x || !out->T) return EMMA_RT_EINVAL;
+  const Shape& s = h->sh;
+  const double c = h->cfg.c_red_cm_s;
+  if (!(dt > 0.0)) return fail(h, EMMA_RT_EINVAL, "dt must be > 0");
+  if (3.0 * c * dt > h->dx * (1.0 + 1e-12)) return fail(h, EMMA_RT_ECFL, "dt = %g exceeds dx/(3 c) = %g (A4)", dt, h->dx / (3 * c));
+  for (int g = 0; g < s.G; g++)
+    if (!in->U[g] || !out->U[g]) return fail(h, EMMA_RT_EINVAL, "NULL radiation array of group %d", g);
+  TransportParams tp;
+  ChemParams cp;
+  bool any_inflow = false;
+  base_params(h, dt, tp, cp, any_inflow);
+  if (s.slab_planes == 0 || any_inflow || h->flux != EMMA_RT_FLUX_GLF || !h->fused || !h->tune.fused)
+    return fail(h, EMMA_RT_ESTATE, "emma_rt_step_host needs a uniform grid, chemistry on, the GLF flux, the fused schedule and no inflow face");
+  tp.tiles_y = (s.n + fused_tile_y() - 1) / fused_tile_y();
+  const int nblk = tp.tiles_x * tp.tiles_y;                            // one CTA per tile column and slab
+  const int tail_blocks = std::min(h->sm_count * 8, MAX_PART_BLOCKS);
+  int zs = s.slab_planes;
+  while ((long long)((s.n + zs - 1) / zs) * (nblk + tail_blocks) > PART_SLOTS && zs < s.n) zs *= 2;   // fewer, thicker slabs
+  // thicker slabs than the staging area holds are never needed for n <= 1290 (41 x 81 tiles x 32 slabs fit the slots)
+  if (zs > s.slab_planes) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
+  const int K = (s.n + zs - 1) / zs;
+  if (!h->s_in) {
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming));
+  }
+  while ((int)h->ev_in.size() < K) {
+    cudaEvent_t a, b;
+    CUDA_TRY(h, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    h->ev_in.push_back(a); h->ev_c.push_back(b);
+  }
+  const size_t plane = (size_t)s.n * s.n;
+  const float cr = (float)c;
+  LevelDev& L0 = h->lv[0];
+  float4* Uold = h->U(h->cur);
+  float4* Unew = h->U(1 - h->cur);
+  unsigned int* bad_dev = h->qcount() + 32;
+  char* stage = h->arena + h->lay.host_stage;
+  auto z_lo = [&](int k) { return k * zs; };
+  auto z_hi = [&](int k) { return std::min(s.n, (k + 1) * zs); };
+
+  // the copy streams start after whatever the caller's stream still has in flight on this state
+  CUDA_TRY(h, cudaEventRecord(h->ev_start, h->st));
+  CUDA_TRY(h, cudaStreamWaitEvent(h->s_in, h->ev_start, 0));
+  CUDA_TRY(h, cudaStreamWaitEvent(h->s_out, h->ev_start, 0));
+
+  // ---- uploads, in the order the compute needs them: slab 0 reads the last plane of slab K-1 (periodic z), so K-1 goes
+  // first.  Raw bytes land in the state arrays themselves and are converted in place (F -> F/c, x -> code, T -> e/n0).
+  auto upload = [&](int k) -> int {
+    const size_t off = (size_t)z_lo(k) * plane, cnt = (size_t)(z_hi(k) - z_lo(k)) * plane;
+    for (int g = 0; g < s.G; g++) {
+      float4* Ug = Uold + (size_t)g * s.ncell[0];
+      CUDA_TRY(h, cudaMemcpyAsync(Ug + off, in->U[g] + 4 * off, cnt * 16, cudaMemcpyHostToDevice, h->s_in));
+      h->launches += launch_import(EMMA_RT_FIELD_U, L0, Ug, cr, (long long)off, (long long)cnt, Ug + off, nullptr, h->s_in);
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(L0.xs + off, in->x + off, cnt * 4, cudaMemcpyHostToDevice, h->s_in));
+    h->launches += launch_import(EMMA_RT_FIELD_X, L0, nullptr, cr, (long long)off, (long long)cnt, L0.xs + off, bad_dev, h->s_in);
+    CUDA_TRY(h, cudaMemcpyAsync(L0.eps + off, in->T + off, cnt * 4, cudaMemcpyHostToDevice, h->s_in));
+    h->launches += launch_import(EMMA_RT_FIELD_T, L0, nullptr, cr, (long long)off, (long long)cnt, L0.eps + off, bad_dev, h->s_in);
+    CUDA_TRY(h, cudaEventRecord(h->ev_in[k], h->s_in));
+    return EMMA_RT_OK;
+  };
+  int rc;
+  if (K > 1 && (rc = upload(K - 1)) != EMMA_RT_OK) return rc;
+  for (int k = 0; k < (K > 1 ? K - 1 : 1); k++)
+    if ((rc = upload(k)) != EMMA_RT_OK) return rc;
+
+  // ---- per slab: fused pass + tail on the caller's stream once its three input slabs are there; export + download behind it
+  int off_parts = 0;
+  Partial* P = h->parts();
+  int* queue = (int*)(h->arena + h->lay.queue);
+  for (int k = 0; k < K; k++) {
+    for (int q : {(k + K - 1) % K, k, (k + 1) % K}) CUDA_TRY(h, cudaStreamWaitEvent(h->st, h->ev_in[q], 0));
+    TransportParams fp = tp;
+    fp.z_lo = z_lo(k); fp.z_hi = z_hi(k);
+    fp.zchunk = fp.z_hi - fp.z_lo; fp.nzc = 1;
+    int np = 0;
+    h->prof.begin(EMMA_RT_K_FUSED);
+    const int kf = launch_fused(fp, h->tmaps_f[h->cur], Unew, cp, L0, queue, h->qcount(), P + off_parts, &np, h->st);
+    if (!kf) return fail(h, EMMA_RT_ECUDA, "fused launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    h->prof.end();
+    h->launches += kf;
+    off_parts += np;
+    if (cp.thermal) {
+      h->launches += launch_chem_tail(cp, L0, Unew, s.ncell[0], queue, h->qcount(), P + off_parts, &np, h->sm_count, h->st, &h->prof);
+      off_parts += np;
+      CUDA_TRY(h, cudaMemsetAsync(h->qcount(), 0, 8, h->st));           // queue counters of the next slab
+    }
+    CUDA_TRY(h, cudaEventRecord(h->ev_c[k], h->st));
+    // download: everything on s_out is in order, so the one staging slab is free again when the next export starts
+    CUDA_TRY(h, cudaStreamWaitEvent(h->s_out, h->ev_c[k], 0));
+    const size_t off = (size_t)z_lo(k) * plane, cnt = (size_t)(z_hi(k) - z_lo(k)) * plane;
+    char* sp = stage;
+    for (int g = 0; g < s.G; g++, sp += cnt * 16) {
+      h->launches += launch_export(EMMA_RT_FIELD_U, L0, Unew + (size_t)g * s.ncell[0], cr, (long long)off, (long long)cnt, sp, h->s_out);
+      CUDA_TRY(h, cudaMemcpyAsync(out->U[g] + 4 * off, sp, cnt * 16, cudaMemcpyDeviceToHost, h->s_out));
+    }
+    h->launches += launch_export(EMMA_RT_FIELD_X, L0, nullptr, cr, (long long)off, (long long)cnt, sp, h->s_out);
+    CUDA_TRY(h, cudaMemcpyAsync(out->x + off, sp, cnt * 4, cudaMemcpyDeviceToHost, h->s_out));
+    sp += cnt * 4;
+    h->launches += launch_export(EMMA_RT_FIELD_T, L0, nullptr, cr, (long long)off, (long long)cnt, sp, h->s_out);
+    CUDA_TRY(h, cudaMemcpyAsync(out->T + off, sp, cnt * 4, cudaMemcpyDeviceToHost, h->s_out));
+  }
+  h->cur = 1 - h->cur;
+  h->t_sim += dt;
+  h->prof.begin(EMMA_RT_K_FINALIZE);
+  h->launches += launch_finalize(P, off_parts, h->diag(), h->qcount(), h->t_sim, h->st);
+  h->prof.end();
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, cudaMemcpyAsync(h->diag_pinned, h->diag(), sizeof(DiagDev), cudaMemcpyDeviceToHost, h->st));
+  CUDA_TRY(h, cudaMemcpyAsync(&h->diag_pinned->pad_bad, bad_dev, 4, cudaMemcpyDeviceToHost, h->st));
+  CUDA_TRY(h, cudaStreamSynchronize(h->s_in));
+  CUDA_TRY(h, cudaStreamSynchronize(h->st));
+  CUDA_TRY(h, cudaStreamSynchronize(h->s_out));
+  if (h->diag_pinned->pad_bad) {
+    const unsigned int n_bad = h->diag_pinned->pad_bad;
+    CUDA_TRY(h, cudaMemsetAsync(bad_dev, 0, 4, h->st));
+    return fail(h, EMMA_RT_EINVAL, "%u invalid value(s) in the host state (need finite T > 0, 0 <= x <= 1)", n_bad);
+  }
+  if (diag_last) *diag_last = h->diag_pinned->d;
+  if (h->diag_pinned->d.n_nonfinite > 0) return fail(h, EMMA_RT_ENONFINITE, "%lld non-finite cells", (long long)h->diag_pinned->d.n_nonfinite);
+  if (h->diag_pinned->err_last & 1u) return fail(h, EMMA_RT_ESUBCYCLE, "sub-cycle guard hit (max_halvings or %d sub-steps)", EMMA_RT_MAX_SUBSTEPS);
+  return EMMA_RT_OK;
+}
+
 int read_impl(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
 {
   if (!h || !dst) return EMMA_RT_EINVAL;
@@ -1041,6 +1192,11 @@ int emma_rt_step(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last
   return guarded(h, true, [&] { return step_impl(h, dt, n_steps, diag_last); });
 }
 
+int emma_rt_step_host(emma_rt* h, double dt, const emma_rt_host_state* in, const emma_rt_host_state* out, emma_rt_diag* diag_last)
+{
+  return guarded(h, true, [&] { return step_host_impl(h, dt, in, out, diag_last); });
+}
+
 int emma_rt_read(emma_rt* h, int32_t field, int32_t level, int32_t group, void* dst, size_t bytes, int32_t dst_is_device)
 {
   return guarded(h, true, [&] { return read_impl(h, field, level, group, dst, bytes, dst_is_device); });
@@ -1102,6 +1258,11 @@ void emma_rt_free(emma_rt* h)
 {
   if (!h) return;
   if (h->diag_pinned) cudaFreeHost(h->diag_pinned);
+  for (cudaEvent_t e : h->ev_in) cudaEventDestroy(e);
+  for (cudaEvent_t e : h->ev_c) cudaEventDestroy(e);
+  if (h->ev_start) cudaEventDestroy(h->ev_start);
+  if (h->s_in) cudaStreamDestroy(h->s_in);
+  if (h->s_out) cudaStreamDestroy(h->s_out);
   for (cudaEvent_t e : h->prof.pool) cudaEventDestroy(e);
   delete h;
 }

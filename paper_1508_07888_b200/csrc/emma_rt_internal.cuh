@@ -35,6 +35,7 @@ struct DiagDev {                               // device-resident, written by fi
   emma_rt_diag d;
   unsigned int err_sticky;                     // OR of every step's flags since init (bit 0 ESUBCYCLE, bit 1 non-finite)
   unsigned int err_last;                       // flags of the last step
+  unsigned int pad_bad;                        // host side only: invalid-input count read back by emma_rt_step_host
 };
 
 // physics + geometry constants of the chemistry kernels
@@ -79,6 +80,7 @@ struct TransportParams {
   int n, G;
   int bc[6];
   int zchunk, nzc, tiles_x, tiles_y;
+  int z_lo, z_hi;          // planes [z_lo, z_hi) this launch covers (fused pass; the whole grid unless emma_rt_step_host slabs it)
   int nst;                 // stages of the TMA ring (transport_tma.cu)
   int pf;                  // planes ahead of the march that are prefetched into L2 (0 = off)
   int want_total;          // 1 when chemistry is off: the transport pass also sums N dV

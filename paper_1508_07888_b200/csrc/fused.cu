@@ -73,7 +73,7 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
   const int izc = bid;
   const int x0 = tix * TX, y0 = tiy * TY;
   const int wx = min(TX, n - x0), wy = min(TY, n - y0);
-  const int z0 = izc * p.zchunk, z1 = min(n, z0 + p.zchunk);
+  const int z0 = p.z_lo + izc * p.zchunk, z1 = min(p.z_hi, z0 + p.zchunk);
   const int zc = z1 - z0;
   const int t = threadIdx.x, lane = t & 31;
   const int tx = t % TX, ty = t / TX;

@@ -62,8 +62,10 @@ __global__ void export_kernel(int field, const LevelDev L, const float4* __restr
   }
 }
 
-__global__ void import_kernel(int field, const LevelDev L, float4* __restrict__ Ug, float c_red, long long off,
-                              long long cnt, const void* __restrict__ src, unsigned int* __restrict__ bad)
+// src may be the destination itself (emma_rt_step_host uploads raw bytes into the state arrays and converts in place):
+// every thread reads its element before it writes it, and no pointer is declared restrict
+__global__ void import_kernel(int field, const LevelDev L, float4* Ug, float c_red, long long off,
+                              long long cnt, const void* src, unsigned int* bad)
 {
   const float rc = 1.f / c_red;
   unsigned int n_bad = 0;
