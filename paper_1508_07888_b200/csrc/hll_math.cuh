@@ -22,7 +22,7 @@ __device__ __forceinline__ Aux make_aux(const float4& U)
   const float i2 = frcp(2.f + xi);
   const float q = f2 * i2;
   A.a = fmaf(-U.x, q, 0.33333334f * U.x);
-  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
+  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * i2 * rN * rcp_if_gt1(f2raw));       // = 3 q / (N f^2), see closure_ab
   if (f2raw > 1.f) { const float s = rsqrtf(f2raw); rx *= s; ry *= s; rz *= s; }   // f clipped to 1: r -> unit vector
   const float k = 2.f * (1.f - f2) * frcp(xi + 1.f), ixi = frcp(xi), t3 = 3.f * i2;
   const float sx = fsqrt(fmaxf(k * fmaf(-t3 * rx, rx, xi), 0.f));
@@ -34,15 +34,23 @@ __device__ __forceinline__ Aux make_aux(const float4& U)
   return A;
 }
 
-// flux vector G_d of a cell and the HLL combination for the face between L (towards -d) and R (towards +d)
+// packed helpers (sm_100a FADD2 / FMUL2 / FFMA2 on register pairs)
+__device__ __forceinline__ void sub2(float& dx, float& dy, float ax, float ay, float bx, float by)
+{
+  fma2(dx, dy, bx, by, -1.f, -1.f, ax, ay);
+}
+
+// flux vector G_d of a cell and the HLL combination for the face between L (towards -d) and R (towards +d):
+// H = wl G_L + wr G_R + wd (U_R - U_L), evaluated on the (N, phi_x) and (phi_y, phi_z) halves with packed arithmetic
 template <int D>
 __device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL, float lmL, float lpL,
                                            const float4& UR, float aR, float bR, float lmR, float lpR)
 {
   const float pL = comp<D>(UL), pR = comp<D>(UR);
   const float uL = bL * pL, uR = bR * pR;
-  float4 GL = make_float4(pL, uL * UL.y, uL * UL.z, uL * UL.w);
-  float4 GR = make_float4(pR, uR * UR.y, uR * UR.z, uR * UR.w);
+  float4 GL, GR;
+  GL.x = pL; GL.y = uL * UL.y; mul2(GL.z, GL.w, UL.z, UL.w, uL, uL);
+  GR.x = pR; GR.y = uR * UR.y; mul2(GR.z, GR.w, UR.z, UR.w, uR, uR);
   if (D == 0) { GL.y += aL; GR.y += aR; } else if (D == 1) { GL.z += aL; GR.z += aR; } else { GL.w += aL; GR.w += aR; }
   const float lp = fmaxf(0.f, fmaxf(lpL, lpR)), lm = fminf(0.f, fminf(lmL, lmR));
   const float den = lp - lm;
@@ -50,11 +58,11 @@ __device__ __forceinline__ float4 hll_face(const float4& UL, float aL, float bL,
   // denormal den (transverse speeds of ~1e-38 from rounding dust in phi), whose approximate reciprocal is inf
   const float inv = (den > 1e-20f) ? frcp(den) : 0.f;
   const float wl = lp * inv, wr = -lm * inv, wd = lp * lm * inv;
-  float4 H;
-  H.x = fmaf(wl, GL.x, fmaf(wr, GR.x, wd * (UR.x - UL.x)));
-  H.y = fmaf(wl, GL.y, fmaf(wr, GR.y, wd * (UR.y - UL.y)));
-  H.z = fmaf(wl, GL.z, fmaf(wr, GR.z, wd * (UR.z - UL.z)));
-  H.w = fmaf(wl, GL.w, fmaf(wr, GR.w, wd * (UR.w - UL.w)));
+  float4 H, dU;
+  sub2(dU.x, dU.y, UR.x, UR.y, UL.x, UL.y); sub2(dU.z, dU.w, UR.z, UR.w, UL.z, UL.w);
+  mul2(H.x, H.y, dU.x, dU.y, wd, wd); mul2(H.z, H.w, dU.z, dU.w, wd, wd);
+  fma2(H.x, H.y, GR.x, GR.y, wr, wr, H.x, H.y); fma2(H.z, H.w, GR.z, GR.w, wr, wr, H.z, H.w);
+  fma2(H.x, H.y, GL.x, GL.y, wl, wl, H.x, H.y); fma2(H.z, H.w, GL.z, GL.w, wl, wl, H.z, H.w);
   return H;
 }
 
@@ -72,7 +80,7 @@ __device__ __forceinline__ AuxD make_aux_dir(const float4& U, int d)
   const float i2 = frcp(2.f + xi);
   const float q = f2 * i2;
   A.a = fmaf(-U.x, q, 0.33333334f * U.x);
-  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * q * rN * frcp(f2raw));
+  A.b = sel_ge(f2raw, 1.0000001e-30f, 3.f * i2 * rN * rcp_if_gt1(f2raw));
   float rd = (d == 0) ? rx : (d == 1) ? ry : rz;
   if (f2raw > 1.f) rd *= rsqrtf(f2raw);
   const float k = 2.f * (1.f - f2) * frcp(xi + 1.f), ixi = frcp(xi), t3 = 3.f * i2;

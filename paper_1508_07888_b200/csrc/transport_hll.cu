@@ -86,14 +86,14 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     if (ty == 0 && y0 == 0 && p.bc[2] == EMMA_RT_BC_REFLECTIVE) sym = -1.f;
     if (ty == wy - 1 && y0 + wy == n && p.bc[3] == EMMA_RT_BC_REFLECTIVE) syp = -1.f;
   }
-  // halo cells: dealt round-robin over the warps, at most one per thread; a reflective ghost gets its aux from the
-  // mirrored state (face-normal component negated)
+  // halo cells: dealt in order, task h -> thread h (96 tasks = 3 whole warps; the others skip the work, and consecutive
+  // lanes read consecutive cells); a reflective ghost gets its aux from the mirrored state (face-normal component negated)
   int hoff = -1;
   float hsx = 1.f, hsy = 1.f;
   bool hin = false;                            // my halo cell is the ghost of an inflow face (A20): a prescribed state
   float4 hval = make_float4(0.f, 0.f, 0.f, 0.f);
   {
-    const int nh = 2 * wy + 2 * wx, h = lane * (NT / 32) + warp;
+    const int nh = 2 * wy + 2 * wx, h = t;
     if (BCGEN && h < nh) {
       const int face = (h < wy) ? (x0 == 0 ? 0 : -1) : (h < 2 * wy) ? (x0 + wx == n ? 1 : -1)
                      : (h < 2 * wy + wx) ? (y0 == 0 ? 2 : -1) : (y0 + wy == n ? 3 : -1);
