@@ -185,6 +185,7 @@ struct emma_rt {
   Profiler prof;
   TransportMaps tmaps[2];                      // TMA descriptors of U[0], U[1]
   TransportMaps tmaps_f[2];                    // the same with the fused pass's tile height
+  TransportMaps tmaps_h[2];                    // the same with the HLL pass's tile width
   int fused;                                   // schedule of the coupled step (emma_rt_set_schedule)
   int flux;                                    // interface flux of the transport update (emma_rt_set_flux)
   float4 inflow[6][MAXG];                      // ghost state (N, phi) of inflow faces (emma_rt_set_inflow)
@@ -326,7 +327,7 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
         // sparse correction of the leaves that touch a split cell
         h->prof.begin(EMMA_RT_K_TRANSPORT);
         if (hll) {
-          const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+          const int k = launch_transport_hll(hp, h->tmaps_h[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
           if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
           h->launches += k;
         } else if (use_tma) {
@@ -653,6 +654,8 @@ int init_impl(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, 
   for (int b = 0; b < 2; b++) {
     const int r = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps[b]);
     if (r != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", r);
+    const int rh = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_h[b], 16, hll_tile_x());
+    if (rh != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", rh);
     const int rf = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_f[b], fused_tile_y());
     if (rf != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", rf);
   }
@@ -858,7 +861,8 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
 
   // fused schedule (fused.cu): all G groups of a tile in one CTA, one CTA per SM
   const bool hll = h->flux == EMMA_RT_FLUX_HLL;
-  TransportParams hp = tp;                     // HLL pass (transport_hll.cu): one group per CTA, one CTA per SM
+  TransportParams hp = tp;                     // HLL pass (transport_hll.cu): one group per CTA, 31-cell-wide tiles
+  hp.tiles_x = (s.n + hll_tile_x() - 1) / hll_tile_x();
   if (hll && !pick_zchunks(hp, hp.tiles_x * hp.tiles_y * s.G, hll_ctas_per_sm())) return fail(h, EMMA_RT_EINVAL, "grid too large for the partial-sum slots");
   const bool fused = !hll && !any_inflow && h->cfg.chemistry && h->fused && h->tune.fused != 0;
   TransportParams fp = tp;
@@ -901,7 +905,7 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
     // 1. coarse transport, old buffer -> new buffer (Jacobi)
     h->prof.begin(EMMA_RT_K_TRANSPORT);
     if (hll) {
-      const int k = launch_transport_hll(hp, h->tmaps[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
+      const int k = launch_transport_hll(hp, h->tmaps_h[h->cur], h->U(1 - h->cur), P + off, &np, h->st);
       if (!k) return fail(h, EMMA_RT_ECUDA, "HLL transport launch failed: %s", cudaGetErrorString(cudaGetLastError()));
       h->launches += k;
     } else if (use_tma) {
