@@ -10,8 +10,12 @@
 //     the list of faces towards a coarser leaf with their six resolved coarse references, the leaves that receive
 //     deposits.  Siblings sit in the same 128-byte oct record and are exchanged by warp shuffles.  A face towards a split
 //     cell computes nothing (the fine cells behind it deposit).
-//   * amr_ghost_faces_kernel: the faces towards a coarser leaf, one thread per face from a host-built list: MinMod-limited
-//     linear ghost, flux, the fine cell's change and the same flux / 8 deposited into that leaf (red.global.add.f32).
+//   * amr_ghost_faces_kernel: the faces towards a coarser leaf, one thread per face from a host-built list, BEFORE the
+//     per-cell kernel of the sweep and from start-of-step states only: MinMod-limited linear ghost, flux, and two kinds of
+//     records -- the fine cell's change (one per face; the per-cell kernel adds its cell's <= 3 records to its result in
+//     the order x, y, z) and what the oct side hands to the coarse leaf (one per (oct, face), the two sub-steps summed by
+//     the thread that owns the side; the leaf gathers its <= 6 records in face order when its own step comes).  No
+//     read-modify-write of a state buffer and no atomics: the mode is bit-reproducible.
 //   * level 0 keeps the dense TMA kernel (transport_tma.cu) for the whole block; amr_fix0_kernel then recomputes the
 //     (few) leaves that touch a split cell without the faces towards it and adds what the fine cells deposited: the
 //     regular block stays on the bandwidth-bound kernel, the irregular part is a sparse second pass.
@@ -112,9 +116,28 @@ __device__ __forceinline__ float4 face_change(int a, int side, const float4& Ui,
   return face_change_pre(a, side, Ui, ai, bi, Un, an, bn, nuh);
 }
 
-__device__ __forceinline__ void red_add4(float4* p, const float4& v)
+// position of child k among the 4 cells of its oct's side across axis a, in the order of the host-built face list
+// (k increasing with bit a fixed): the bits of k without bit a
+__device__ __forceinline__ int side_pos(int k, int a)
 {
-  atomicAdd(p, v);                                                  // sm_90+: one 16-byte vector reduction (red.global.add.v4.f32)
+  return (a == 0) ? (k >> 1) : (a == 1) ? (((k >> 2) << 1) | (k & 1)) : (k & 3);
+}
+
+// What the fine cells behind face f of a leaf of level l handed to it during the two sub-steps of level l + 1 (Fig. 3 (i)-(ii)):
+// `o2` is the oct of level l + 1 that fills the split neighbour; its side facing back (f ^ 1) looks at a coarser leaf -- this
+// one.  The records are indexed by (oct, face) of the fine level and hold the sum of the two sub-steps (first + second, added by
+// the one thread that owns the side in amr_ghost_faces_kernel).
+template <int G>
+__device__ __forceinline__ void gather_side(const AmrDev& A, int l, int o2, int f, float4 (&sum)[G])
+{
+  const size_t s = (size_t)o2 * 6 + (f ^ 1);
+  const float4* __restrict__ R = A.depS[l + 1];
+  const size_t cap = (size_t)A.scap[l + 1];
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const float4 r = R[(size_t)g * cap + s];
+    sum[g].x += r.x; sum[g].y += r.y; sum[g].z += r.z; sum[g].w += r.w;
+  }
 }
 
 // ---- HLL variant (reading A19) of the refined-level kernels: face by face, no cancellation algebra ------------------
@@ -161,17 +184,29 @@ amr_transport_hll_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ 
     const bool hd = leaf && l < A.nl && ((A.hasdep[l][cell >> 5] >> (cell & 31)) & 1u);
     const int k = (int)(cell & 7);
     const long long oct = cell >> 3;
+    // what the finer level deposited into this leaf (only leaves next to a split cell of their own level: host bitmap)
+    float4 dsum[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) dsum[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (hd) {
+#pragma unroll
+      for (int a = 0; a < 3; a++) {
+        const int bit = (k >> a) & 1;
+        const int chs = child[cell ^ (1 << a)];                       // sibling across a
+        if (chs >= 0) gather_side<G>(A, l, chs, 2 * a + (1 - bit), dsum);
+        const int no = nbo[oct * 6 + 2 * a + bit];
+        if (no >= 0) {
+          const int cho = child[(((long long)no << 3) | (k ^ (1 << a)))];
+          if (cho >= 0) gather_side<G>(A, l, cho, 2 * a + bit, dsum);
+        }
+      }
+    }
 #pragma unroll
     for (int g = 0; g < G; g++) {
       const float4 Ui = valid ? Ul[(size_t)g * ncell + cell] : make_float4(0.f, 0.f, 0.f, 0.f);
       const Aux Xi = make_aux(Ui);
       float4 ac = Ui;
-      if (hd) {
-        float4* dp = A.dep[l] + (size_t)g * ncell + cell;
-        const float4 d = *dp;
-        ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
-        *dp = make_float4(0.f, 0.f, 0.f, 0.f);
-      }
+      ac.x += dsum[g].x; ac.y += dsum[g].y; ac.z += dsum[g].z; ac.w += dsum[g].w;
 #pragma unroll
       for (int a = 0; a < 3; a++) {
         const int bit = (k >> a) & 1;
@@ -189,7 +224,11 @@ amr_transport_hll_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ 
         }
         if (!leaf) continue;
         const int no = nbo[oct * 6 + 2 * a + bit];
-        if (no == -1) continue;
+        if (no <= -16) {                                               // a coarser leaf: the face's record (amr_ghost_faces_kernel)
+          const float4 d = A.dU[l][(size_t)g * A.ucap[l] + 4 * (size_t)(-16 - no) + side_pos(k, a)];
+          ac.x += d.x; ac.y += d.y; ac.z += d.z; ac.w += d.w;
+          continue;
+        }
         float4 Un;
         bool box = false;
         if (no >= 0) {
@@ -238,12 +277,8 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
   // a level has < 2^31 cells (checked at init): 32-bit cell indices inside a group, one base pointer per group
   const float4* __restrict__ Ug[G];
   float4* __restrict__ Vg[G];
-  float4* __restrict__ Dg[G];
 #pragma unroll
-  for (int g = 0; g < G; g++) {
-    Ug[g] = Ul + (size_t)g * ncell; Vg[g] = Unew + (size_t)g * ncell;
-    Dg[g] = (l < A.nl) ? A.dep[l] + (size_t)g * ncell : nullptr;
-  }
+  for (int g = 0; g < G; g++) { Ug[g] = Ul + (size_t)g * ncell; Vg[g] = Unew + (size_t)g * ncell; }
   const long long span = (long long)gridDim.x * blockDim.x;
   for (long long base = (long long)blockIdx.x * blockDim.x; base < ncell; base += span) {
     const long long cell = base + threadIdx.x;
@@ -253,22 +288,18 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
     // deposit is requested together with the cell's own state so that its latency overlaps with the face work
     const unsigned ci = (unsigned)cell;
     const bool hd = leaf && l < A.nl && ((A.hasdep[l][cell >> 5] >> (cell & 31)) & 1u);
-    float4 Ui[G], sum[G];
+    float4 Ui[G], sum[G], dsum[G];
     float ai[G], bi[G];
+    const int k = (int)(cell & 7);
+    const long long oct = cell >> 3;
 #pragma unroll
     for (int g = 0; g < G; g++) {
       Ui[g] = valid ? Ug[g][ci] : make_float4(0.f, 0.f, 0.f, 0.f);
-      sum[g] = hd ? Dg[g][ci] : make_float4(0.f, 0.f, 0.f, 0.f);
+      sum[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+      dsum[g] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 #pragma unroll
-    for (int g = 0; g < G; g++) {
-      closure_ab(Ui[g], ai[g], bi[g]);
-      // sum accumulates (U_n -/+ G_n) and is multiplied by nu/2 at the end: the deposit enters divided by nu/2
-      const float inv = 1.f / nuh;
-      sum[g].x *= inv; sum[g].y *= inv; sum[g].z *= inv; sum[g].w *= inv;
-    }
-    const int k = (int)(cell & 7);
-    const long long oct = cell >> 3;
+    for (int g = 0; g < G; g++) closure_ab(Ui[g], ai[g], bi[g]);
     int m = 0;                                                       // faces that exist
     int pmask = 0;                                                   // 2 bits per direction: (- face exists) | (+ face exists) << 1
     // outer faces, indices first (all three pointer loads, then all three split tests, in flight together); a face that
@@ -314,7 +345,7 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
         sum[g].z = fmaf(wgt, T.z, sum[g].z); sum[g].w = fmaf(wgt, T.w, sum[g].w);
       }
       if (reg[a]) { m++; pmask |= 1 << (2 * a + bit); }
-      if (leaf && no[a] <= -2) {                                     // box face: -2 - bc (rare: the slow path)
+      if (leaf && no[a] <= -2 && no[a] > -16) {                      // box face: -2 - bc (rare: the slow path)
         const NbRef r = box_ghost(-2 - no[a], a, bit, l, cell);
 #pragma unroll
         for (int g = 0; g < G; g++) {
@@ -353,10 +384,31 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
         }
       }
     }
-    if (hd) {
+    // the finer level's deposits (gathered here, after the regular faces: only few cells have any, and their dependent loads
+    // must not sit in front of everyone's neighbour loads), then the faces towards a coarser leaf (records of
+    // amr_ghost_faces_kernel), x, y, z: a fixed order of plain additions -- no other thread touches this cell
+    if (hd) {                                                        // gather the finer level's deposits (few cells)
 #pragma unroll
-      for (int g = 0; g < G; g++) Dg[g][ci] = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int a = 0; a < 3; a++) {
+        const int bit = (k >> a) & 1;
+        const int chs = child[cell ^ (1 << a)];                      // the sibling across a (same oct record)
+        if (chs >= 0) gather_side<G>(A, l, chs, 2 * a + (1 - bit), dsum);
+        if (chn[a] >= 0) gather_side<G>(A, l, chn[a], 2 * a + bit, dsum);
+      }
     }
+
+#pragma unroll
+    for (int g = 0; g < G; g++) { ac[g].x += dsum[g].x; ac[g].y += dsum[g].y; ac[g].z += dsum[g].z; ac[g].w += dsum[g].w; }
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+      if (no[a] <= -16) {
+        const size_t rec = 4 * (size_t)(-16 - no[a]) + side_pos(k, a);
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+          const float4 d = A.dU[l][(size_t)g * A.ucap[l] + rec];
+          ac[g].x += d.x; ac[g].y += d.y; ac[g].z += d.z; ac[g].w += d.w;
+        }
+      }
 #pragma unroll
     for (int g = 0; g < G; g++) Vg[g][ci] = ac[g];
   }
@@ -365,12 +417,12 @@ amr_transport_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew
 
 // The faces of refined leaves that look at a coarser leaf (resolution jump), one thread per face from a list the host
 // built once for the static mesh: the six coarse references are resolved once, then per group the MinMod ghost
-// (PAPER.md:436), the Eq. 32 flux, the fine cell's change (added to what amr_transport_kernel wrote) and the same
-// flux / 8 deposited into the coarse leaf (Fig. 3 (i)-(ii)).  Uniform work per thread: the irregular part of the
+// (PAPER.md:436), the Eq. 32 flux, the fine cell's change (a record the per-cell kernel adds to its result) and the same
+// flux / 8 for the coarse leaf (Fig. 3 (i)-(ii); a record per oct side that the leaf gathers).  Uniform work per thread: the irregular part of the
 // level is taken out of the per-cell kernel, where it made every warp on a patch boundary run the ghost code.
 template <int G, bool HLL>
 __global__ void __launch_bounds__(128)
-amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Unew, const int* __restrict__ slot_cell,
+amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, int sub, const int* __restrict__ slot_cell,
                        const int* __restrict__ slot_coarse, const unsigned char* __restrict__ slot_face,
                        const int* __restrict__ slot_refs, int n_slots)
 {
@@ -421,15 +473,19 @@ amr_ghost_faces_kernel(const AmrDev A, int l, float nuh, float4* __restrict__ Un
       closure_ab(Ui, ai, bi);
       d = face_change(a, side, Ui, ai, bi, Un, nuh);
     }
-    if (live) red_add4(Unew + (size_t)g * ncell + cell, d);         // a cell can have up to 3 such faces
+    if (live) A.dU[l][(size_t)g * A.ucap[l] + i] = d;               // read by the cell kernel of this level, this sweep
     // the 4 faces of one oct side are 4 consecutive list entries (aligned lanes) and share the coarse leaf: one deposit
     float4 s4 = d;
     s4.x += __shfl_xor_sync(0xffffffffu, s4.x, 1); s4.y += __shfl_xor_sync(0xffffffffu, s4.y, 1);
     s4.z += __shfl_xor_sync(0xffffffffu, s4.z, 1); s4.w += __shfl_xor_sync(0xffffffffu, s4.w, 1);
     s4.x += __shfl_xor_sync(0xffffffffu, s4.x, 2); s4.y += __shfl_xor_sync(0xffffffffu, s4.y, 2);
     s4.z += __shfl_xor_sync(0xffffffffu, s4.z, 2); s4.w += __shfl_xor_sync(0xffffffffu, s4.w, 2);
-    if ((threadIdx.x & 3) == 0 && live)
-      red_add4(A.dep[lc] + (size_t)g * ncc + c, make_float4(-0.125f * s4.x, -0.125f * s4.y, -0.125f * s4.z, -0.125f * s4.w));
+    if ((threadIdx.x & 3) == 0 && live) {                             // gathered by the coarse leaf when its own step comes
+      float4* rp = A.depS[l] + (size_t)g * A.scap[l] + (size_t)(cell >> 3) * 6 + f;
+      float4 r = make_float4(-0.125f * s4.x, -0.125f * s4.y, -0.125f * s4.z, -0.125f * s4.w);
+      if (sub) { const float4 o = *rp; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }   // second sub-step: first + second
+      *rp = r;
+    }
   }
 }
 
@@ -577,11 +633,20 @@ amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restr
       if (bc == EMMA_RT_BC_PERIODIC) idx[f] = cell + (side ? -(long long)(n - 1) : (long long)(n - 1)) * stride[a];
       else { idx[f] = cell; ghost[f] = bc; }
     }
-    if (!on[f]) idx[f] = cell;
   }
+  // what the fine cells behind the split neighbours handed to this leaf (Fig. 3 (i)-(ii)): the records of the two sub-steps
+  // of level 1, face by face in a fixed order
+  float4 dpv = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+  for (int f = 0; f < 6; f++)
+    if (!on[f]) {
+      const int o2 = A.child[0][idx[f]];
+      const size_t sd = (size_t)o2 * 6 + (f ^ 1);
+      const float4 r = A.depS[1][(size_t)g * A.scap[1] + sd];
+      dpv.x += r.x; dpv.y += r.y; dpv.z += r.z; dpv.w += r.w;
+      idx[f] = cell;
+    }
   const float4 Ui = Uold[(size_t)g * nc + cell];
-  float4* dp = A.dep[0] + (size_t)g * nc + cell;
-  const float4 dpv = *dp;
   float4 Un[6];
 #pragma unroll
   for (int f = 0; f < 6; f++) Un[f] = Uold[(size_t)g * nc + idx[f]];
@@ -611,7 +676,6 @@ amr_fix0_kernel(const AmrDev A, const float4* __restrict__ Uold, float4* __restr
   }
   ac.x += dpv.x; ac.y += dpv.y; ac.z += dpv.z; ac.w += dpv.w;
   if (HLL) realizable(ac);                                            // A19, after the deposits
-  *dp = make_float4(0.f, 0.f, 0.f, 0.f);
   Unew[(size_t)g * nc + cell] = ac;
 }
 
@@ -678,13 +742,13 @@ int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, do
   return 1;
 }
 
-int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
+int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, int sub, const int* slot_cell, const int* slot_coarse,
                            const unsigned char* slot_face, const int* slot_refs, int n_slots, int hll, cudaStream_t st)
 {
   if (n_slots == 0) return 0;
   const int nb = (n_slots + 127) / 128;
-  if (hll) { AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, true><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots))); }
-  else AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, false><<<nb, 128, 0, st>>>(A, level, nuh, Unew, slot_cell, slot_coarse, slot_face, slot_refs, n_slots)));
+  if (hll) { AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, true><<<nb, 128, 0, st>>>(A, level, nuh, sub, slot_cell, slot_coarse, slot_face, slot_refs, n_slots))); }
+  else AMR_DISPATCH(A.G, (amr_ghost_faces_kernel<GG, false><<<nb, 128, 0, st>>>(A, level, nuh, sub, slot_cell, slot_coarse, slot_face, slot_refs, n_slots)));
   return 1;
 }
 

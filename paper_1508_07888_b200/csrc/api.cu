@@ -36,7 +36,7 @@ struct Layout {
   size_t crta_oct[MAXL + 1], crta_side[MAXL + 1];   // deferred octs of the refined levels under CRTA (chemistry.cu)
   // standard AMR transport (A21): per-level radiation (double-buffered), deposits, oct neighbour pointers, level-0
   // child index and the list of level-0 leaves that touch a split cell
-  size_t aU[2][MAXL + 1], adep[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
+  size_t aU[2][MAXL + 1], adU[MAXL + 1], adepS[MAXL + 1], anbr[MAXL + 1], anbo[MAXL + 1], achild0, afix_cell, afix_mask;
   size_t aslot_cell[MAXL + 1], aslot_coarse[MAXL + 1], aslot_face[MAXL + 1], aslot_refs[MAXL + 1], ahasdep[MAXL + 1], arefined[MAXL + 1];   // faces of refined leaves towards a coarser leaf
   size_t total;
 };
@@ -132,10 +132,14 @@ void make_layout(const Shape& s, Layout& L)
         L.aslot_coarse[l] = take((size_t)s.nocts[l] * 24 * 4);
         L.aslot_face[l] = take((size_t)s.nocts[l] * 24);
         L.aslot_refs[l] = take((size_t)s.nocts[l] * 6 * 6 * 4);     // 6 neighbour references per oct side
+        // what a coarse-facing face does to its fine cell (one record per face and group) and what an oct side hands to
+        // its coarse leaf (one record per side and group, summed over the two sub-steps): written by amr_ghost_faces_kernel, read by the cell
+        // kernels of the two levels -- no read-modify-write, no atomics.  Worst-case capacity, like the lists
+        L.adU[l] = take((size_t)s.G * s.nocts[l] * 24 * sizeof(float4));
+        L.adepS[l] = take((size_t)s.G * s.nocts[l] * 6 * sizeof(float4));
         L.ahasdep[l] = take((size_t)(s.ncell[l] + 31) / 32 * 4);
         L.arefined[l] = take((size_t)(s.ncell[l] + 31) / 32 * 4);     // split cells of the level (chemistry skips them)
       }
-      if (l < s.nl) L.adep[l] = take((size_t)s.G * s.ncell[l] * sizeof(float4));
     }
     L.achild0 = take((size_t)s.ncell[0] * 4);
     L.afix_cell = take((size_t)s.nocts[1] * 6 * 4);
@@ -278,7 +282,9 @@ AmrDev amr_view(const emma_rt* h)
   for (int l = 0; l <= s.nl; l++) {
     A.ncell[l] = s.ncell[l];
     A.U[l] = h->Ulev(l);
-    A.dep[l] = l < s.nl ? (float4*)(h->arena + h->lay.adep[l]) : nullptr;
+    A.dU[l] = l >= 1 ? (float4*)(h->arena + h->lay.adU[l]) : nullptr;
+    A.depS[l] = l >= 1 ? (float4*)(h->arena + h->lay.adepS[l]) : nullptr;
+    A.ucap[l] = 24 * s.nocts[l]; A.scap[l] = 6 * s.nocts[l];
     A.child[l] = l == 0 ? (const int*)(h->arena + h->lay.achild0) : l < s.nl ? h->lv[l].child : nullptr;
     A.nbr[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbr[l]) : nullptr;
     A.nbo[l] = l >= 1 ? (const int*)(h->arena + h->lay.anbo[l]) : nullptr;
@@ -312,6 +318,7 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
     o.push_back({l, dtl, last});
   } };
   Rec::go(order, 0, s.nl, s.ncell, dt, true);
+  int sub_of[MAXL + 1] = {0};                     // a refined level is swept twice per step of the level below: first / second sub-step
   // worst-case partial-sum slots of one coarse step, checked BEFORE the first launch so that a refusal leaves the state
   // untouched: every sweep may use a transport grid, a chemistry main grid and a tail grid
   if ((long long)order.size() * 3 * MAX_PART_BLOCKS + TRANSPORT_MAX_BLOCKS > PART_SLOTS)
@@ -356,11 +363,14 @@ int step_amr(emma_rt* h, double dt, int n_steps, TransportParams& tp, const Tran
       } else {
         AmrDev A = amr_view(h);
         h->prof.begin(EMMA_RT_K_AMR_TRANSPORT);
-        h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, ihll, P + off, &np, h->st);
-        h->launches += launch_amr_ghost_faces(A, l, nuh, h->Ulev(l, 1), (const int*)(h->arena + h->lay.aslot_cell[l]),
+        // the faces towards a coarser leaf first: from the start-of-step states they write the per-face change records the
+        // cell kernel adds to its result and the per-side records the coarse leaf gathers when ITS step comes
+        h->launches += launch_amr_ghost_faces(A, l, nuh, sub_of[l], (const int*)(h->arena + h->lay.aslot_cell[l]),
                                               (const int*)(h->arena + h->lay.aslot_coarse[l]),
                                               (const unsigned char*)(h->arena + h->lay.aslot_face[l]),
                                               (const int*)(h->arena + h->lay.aslot_refs[l]), h->n_slots[l], ihll, h->st);
+        sub_of[l] ^= 1;
+        h->launches += launch_amr_transport(A, l, nuh, h->Ulev(l, 1), h->lv[l].dV, ihll, P + off, &np, h->st);
         h->prof.end();
         off += np;
         h->acur[l] = 1 - h->acur[l];
@@ -461,7 +471,6 @@ int init_amr_topology(emma_rt* h, const std::vector<std::vector<int>>& parent_h,
       if (pcell < 0) { nbo_h[l][i] = pcell - 1; continue; }              // -1 - bc  ->  -2 - bc
       nbo_h[l][i] = (l == 1) ? child0_h[pcell] : child_h[l - 1][pcell];  // oct of level l, or -1: coarser leaf
     }
-    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
   }
   // leaves of a refined level that touch a split cell of the same level (they receive deposits)
   for (int l = 1; l < s.nl; l++) {
@@ -516,6 +525,9 @@ int init_amr_topology(emma_rt* h, const std::vector<std::vector<int>>& parent_h,
             }
             slot_refs_h[l].push_back((int)q);
           }
+        // the side's index (= its first list entry / 4) replaces the "coarser leaf" code -1 of the neighbour-oct table: the
+        // cell kernels find their faces' records through it without another table
+        nbo_h[l][o * 6 + f] = -16 - (int)(slot_cell_h[l].size() >> 2);
         for (int k = 0; k < 8; k++) {                                    // always 4 entries per oct side (kept aligned)
           if (((k >> a) & 1) != side) continue;
           if (l < s.nl && child_h[l][(o << 3) | k] >= 0)
@@ -526,6 +538,7 @@ int init_amr_topology(emma_rt* h, const std::vector<std::vector<int>>& parent_h,
         }
       }
     h->n_slots[l] = (int)slot_cell_h[l].size();
+    CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.anbo[l], nbo_h[l].data(), nbo_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
     if (h->n_slots[l]) {
       CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_cell[l], slot_cell_h[l].data(), slot_cell_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));
       CUDA_TRY(h, cudaMemcpyAsync(h->arena + h->lay.aslot_coarse[l], slot_coarse_h[l].data(), slot_coarse_h[l].size() * 4, cudaMemcpyHostToDevice, h->st));

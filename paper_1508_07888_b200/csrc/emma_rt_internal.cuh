@@ -236,12 +236,17 @@ struct AmrDev {
   int bc[6];
   long long ncell[MAXL + 1];
   float4* U[MAXL + 1];          // current radiation of the level, [G][ncell]
-  float4* dep[MAXL + 1];        // change deposited into leaves by the fluxes of the level above, [G][ncell] (levels < nl)
+  float4* dU[MAXL + 1];         // [G][ucap] change of a fine cell by its face towards a coarser leaf, one record per face of the
+                                // host-built list (levels >= 1)
+  float4* depS[MAXL + 1];       // [G][scap] what an oct side hands to the coarse leaf behind it over the level's two sub-steps of the
+                                // coarse step (Fig. 3 (i)-(ii)), one record per (oct, face) (levels >= 1)
+  long long ucap[MAXL + 1], scap[MAXL + 1];
   const int* child[MAXL + 1];   // [ncell] oct on the level above or -1 (levels < nl)
   const int* nbr[MAXL + 1];     // [nocts][6] cell of the level below next to the oct's parent cell in -x,+x,-y,+y,-z,+z,
                                 // or -1 - bc for a non-periodic box face (levels >= 1)
   const int* nbo[MAXL + 1];     // [nocts][6] derived for the static mesh: the oct of the SAME level behind each face of the
-                                // oct, -1 if that side is a coarser leaf, -2 - bc for a non-periodic box face (levels >= 1)
+                                // oct; -16 - s if that side is a coarser leaf (s = the side's record index); -2 - bc for a
+                                // non-periodic box face (levels >= 1)
   const unsigned int* hasdep[MAXL + 1];   // bitmap over the cells of a level: a leaf with a split face neighbour of its own
                                           // level, i.e. one that receives deposits (1 <= level < nl)
   float4 inflow[6][MAXG];
@@ -249,7 +254,7 @@ struct AmrDev {
 
 int launch_amr_transport(const AmrDev& A, int level, float nuh, float4* Unew, double dV, int hll, Partial* parts, int* n_parts,
                          cudaStream_t st);
-int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, float4* Unew, const int* slot_cell, const int* slot_coarse,
+int launch_amr_ghost_faces(const AmrDev& A, int level, float nuh, int sub, const int* slot_cell, const int* slot_coarse,
                            const unsigned char* slot_face, const int* slot_refs, int n_slots, int hll, cudaStream_t st);
 int launch_amr_chem(const ChemParams& cp, const LevelDev& L, const AmrDev& A, int level, int count_total, int limit,
                     Partial* parts, int* n_parts, cudaStream_t st);
