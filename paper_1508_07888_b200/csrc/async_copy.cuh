@@ -27,32 +27,25 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
 }
+// Wait for a phase.  `try_wait` with a suspend-time hint parks the thread in hardware until the phase completes (or the hint,
+// in ns, runs out) -- a waiting warp then costs one instruction per wake-up instead of a polling loop that takes issue slots
+// from the warps it is waiting for (profiles/r2a_summary.md: polls were 13 % of the fused pass's issued instructions).
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
   unsigned done;
   do {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
   } while (!done);
 }
-// the same with a short sleep between polls: for waits on other warps (not on data), where a spinning warp would only
-// take issue slots from the warps it is waiting for
+// waits on other warps (not on data): the same
 template <int SLEEP_NS = 64>
 __device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
 {
-  unsigned done;
-  for (;;) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    if (done) break;
-    __nanosleep(SLEEP_NS);
-  }
+  mbar_wait(bar, parity);
 }
 // one box of a rank-3 tensor -> shared memory, completion (bytes) on an mbarrier
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int cx, int cy, int cz)
