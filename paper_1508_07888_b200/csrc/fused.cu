@@ -190,9 +190,9 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
     }
   };
 
-  for (int j = 0; j < zc; j++) {
+  size_t cell = (size_t)z0 * plane + (act ? ((size_t)y * n + x) : 0);   // my cell of plane j: advanced by one plane per trip
+  for (int j = 0; j < zc; j++, cell += plane) {
     const int z = z0 + j;
-    const size_t cell = (size_t)z * plane + (act ? ((size_t)y * n + x) : 0);
     // chemistry inputs of my cell: in flight while the transport arithmetic runs
     float n0v = 1.f, xsv = 0.f, epsv = 1.f;
     unsigned srcw = 0;
