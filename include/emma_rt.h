@@ -31,7 +31,9 @@
  *     point that launches work makes the handle's device current (cudaSetDevice) and leaves it current.
  *   - Input validation: `emma_rt_init` and `emma_rt_write` with HOST buffers refuse (EMMA_RT_EINVAL) n0 <= 0, T <= 0,
  *     x outside [0, 1] and non-finite n0, x, T; a non-finite U is accepted and reported by the next step
- *     (EMMA_RT_ENONFINITE).  Device-buffer writes are stream-ordered and not validated (a NaN stays a NaN).
+ *     (EMMA_RT_ENONFINITE).  A refused write has still stored the field (x clamped to [0, 1]): write it again with valid
+ *     values, or discard the handle after a refused init.  Device-buffer writes are stream-ordered and not validated (a
+ *     NaN stays a NaN).
  *   - Environment: five tuning knobs for experiments are read ONCE, by `emma_rt_init`, and ignored when unset, not a
  *     number or out of range: EMMA_RT_TUNE_NZC (z-chunks per tile column of the dense passes, 1..n), EMMA_RT_TUNE_NST
  *     (stages of the transport TMA ring: 4, 6, 8), EMMA_RT_TUNE_TMA (0: non-TMA transport kernel), EMMA_RT_TUNE_FUSED
