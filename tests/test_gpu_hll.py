@@ -23,9 +23,12 @@ C_RED = 0.1 * CGS.c
 HLL = E.FLUX_HLL
 
 
-@pytest.mark.parametrize("n,G,bc", BCS + [(36, 4, (2, 1, 1, 2, 0, 0))])
+@pytest.mark.parametrize("n,G,bc", BCS + [(36, 4, (2, 1, 1, 2, 0, 0)), (32, 2, (2, 1, 0, 0, 1, 2)), (63, 1, (0,) * 6),
+                                          (31, 3, (1, 2, 2, 1, 0, 0)), (62, 1, (2, 2, 0, 0, 0, 0)), (17, 2, (0,) * 6)])
 def test_hll_transport_one_step(n, G, bc):
-    """One HLL transport step on a config-5b-like state (N over 5 decades, f in [0, 0.9]); north_star tolerance, A17 norms."""
+    """One HLL transport step on a config-5b-like state (N over 5 decades, f in [0, 0.9]); north_star tolerance, A17 norms.
+    The kernel's tiles are 31 cells wide and a thread owns two rows: n = 31, 62 (exact tiles), 32, 63 (a last tile ONE cell
+    wide), 33, 17 (an odd last row: the unpaired-row path), with open, reflective and periodic faces on the tile edges."""
     rng = np.random.default_rng(n * 10 + G + 7)
     w = tiny_workload(n, G, bc=bc, chemistry=0, U0=_random_U(rng, G, n ** 3, C_RED, fmax=0.9, lo=-7, hi=-2), courant=0.9)
     orc, gpu, _, diags = run_pair(w, 1, track_signatures=False, flux=HLL)
