@@ -667,7 +667,7 @@ int init_impl(emma_rt** out, const emma_rt_config* cfg, const emma_rt_amr* amr, 
   for (int b = 0; b < 2; b++) {
     const int r = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps[b]);
     if (r != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", r);
-    const int rh = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_h[b], 16, hll_tile_x());
+    const int rh = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_h[b], 16, hll_tile_x(), hll_main_x());
     if (rh != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", rh);
     const int rf = make_transport_maps(h->U(b), s.n, s.G, &h->tmaps_f[b], fused_tile_y());
     if (rf != 0) return fail(h, EMMA_RT_ECUDA, "cuTensorMapEncodeTiled failed (%d)", rf);

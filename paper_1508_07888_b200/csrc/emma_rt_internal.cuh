@@ -126,7 +126,7 @@ struct Profiler {
 // ---- launchers (each returns the number of kernels it launched) ---------------------------------------------
 int launch_transport(const TransportParams& p, const float4* Uin, float4* Uout, Partial* parts, int* n_parts,
                      cudaStream_t st);
-int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int tile_y = 16, int tile_x = 32);
+int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int tile_y = 16, int tile_x = 32, int main_x = 0);
 int launch_transport_tma(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st);
 int launch_chem_level0(const ChemParams& cp, const LevelDev& L0, float4* U, long long ncell, int* queue,
@@ -148,6 +148,7 @@ int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in,
                          int* n_parts, cudaStream_t st);
 int hll_ctas_per_sm();
 int hll_tile_x();
+int hll_main_x();
 int launch_chem_refined(const ChemParams& cp, const LevelDev* lv, int level, int n_levels, float4* U,
                         long long ncell0, const CrtaQueue& q, Partial* parts, int* n_parts, int sm_count, cudaStream_t st);
 int launch_inject_sources(const LevelDev& L0, int G, float dt, float4* U, long long ncell0, Partial* parts,

@@ -38,11 +38,15 @@ using namespace acp;
 
 constexpr int TXC = 31;                        // cells per tile row that this CTA updates (lanes 1..31)
 constexpr int TY = 16, NW = TY / 2, NT = 32 * NW;
-constexpr int ROWB = TXC * 16;                 // bytes of one row of the main box (dense: what the TMA delivers)
+constexpr int TXM = TXC + 2;                   // the main box also brings the x halo: cells x0-1 .. x0+31, cell x0+l-1 in slot l
+constexpr int ROWB = TXM * 16;                 // bytes of one row of the main box (dense: what the TMA delivers)
 constexpr int COLB = TY * 16;                  // bytes of one halo column
-// one plane: [MAIN 16 x 31][BOT 31][TOP 31][LCOL 16][RCOL 16] cells, every box at a 128-byte aligned offset (TMA)
+// One plane: [MAIN 16 x 33][BOT 31][TOP 31][LCOL 16][RCOL 16] cells, every box at a 128-byte aligned offset (TMA).  With the
+// x halo inside the rows a quarter-warp reads 128 contiguous bytes (any 16-byte phase): no bank conflict; a halo taken from
+// a separate column box costs one more wavefront per load (profiles/r2e_hll_summary.md: 29 % of the shared-memory
+// wavefronts).  LCOL / RCOL are read only by the tiles on a box face, where the halo is a periodic image or a ghost.
 constexpr int MAIN = 0, BOT = TY * ROWB, TOP = BOT + 512, LCOL = TOP + 512, RCOL = LCOL + COLB;
-constexpr int SG = RCOL + COLB;                // bytes of one plane (9472 = 74 x 128)
+constexpr int SG = RCOL + COLB;                // bytes of one plane (9984 = 78 x 128)
 static_assert(BOT % 128 == 0 && SG % 128 == 0, "TMA destinations must be 128-byte aligned");
 constexpr int NST = 6;                         // stages of the ring
 constexpr int AUXB = 2 * SG;                   // aux plane: two sub-planes of one float4 per cell, each laid out like a stage
@@ -90,15 +94,17 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
   const bool act0 = col && r0 < wy, act1 = col && pair;
   const bool ghostL = BCGEN && lane == 0 && x0 == 0 && p.bc[0] != EMMA_RT_BC_PERIODIC;   // my cells are ghosts of the -x face
 
-  // byte offsets inside a plane
-  const int c16 = (lane - 1) * 16;
-  const int own0 = (lane == 0) ? LCOL + r0 * 16 : MAIN + r0 * ROWB + c16;
-  const int own1 = (lane == 0) ? LCOL + (r0 + 1) * 16 : own0 + ROWB;
-  const int oxp0 = (lane == 0) ? MAIN + r0 * ROWB : (lane >= wx) ? RCOL + r0 * 16 : own0 + 16;
-  const int oxp1 = (lane == 0) ? MAIN + (r0 + 1) * ROWB : (lane >= wx) ? RCOL + (r0 + 1) * 16 : own1 + 16;
-  const int cc = (lane == 0) ? 0 : c16;        // lane 0 needs no y faces: any valid column
-  const int oym0 = (r0 == 0) ? BOT + cc : MAIN + (r0 - 1) * ROWB + cc;
-  const int oyp = (r0 + (pair ? 2 : 1) < wy) ? MAIN + (r0 + 2) * ROWB + cc : TOP + cc;   // above my upper cell
+  // byte offsets inside a plane.  edgeL / edgeR: the tile touches the -x / +x face of the box, its halo there is not the
+  // neighbour in memory (periodic image, ghost; also the ragged last tile): it comes from the column boxes
+  const bool edgeL = x0 == 0, edgeR = x0 + wx == n;
+  const int c16 = lane * 16;
+  const int own0 = (lane == 0 && edgeL) ? LCOL + r0 * 16 : MAIN + r0 * ROWB + c16;
+  const int own1 = (lane == 0 && edgeL) ? LCOL + (r0 + 1) * 16 : MAIN + (r0 + 1) * ROWB + c16;
+  const int oxp0 = (lane >= wx && edgeR) ? RCOL + r0 * 16 : MAIN + r0 * ROWB + c16 + 16;
+  const int oxp1 = (lane >= wx && edgeR) ? RCOL + (r0 + 1) * 16 : MAIN + (r0 + 1) * ROWB + c16 + 16;
+  const int cl = (lane == 0) ? 1 : lane;       // lane 0 needs no y faces: any valid column
+  const int oym0 = (r0 == 0) ? BOT + (cl - 1) * 16 : MAIN + (r0 - 1) * ROWB + cl * 16;
+  const int oyp = (r0 + (pair ? 2 : 1) < wy) ? MAIN + (r0 + 2) * ROWB + cl * 16 : TOP + (cl - 1) * 16;   // above my upper cell
   float sxp = 1.f, sym = 1.f, syp = 1.f;       // reflective faces: sign of the face-normal flux of that neighbour (A13)
   if (BCGEN) {
     if (lane == wx && x0 + wx == n && p.bc[1] == EMMA_RT_BC_REFLECTIVE) sxp = -1.f;
@@ -123,7 +129,7 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     const int nh = wy + 2 * wx, h = t;
     if (h < nh) {
       int face;
-      if (h < wy) { hoff = RCOL + h * 16; face = (x0 + wx == n) ? 1 : -1; }
+      if (h < wy) { hoff = edgeR ? RCOL + h * 16 : MAIN + h * ROWB + (TXC + 1) * 16; face = edgeR ? 1 : -1; }
       else if (h < wy + wx) { hoff = BOT + (h - wy) * 16; face = (y0 == 0) ? 2 : -1; }
       else { hoff = TOP + (h - wy - wx) * 16; face = (y0 + wy == n) ? 3 : -1; }
       if (BCGEN && face >= 0) {
@@ -147,9 +153,9 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
     if (lane != 0 || warp >= 5) return;
     const int zg = g * n + ((j < 0) ? zm : (j >= zc) ? ztop : z0 + j);
     const unsigned bar = bar0 + 8 * s, dst = stage0 + s * SG;
-    if (warp == 0) { mbar_expect_tx(bar, TY * ROWB); tma_load_3d(dst + MAIN, &maps.main, bar, 4 * x0, y0, zg); }
-    else if (warp == 1) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst + BOT, &maps.row, bar, 4 * x0, cyb, zg); }
-    else if (warp == 2) { mbar_expect_tx(bar, ROWB); tma_load_3d(dst + TOP, &maps.row, bar, 4 * x0, cyt, zg); }
+    if (warp == 0) { mbar_expect_tx(bar, TY * ROWB); tma_load_3d(dst + MAIN, &maps.main, bar, 4 * (x0 - 1), y0, zg); }
+    else if (warp == 1) { mbar_expect_tx(bar, TXC * 16); tma_load_3d(dst + BOT, &maps.row, bar, 4 * x0, cyb, zg); }
+    else if (warp == 2) { mbar_expect_tx(bar, TXC * 16); tma_load_3d(dst + TOP, &maps.row, bar, 4 * x0, cyt, zg); }
     else if (warp == 3) { mbar_expect_tx(bar, COLB); tma_load_3d(dst + LCOL, &maps.col, bar, cxl, y0, zg); }
     else { mbar_expect_tx(bar, COLB); tma_load_3d(dst + RCOL, &maps.col, bar, cxr, y0, zg); }
   };
@@ -267,11 +273,14 @@ transport_hll_kernel(const TransportParams p, const __grid_constant__ TransportM
 
     auto update = [&](const float4& cu, const float4& Hxm, const float4& Hxp, const float4& Hym, const float4& Hyp,
                       const float4& Hzm, const float4& Hzp) -> float4 {
-      float4 o;                                                        // Eq. 30, unsplit (A4)
-      o.x = fmaf(-nu, (Hxp.x - Hxm.x) + (Hyp.x - Hym.x) + (Hzp.x - Hzm.x), cu.x);
-      o.y = fmaf(-nu, (Hxp.y - Hxm.y) + (Hyp.y - Hym.y) + (Hzp.y - Hzm.y), cu.y);
-      o.z = fmaf(-nu, (Hxp.z - Hxm.z) + (Hyp.z - Hym.z) + (Hzp.z - Hzm.z), cu.z);
-      o.w = fmaf(-nu, (Hxp.w - Hxm.w) + (Hyp.w - Hym.w) + (Hzp.w - Hzm.w), cu.w);
+      // Eq. 30, unsplit (A4): o = cu - nu [(Hxp - Hxm) + (Hyp - Hym) + (Hzp - Hzm)], on the (N, phi_x) and (phi_y, phi_z) halves
+      float4 o, dx, dy, dz;
+      sub2(dx.x, dx.y, Hxp.x, Hxp.y, Hxm.x, Hxm.y); sub2(dx.z, dx.w, Hxp.z, Hxp.w, Hxm.z, Hxm.w);
+      sub2(dy.x, dy.y, Hyp.x, Hyp.y, Hym.x, Hym.y); sub2(dy.z, dy.w, Hyp.z, Hyp.w, Hym.z, Hym.w);
+      sub2(dz.x, dz.y, Hzp.x, Hzp.y, Hzm.x, Hzm.y); sub2(dz.z, dz.w, Hzp.z, Hzp.w, Hzm.z, Hzm.w);
+      fma2(dx.x, dx.y, dx.x, dx.y, 1.f, 1.f, dy.x, dy.y); fma2(dx.z, dx.w, dx.z, dx.w, 1.f, 1.f, dy.z, dy.w);
+      fma2(dx.x, dx.y, dx.x, dx.y, 1.f, 1.f, dz.x, dz.y); fma2(dx.z, dx.w, dx.z, dx.w, 1.f, 1.f, dz.z, dz.w);
+      fma2(o.x, o.y, dx.x, dx.y, -nu, -nu, cu.x, cu.y); fma2(o.z, o.w, dx.z, dx.w, -nu, -nu, cu.z, cu.w);
       // A19: keep the state realizable, |phi| <= max(N, 0)
       const float p2 = fmaf(o.y, o.y, fmaf(o.z, o.z, o.w * o.w)), Np = fmaxf(o.x, 0.f);
       if (p2 > Np * Np) { const float sc = Np * rsqrtf(p2); o.y *= sc; o.z *= sc; o.w *= sc; }
@@ -348,6 +357,7 @@ cudaError_t configure_transport_hll()
 
 int hll_ctas_per_sm() { return 2; }
 int hll_tile_x() { return TXC; }
+int hll_main_x() { return TXM; }
 
 int launch_transport_hll(const TransportParams& p, const TransportMaps& maps_in, float4* Uout, Partial* parts,
                          int* n_parts, cudaStream_t st)

@@ -336,15 +336,16 @@ cudaError_t configure_transport_tma()
 }
 
 // Tensor maps of one radiation buffer U[G][n][n][n] float4, seen as a rank-3 fp32 tensor (4n, n, G n).
+// `main_x` > 0: the main box is that many cells wide (a kernel whose rows carry their x halo), the row box stays tile_x wide.
 // Returns 0 on success, the CUresult (or -1 when the driver entry point is missing) otherwise.
-int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int tile_y, int tile_x)
+int make_transport_maps(const float4* U, int n, int G, TransportMaps* out, int tile_y, int tile_x, int main_x)
 {
   EncodeTiledFn enc = encode_tiled();
   if (!enc) return -1;
   const cuuint64_t gdim[3] = {(cuuint64_t)4 * n, (cuuint64_t)n, (cuuint64_t)n * G};
   const cuuint64_t gstr[2] = {(cuuint64_t)16 * n, (cuuint64_t)16 * n * n};
   const cuuint32_t estr[3] = {1, 1, 1};
-  const cuuint32_t box_main[3] = {4 * (cuuint32_t)tile_x, (cuuint32_t)tile_y, 1}, box_row[3] = {4 * (cuuint32_t)tile_x, 1, 1}, box_col[3] = {4, (cuuint32_t)tile_y, 1};
+  const cuuint32_t box_main[3] = {4 * (cuuint32_t)(main_x > 0 ? main_x : tile_x), (cuuint32_t)tile_y, 1}, box_row[3] = {4 * (cuuint32_t)tile_x, 1, 1}, box_col[3] = {4, (cuuint32_t)tile_y, 1};
   CUresult r;
   r = enc(&out->main, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)U, gdim, gstr, box_main, estr,
           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
