@@ -190,8 +190,11 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
     }
   };
 
-  size_t cell = (size_t)z0 * plane + (act ? ((size_t)y * n + x) : 0);   // my cell of plane j: advanced by one plane per trip
-  for (int j = 0; j < zc; j++, cell += plane) {
+  // my cell of plane j, advanced by one plane per trip: 32 bits (n <= 1290, checked at init), so that an array element's
+  // address is one IMAD.WIDE
+  const unsigned plane32 = (unsigned)n * (unsigned)n;
+  unsigned cell = (unsigned)z0 * plane32 + (act ? (unsigned)y * (unsigned)n + (unsigned)x : 0u);
+  for (int j = 0; j < zc; j++, cell += plane32) {
     const int z = z0 + j;
     // chemistry inputs of my cell: in flight while the transport arithmetic runs
     float n0v = 1.f, xsv = 0.f, epsv = 1.f;
@@ -311,13 +314,12 @@ fused_kernel(const TransportParams p, const __grid_constant__ TransportMaps maps
         store_cell<G>(L, (long long)cell, Uout, (long long)ncell, c, tl, cp.record);
         t_abs += (double)tl.absorbed;
         t_tot += (double)sumN;
-        if ((srcw >> (cell & 31)) & 1u) {
-          float inj = 0.f;
+        // S is 0 outside source cells and r.rec is 0 with OTSA: adding +0.0 leaves the sums as they are, without the predicates
+        float inj = 0.f;
 #pragma unroll
-          for (int g = 0; g < G; g++) inj = fmaf(c.S[g], cp.dt, inj);
-          t_inj += (double)inj;
-        }
-        if (!cp.otsa) t_rec += (double)(r.rec * cp.dt);
+        for (int g = 0; g < G; g++) inj = fmaf(c.S[g], cp.dt, inj);
+        t_inj += (double)inj;
+        t_rec += (double)(r.rec * cp.dt);
         n_fast++;
         acc_d.dtau_min = fminf(acc_d.dtau_min, dmin);
         if (!finite_cell<G>(c)) acc_d.nonfinite++;
