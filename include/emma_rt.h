@@ -225,6 +225,32 @@ EMMA_RT_API int emma_rt_set_flux(emma_rt* h, int32_t flux);
 EMMA_RT_API const char* emma_rt_last_error(const emma_rt* h);                  /* handle-owned; "" if none                   */
 EMMA_RT_API void emma_rt_free(emma_rt* h);                                     /* does not free the arena                    */
 
+/* ---- the one entry point that allocates nothing ------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it)
+ * and so cannot create a handle, whose arena is where every other kernel keeps its scratch.
+ *
+ * Photon total of A15 (emma_rt_diag.photons_total, Eq. 30 conserves it up to sources and sinks):
+ *     *total_dev = dV * sum_{i < n_cellgroups} U_dev[i].N
+ * -- the same kernels, grid and summation order as the state query emma_rt_step(h, dt, 0, &diag), hence the same bits.
+ *   U_dev         DEVICE pointer, borrowed: n_cellgroups x (N, Fx, Fy, Fz) float, 16-byte aligned -- the layout of
+ *                 EMMA_RT_FIELD_U, the groups of a level one after the other (only N is read); may be NULL if n = 0
+ *   n_cellgroups  cells x groups, 0 .. EMMA_RT_NOALLOC_MAX_CELLGROUPS (2^33: the largest grid emma_rt_init accepts,
+ *                 1290^3 x 4 groups, fits); beyond that EMMA_RT_EINVAL and nothing is launched: sum the array in pieces
+ *   dV            cell volume [cm^3], positive and finite
+ *   total_dev     DEVICE pointer to one double, written by the second kernel (stream-ordered; the call does not wait)
+ *   stream        cudaStream_t of the caller, borrowed; 0 = default stream
+ *   err, err_len  optional HOST buffer for the error text ("" on success); may be NULL
+ * Returns EMMA_RT_OK, EMMA_RT_EINVAL (bad argument, size beyond the maximum) or EMMA_RT_ECUDA.  Calls no cudaMalloc /
+ * cudaFree / allocating routine, synchronises nothing, and launches two kernels on `stream`.  The scratch (1024 block sums,
+ * 88 KB) is a static device array that every GPU which loads the library holds until the process exits; its device
+ * address is looked up (cudaGetSymbolAddress) in the first call on each device, with the caller's current device -- make
+ * that first call (n_cellgroups = 0 will do) outside graph capture.  ALL calls share the scratch: calls on one stream are
+ * safe (every slot a call reads it has written itself: nothing is carried over from the last call), calls that overlap on
+ * the GPU (several streams, concurrent graph replays) race. */
+#define EMMA_RT_NOALLOC_MAX_CELLGROUPS (1ll << 33)
+EMMA_RT_API int emma_rt_photons_total_noalloc(const void* U_dev, int64_t n_cellgroups, double dV, double* total_dev,
+                                              void* stream, char* err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

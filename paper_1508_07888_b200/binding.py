@@ -18,7 +18,9 @@ _FIELD_SHAPE = {FIELD_U: (4, np.float32), FIELD_F: (3, np.float32), FIELD_SUBCYC
 
 EXPORTED_SYMBOLS = ["emma_rt_arena_bytes", "emma_rt_init", "emma_rt_set_sources", "emma_rt_dt_cfl", "emma_rt_step",
                     "emma_rt_step_host", "emma_rt_read", "emma_rt_write", "emma_rt_level_cells", "emma_rt_kernel_launches",
-                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_set_inflow", "emma_rt_last_error", "emma_rt_free"]
+                    "emma_rt_profile", "emma_rt_set_schedule", "emma_rt_set_flux", "emma_rt_set_inflow", "emma_rt_last_error", "emma_rt_free",
+                    "emma_rt_photons_total_noalloc"]
+NOALLOC_MAX_CELLGROUPS = 1 << 33              # EMMA_RT_NOALLOC_MAX_CELLGROUPS
 FLUX_GLF, FLUX_HLL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
 KERNEL_KINDS = ["transport", "chem_main", "chem_tail", "chem_refined", "finalize", "other", "fused", "amr_transport", "amr_chem"]
@@ -110,6 +112,8 @@ def lib():
     L.emma_rt_set_flux.argtypes = [C.c_void_p, C.c_int32]
     L.emma_rt_last_error.restype = C.c_char_p
     L.emma_rt_last_error.argtypes = [C.c_void_p]
+    L.emma_rt_photons_total_noalloc.restype = C.c_int
+    L.emma_rt_photons_total_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]
     L.emma_rt_free.restype = None
     L.emma_rt_free.argtypes = [C.c_void_p]
     _lib = L
@@ -205,6 +209,15 @@ def emma_rt_write(h, field, level, group, src_ptr, nbytes, src_is_device):
 
 def emma_rt_free(h):
     lib().emma_rt_free(h)
+
+
+def emma_rt_photons_total_noalloc(U_dev_ptr, n_cellgroups, dV, total_dev_ptr, stream=0):
+    """dV * sum of N over n_cellgroups (N, Fx, Fy, Fz) float records at the DEVICE address U_dev_ptr -> the double at the DEVICE
+    address total_dev_ptr, stream-ordered, without any allocation (include/emma_rt.h).  Returns (rc, error text)."""
+    err = C.create_string_buffer(256)
+    rc = lib().emma_rt_photons_total_noalloc(C.c_void_p(U_dev_ptr), int(n_cellgroups), float(dV), C.c_void_p(total_dev_ptr),
+                                             C.c_void_p(stream), err, len(err))
+    return rc, err.value.decode()
 
 
 # ---- convenience wrapper ---------------------------------------------------------------------------------------

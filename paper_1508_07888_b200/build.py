@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libemma_rt.so")
-SOURCES = ["api.cu", "amr.cu", "transport.cu", "transport_tma.cu", "transport_hll.cu", "chemistry.cu", "fused.cu", "util.cu"]
+SOURCES = ["api.cu", "amr.cu", "transport.cu", "transport_tma.cu", "transport_hll.cu", "chemistry.cu", "fused.cu", "util.cu", "noalloc.cu"]
 import glob
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(INC, "*.h")))     # every header is a dependency
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
