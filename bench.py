@@ -30,6 +30,7 @@ METRIC = "cell_group_updates_per_s"
 UNIT = "cell-group updates/s"
 ORACLE_SAMPLE_N = 128             # the oracle's bounded sample of config 5: 128^3 x 3 groups (0.3 s per step on 16 cores)
 ORACLE_SAMPLE_STEPS = 30          # at most this many timed steps (~10 s of host time), after the same warm-up as the GPU arm
+REFERENCE_MAX_STEPS = 300         # --impl reference times exactly K steps up to this many (a few minutes of host time)
 ORACLE_1T_N = 64                  # single-thread figure ("one GPU against one CPU core"): 64^3 x 3 groups
 ORACLE_1T_STEPS = 8
 
@@ -185,8 +186,9 @@ def run_reference(args):
         return
     n = ORACLE_SAMPLE_N if args.config == 5 else 96
     # per "step" of this arm: one oracle step on the n^3 sample, timed over the SAME step range as the GPU arm (W untimed
-    # warm-up steps from the seeded initial state, then K timed steps, K capped so the run stays within a few minutes)
-    steps, warm = max(1, min(args.steps, ORACLE_SAMPLE_STEPS)), max(0, args.warmup)
+    # warm-up steps from the seeded initial state, then EXACTLY K timed steps: ~0.3-0.8 s each on 8-16 cores, so the default
+    # K = 50 takes under a minute; only a K beyond REFERENCE_MAX_STEPS is cut, and the line then says so)
+    steps, warm = max(1, min(args.steps, REFERENCE_MAX_STEPS)), max(0, args.warmup)
     val, secs, cores, d = time_oracle(n, steps, warm, args.variant, args.config)
     label = ("5" + args.variant) if args.config == 5 else "4 (CRTA, 2 refined levels)"
     sample = ("config %s recipe at %d^3 x 3 groups (a bounded sample of the full grid), steps %d..%d from the seeded initial state, "
@@ -194,7 +196,11 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE config %s sampled at %d^3 (oracle on host cores)" % (label, n)},
+            "config": {"workload": ("BASELINE config %s: %d^3 x 3 groups, coupled RT+chemistry, timed after %d warm-up steps (the GPU arm's "
+                                    "workload); each step of this arm is a bounded sample of it: the same recipe at %d^3, oracle on host cores"
+                                    % (label, args.n if args.config == 5 else 256, warm, n)),
+                       "n_coarse": args.n if args.config == 5 else 256, "groups": 3, "sample_n_coarse": n,
+                       "steps_requested": args.steps},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                              "cpu_model": cpu_model(), "step_range": [warm + 1, warm + steps],
                              "subcycles_mean_last_step": d["subcycles_total"] / float(n ** 3) if args.config == 5 else None},
