@@ -864,7 +864,8 @@ int step_impl(emma_rt* h, double dt, int32_t n_steps, emma_rt_diag* diag_last)
       const double cost = (double)((blocks + slots - 1) / slots) * (zc + 3);
       if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = nzc; }
     }
-    if (env_nzc > 0 && env_nzc <= s.n) best = env_nzc;
+    // the override applies to every dense pass whose partial-sum slots it fits (a pass that is not even used must not refuse the step)
+    if (env_nzc > 0 && env_nzc <= s.n && (long long)per * env_nzc <= TRANSPORT_MAX_BLOCKS) best = env_nzc;
     q.zchunk = (s.n + best - 1) / best;
     q.nzc = (s.n + q.zchunk - 1) / q.zchunk;
     return (long long)per * q.nzc <= TRANSPORT_MAX_BLOCKS;
