@@ -35,7 +35,8 @@
  *     values, or discard the handle after a refused init.  Device-buffer writes are stream-ordered and not validated (a
  *     NaN stays a NaN).
  *   - Environment: five tuning knobs for experiments are read ONCE, by `emma_rt_init`, and ignored when unset, not a
- *     number or out of range: EMMA_RT_TUNE_NZC (z-chunks per tile column of the dense passes, 1..n), EMMA_RT_TUNE_NST
+ *     number or out of range: EMMA_RT_TUNE_NZC (z-chunks per tile column of the dense passes, 1..n; a pass whose
+ *     partial-sum slots that count would overflow keeps its own choice), EMMA_RT_TUNE_NST
  *     (stages of the transport TMA ring: 4, 6, 8), EMMA_RT_TUNE_TMA (0: non-TMA transport kernel), EMMA_RT_TUNE_FUSED
  *     (0: two-pass schedule), EMMA_RT_TUNE_CHEMCTAS (persistent CTAs per SM of the chemistry main pass, 1..32).  None
  *     changes results beyond fp32 rounding order of nothing (same arithmetic); `emma_rt_step` reads no environment.
