@@ -123,3 +123,25 @@ def test_hll_config1_stromgren_60_steps():
     assert rep["flips"] <= max(1, 1e-4 * rep["cells"]), rep
     assert rep["x"] <= TOL_XT and rep["T"] <= TOL_XT, rep
     assert worst <= TOL_BUDGET, worst
+
+
+def test_hll_config5_recipe_64_20_coupled_steps_whole_grid():
+    """The metric's workload shape (config 5b recipe: lognormal density, random x, T, 3 groups, many sources) at 64^3 with the
+    HLL flux for 20 coupled steps, every cell against the oracle with the flip protocol: the two-pass schedule around
+    transport_hll_kernel (2 x 3 tiles of 31 cells, a ragged 2-cell tile, 4 tile rows) through the sub-cycling transient."""
+    w = make_config(5, n=64, variant="b")
+    orc, gpu, flips, diags = run_pair(w, 20, flux=HLL)
+    rep = compare(orc, gpu, w, flips, 20, radius=4)
+    prev, worst = None, 0.0
+    for do, dg in diags:
+        if prev is not None:
+            worst = max(worst, budget_residual(dg, prev))
+        prev = dg["photons_total"]
+        assert dg["n_nonfinite"] == 0
+    print("HLL config 5b 64^3 x 20 steps", {k: (float("%.3g" % v) if isinstance(v, float) else v) for k, v in rep.items()})
+    assert diags[0][1]["subcycles_max"] > 10 and diags[0][1]["n_deferred"] > 1000       # the random T state sub-cycles hard
+    assert rep["flips"] <= max(2, 1e-3 * rep["cells"]), rep
+    assert rep["x"] <= TOL_XT and rep["T"] <= TOL_XT, rep
+    assert worst <= TOL_BUDGET, worst
+    do, dg = diags[-1]
+    assert abs(dg["photons_total"] - do["photons_total"]) <= 1e-5 * abs(do["photons_total"])

@@ -103,3 +103,33 @@ def test_step_host_refusals():
     rc, _ = gpu.step_host(w.dt, U, x, T)
     assert rc == E.ESTATE
     gpu.close()
+
+
+def test_step_host_256_many_slabs_bit_equal():
+    """At size: 256^3 x 3 groups (0.8 GB of radiation each way per step) goes through the device in 32 slabs of 8 planes on
+    three streams; two steps in place on pinned host tensors must leave the same bits as write -> step -> read."""
+    import torch
+    w = make_config(5, n=256, variant="b")
+    ref = E.EmmaRT(w)
+    gpu = E.EmmaRT(w)
+    U = [torch.from_numpy(np.ascontiguousarray(w.U0[g], np.float32).copy()).pin_memory() for g in range(w.G)]
+    x = torch.from_numpy(w.x[0].copy()).pin_memory()
+    T = torch.from_numpy(w.T[0].copy()).pin_memory()
+    for step in range(2):
+        rc, d = gpu.step_host(w.dt, U, x, T)
+        assert rc == E.OK, gpu.last_error()
+        rcr, dr = ref.step(w.dt, 1)
+        assert rcr == E.OK
+        Ur = [ref.read(E.FIELD_U, 0, g) for g in range(w.G)]
+        xr, Tr = ref.read(E.FIELD_X), ref.read(E.FIELD_T)
+        for g in range(w.G):
+            assert ref.write(E.FIELD_U, 0, g, Ur[g]) == E.OK          # the reference's next step starts from the host values too
+        assert ref.write(E.FIELD_X, 0, 0, xr) == E.OK and ref.write(E.FIELD_T, 0, 0, Tr) == E.OK
+        for g in range(w.G):
+            assert np.array_equal(U[g].numpy(), Ur[g]), (step, g)
+        assert np.array_equal(x.numpy(), xr) and np.array_equal(T.numpy(), Tr)
+        assert d["subcycles_total"] == dr["subcycles_total"] and d["n_deferred"] == dr["n_deferred"]
+        assert abs(d["photons_total"] - dr["photons_total"]) <= 1e-12 * dr["photons_total"]
+    assert d["subcycles_max"] > 1                                        # the random initial T: the tail kernel ran on slabs too
+    gpu.close()
+    ref.close()
